@@ -1,0 +1,180 @@
+/*
+ * petar.h -- C ABI of the B200-native long-range P3T force path of PeTar (arxiv 2006.16560).
+ *
+ * What the library computes (citations are PAPER.md:<line>):
+ *   For N particles with masses m_i, positions and individual changeover radii r_out,i
+ *   (Eq. 12, :226-231), an opening angle theta (:207) and a multipole order (:645):
+ *     - the LONG-range acceleration and specific potential of H_L (Eq. 11, :184-187), i.e.
+ *       Barnes-Hut tree gravity in which every particle-particle pair is weighted by the paper's
+ *       changeover functions, force weight 1-K(x) (Eq. 17, :265) and potential weight 1-W(x)
+ *       (Eq. 15, :247), x and Lambda from the pairwise maxima of the radii (Eq. 16, :252-261);
+ *     - the neighbour list { j != i : r_ij < max(r_search,i, r_search,j) } that hands particles
+ *       to the short-range integrators (:209, :347; r_search = r_out on this path, the
+ *       velocity-dependent radius of Eq. 24, :341, can be passed through r_search).
+ *
+ * Conventions
+ *   - Every array pointer is a DEVICE pointer (CUDA global memory of the current device) unless the
+ *     parameter comment says HOST.  All particle arrays are SoA, length N, fp64, caller's order.
+ *   - The caller owns every input, every output and the workspace; the library never allocates
+ *     device memory.  Inputs are read-only and must stay alive (and unmodified) until the stream
+ *     has passed the last call that uses the tree.  The tree handle is a small host object that
+ *     points into the workspace; it dies with petar_tree_destroy or with the workspace.
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
+ *     enqueued on it; calls return without synchronising unless a HOST output is requested.
+ *   - Return value: 0 = PETAR_OK, negative = error (below).  No exceptions, no exit(), no stdout.
+ *     Data-dependent failures found on the device (non-finite input, node/list/neighbour capacity
+ *     exceeded) are recorded in a device status word, see petar_tree_status.
+ */
+#ifndef PETAR_H_
+#define PETAR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PETAR_OK 0
+#define PETAR_EINVAL (-1)     /* bad N / params / NULL pointer                                   */
+#define PETAR_EWORKSPACE (-2) /* workspace too small or misaligned (needs 256-byte alignment)     */
+#define PETAR_ECUDA (-3)      /* CUDA launch/runtime error; petar_strerror gives the CUDA text    */
+#define PETAR_ENOTBUILT (-4)  /* handle is NULL, destroyed, or no tree has been built into it     */
+#define PETAR_ESTATUS (-5)    /* device status word is non-zero (returned only by calls that sync) */
+
+/* bits of the device status word */
+#define PETAR_ST_NONFINITE 1     /* a position, mass or radius is NaN/Inf, or a radius is <= 0     */
+#define PETAR_ST_NODE_CAP 2      /* more tree nodes than the workspace was sized for               */
+#define PETAR_ST_LIST_CAP 4      /* interaction-list arena exhausted (lists truncated)             */
+#define PETAR_ST_STACK 8         /* walk frontier overflow (never expected)                        */
+#define PETAR_ST_NB_CAP 16       /* neighbour indices did not fit `capacity`                       */
+
+typedef struct petar_tree petar_tree; /* opaque */
+
+typedef struct {
+    double G;               /* gravitational constant; 1.0 in Henon units (:580, :625)              */
+    double theta;           /* opening angle (:207); 0 => every leaf opened => direct summation     */
+    double r_in_over_r_out; /* r_in/r_out, in (0,1); the paper fixes 0.1 (:650)                     */
+    int32_t multipole;      /* 1 = monopole, 2 = quadrupole super-particles (:645)                  */
+    int32_t n_leaf_limit;   /* leaf capacity of the octree, 1..64 (8)                               */
+    int32_t n_group_limit;  /* i-group capacity, n_leaf_limit..64 (64)                              */
+    int32_t flags;          /* reserved, must be 0                                                  */
+    double list_entries_per_particle; /* sizing of the interaction-list arena in 4-byte entries per
+                               particle; <= 0 selects the default (see petar_workspace_bytes)       */
+} petar_params;
+
+/* Interaction counters (HOST struct).  Self pairs are counted in n_epep, as in rule O7.            */
+typedef struct {
+    int64_t n_groups, n_nodes;
+    int64_t n_epep;         /* sum over groups n_i * n_ep   (particle-particle interactions)        */
+    int64_t n_epsp;         /* sum over groups n_i * n_sp   (particle-cell interactions)            */
+    int64_t n_epep_near;    /* part of n_epep that went through the changeover polynomials          */
+    int64_t n_ep_list;      /* sum over groups of EP leaf ranges                                    */
+    int64_t n_sp_list;      /* sum over groups of accepted cells                                    */
+    int64_t list_entries_used; /* 4-byte arena entries used                                         */
+} petar_counts;
+
+/* HOST-only query: bytes of device workspace petar_tree_build needs for N particles.
+ * Returns 0 if N < 0 or the parameters are invalid.  Sized for: sorted copies of the inputs, keys,
+ * the node table (capacity N + 4096 nodes for n_leaf_limit >= 4, else 3N + 4096), group table and
+ * the list arena (default 1024 entries per particle, at least 16 Mi entries).                        */
+size_t petar_workspace_bytes(int64_t N, const petar_params* p /* HOST */);
+
+/* Steps S0-S6 of the path: bounding cube, 63-bit Morton keys, stable radix sort, sorted SoA copies,
+ * octree (leaf iff count <= n_leaf_limit or level 21), bottom-up monopole/quadrupole moments with
+ * tight boxes, i-groups (tree cells with <= n_group_limit members).  The paper delegates this to
+ * FDPS (:195, :615); the rules are DESIGN.md's readings O1-O6.
+ *   x,y,z,m,r_out : DEVICE fp64[N]; r_out > 0.   r_search: DEVICE fp64[N] or NULL (=> r_out);
+ *                   must be >= r_out elementwise if given.
+ *   workspace     : DEVICE, 256-byte aligned, >= petar_workspace_bytes(N,p) bytes.
+ *   tree_out      : HOST, receives the handle (also for N == 0).
+ * Errors: PETAR_EINVAL, PETAR_EWORKSPACE, PETAR_ECUDA.                                              */
+int petar_tree_build(const double* x, const double* y, const double* z, const double* m,
+                     const double* r_out, const double* r_search, int64_t N,
+                     const petar_params* p /* HOST */, void* workspace, size_t workspace_bytes,
+                     void* cuda_stream, petar_tree** tree_out /* HOST */);
+
+/* Steps S7-S8: per-group interaction-list walk (cell forced open when its box comes within
+ * max(rmax_group, rmax_cell) of the group's box, else accepted iff edge < theta * distance, rule O7)
+ * and the fp32 pairwise force + potential kernel (rule O8) with the changeover weights (Eq. 15-17).
+ *   acc_x, acc_y, acc_z, pot : DEVICE fp64[N], caller's particle order; pot is the specific
+ *                              long-range potential phi_L,i (negative).  Any may be NULL (skipped).
+ *   counts_host_or_null      : HOST; if non-NULL the call synchronises the stream and fills it, and
+ *                              returns PETAR_ESTATUS if the device status word is non-zero.
+ * Errors: PETAR_ENOTBUILT, PETAR_ECUDA, PETAR_ESTATUS.                                              */
+int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_y, double* acc_z, double* pot,
+                           petar_counts* counts_host_or_null, void* cuda_stream);
+
+/* Step S9: compacted neighbour list in CSR form, caller's particle indices (rule O9, fp64 test
+ * r2 < R_ij^2 with R_ij = max(r_search,i, r_search,j), strict).
+ *   offsets    : DEVICE int64[N+1]; always written; offsets[N] = total number of neighbours.
+ *   indices    : DEVICE int32[capacity] or NULL.  NULL => only offsets (count + scan) are written;
+ *                the caller reads offsets[N], allocates, and calls again (two-phase output).
+ *   status_dev : DEVICE int32[1] or NULL; set to 0, or 1 if offsets[N] > capacity (then rows that
+ *                do not fit are not written).
+ * Row order is deterministic but unspecified (compare rows as sets).
+ * Errors: PETAR_ENOTBUILT, PETAR_EINVAL (capacity < 0), PETAR_ECUDA.                                */
+int petar_neighbor_list(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity,
+                        int32_t* status_dev, void* cuda_stream);
+
+/* Synchronises the stream and returns the device status word (PETAR_ST_* bits) in *status_host.    */
+int petar_tree_status(petar_tree* t, int32_t* status_host /* HOST */, void* cuda_stream);
+
+/* Invalidates and frees the HOST handle (the workspace stays the caller's).  NULL is allowed.      */
+int petar_tree_destroy(petar_tree* t);
+
+/* Static text for an error code; for PETAR_ECUDA the text of the last CUDA error seen.             */
+const char* petar_strerror(int code);
+
+/* ---- test hooks (not part of the timed path) ---------------------------------------------------
+ * petar_debug_export copies an intermediate to `dst` (DEVICE, dst_bytes) and synchronises.
+ * Layouts (n = N, nn = n_nodes, ng = n_groups; nodes in (level, begin) order, which is the
+ * library's own node numbering):
+ *   PETAR_DBG_HEADER   int64[8]  : n_nodes, n_groups, status, arena entries used, 0...
+ *   PETAR_DBG_ROOT     double[4] : root cube centre c[3], half edge h
+ *   PETAR_DBG_KEYS     uint64[n] : sorted Morton keys
+ *   PETAR_DBG_PERM     int32[n]  : sorted position -> caller's index
+ *   PETAR_DBG_NODE_INT int32[nn*4]: begin, end, first_child, level | nchild<<8 | leaf<<16
+ *   PETAR_DBG_NODE_DBL double[nn*17]: M, com[3], lo[3], hi[3], rmax, Q[6] (xx yy zz xy xz yz about com)
+ *   PETAR_DBG_GROUP_INT int32[ng*2]: begin, end
+ *   PETAR_DBG_GROUP_DBL double[ng*7]: lo[3], hi[3], rmax
+ *   PETAR_DBG_GROUP_CNT int32[ng*4]: n_sp, n_ep ranges (near), n_ep ranges (far), n_ep particles
+ *   PETAR_DBG_LIST_OFFS int64[ng*3+1]: start of each group's SP / near-EP / far-EP block in the
+ *                        flattened list below, in 4-byte entries; last = total
+ *   PETAR_DBG_LISTS    int32[total]: SP node ids; EP ranges as (begin, end) pairs
+ * The LIST_* exports require a prior petar_long_range_force or petar_neighbor_list on the tree.     */
+#define PETAR_DBG_HEADER 0
+#define PETAR_DBG_ROOT 1
+#define PETAR_DBG_KEYS 2
+#define PETAR_DBG_PERM 3
+#define PETAR_DBG_NODE_INT 4
+#define PETAR_DBG_NODE_DBL 5
+#define PETAR_DBG_GROUP_INT 6
+#define PETAR_DBG_GROUP_DBL 7
+#define PETAR_DBG_GROUP_CNT 8
+#define PETAR_DBG_LIST_OFFS 9
+#define PETAR_DBG_LISTS 10
+int petar_debug_export(petar_tree* t, int what, void* dst, size_t dst_bytes, void* cuda_stream);
+
+/* Per-stage device times of the last build / force / neighbour call on this tree, in ms, measured
+ * with CUDA events when profiling was switched on with petar_set_profiling(1) (HOST; default off;
+ * switching it on makes the calls synchronise).  stage_ms: HOST float[PETAR_N_STAGES].             */
+#define PETAR_STAGE_BBOX_KEYS 0
+#define PETAR_STAGE_SORT 1
+#define PETAR_STAGE_GATHER 2
+#define PETAR_STAGE_TREE 3
+#define PETAR_STAGE_MOMENTS 4
+#define PETAR_STAGE_GROUPS 5
+#define PETAR_STAGE_WALK 6
+#define PETAR_STAGE_FORCE 7
+#define PETAR_STAGE_NEIGHBOR 8
+#define PETAR_N_STAGES 9
+int petar_set_profiling(int on);
+int petar_stage_times(petar_tree* t, float* stage_ms /* HOST */);
+/* Number of kernel launches the library has enqueued since process start (HOST counter).           */
+int64_t petar_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PETAR_H_ */

@@ -1,0 +1,16 @@
+"""B200-native long-range P3T force path of PeTar (arxiv 2006.16560).
+
+The product is the C-ABI library ``libpetar_b200.so`` (include/petar.h, hand-written CUDA for
+sm_100a).  This package is the thin Python binding with the same names: it marshals arguments
+only -- every step of the path runs in the library's kernels.  PyTorch supplies device memory and
+streams.  There is no CPU fallback: if the library is missing or no CUDA device is present the
+calls raise.
+"""
+from .binding import (  # noqa: F401
+    PetarParams, PetarCounts, PetarError, Tree,
+    lib, library_path, exported_symbols,
+    petar_workspace_bytes, petar_tree_build, petar_long_range_force, petar_neighbor_list,
+    petar_tree_status, petar_tree_destroy, petar_strerror, petar_debug_export,
+    petar_set_profiling, petar_stage_times, petar_launch_count,
+    STAGE_NAMES,
+)

@@ -1,0 +1,277 @@
+// api.cu -- the C ABI of include/petar.h: argument checks, workspace carving, launch sequences.
+#include <stdio.h>
+#include <string.h>
+#include <stdlib.h>
+#include <atomic>
+#include <new>
+#include "internal.cuh"
+
+static thread_local cudaError_t g_last_cuda = cudaSuccess;
+static std::atomic<long long> g_launches{0};
+static int g_profiling = 0;
+static cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
+
+void petar_count_launch(int n) { g_launches += n; }
+void petar_debug_check(cudaStream_t s, const char* name) {
+    static int mode = -1;
+    if (mode < 0) { const char* e = getenv("PETAR_DEBUG_SYNC"); mode = (e && e[0] == '1') ? 1 : 0; }
+    if (!mode) return;
+    cudaError_t e = cudaStreamSynchronize(s);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) fprintf(stderr, "[petar] kernel %s failed: %s\n", name, cudaGetErrorString(e));
+}
+void stage_begin(petar_tree* t, cudaStream_t s) {
+    (void)t;
+    if (!g_profiling) return;
+    if (!g_ev0) { cudaEventCreate(&g_ev0); cudaEventCreate(&g_ev1); }
+    cudaEventRecord(g_ev0, s);
+}
+void stage_end(petar_tree* t, int stage, cudaStream_t s) {
+    if (!g_profiling) return;
+    cudaEventRecord(g_ev1, s);
+    cudaEventSynchronize(g_ev1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, g_ev0, g_ev1);
+    t->stage_ms[stage] = ms;
+}
+
+static inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+static bool params_ok(const petar_params* p) {
+    if (!p) return false;
+    if (!(p->G == p->G) || !(p->theta >= 0.0) || !(p->r_in_over_r_out > 0.0 && p->r_in_over_r_out < 1.0)) return false;
+    if (p->multipole != 1 && p->multipole != 2) return false;
+    if (p->n_leaf_limit < 1 || p->n_leaf_limit > 64) return false;
+    if (p->n_group_limit < p->n_leaf_limit || p->n_group_limit > 64) return false;
+    if (p->flags != 0) return false;
+    return true;
+}
+
+static int node_capacity(int64_t N, const petar_params* p) { return (int)((p->n_leaf_limit >= 4 ? N : 3 * N) + 4096); }
+static long long arena_chunks_for(int64_t N, const petar_params* p) {
+    double per = p->list_entries_per_particle > 0.0 ? p->list_entries_per_particle : 1024.0;
+    double entries = per * (double)N;
+    if (p->list_entries_per_particle <= 0.0 && entries < 16.0 * 1024 * 1024) entries = 16.0 * 1024 * 1024;
+    long long chunks = (long long)(entries / PETAR_CHUNK) + 64;
+    if (chunks > 2000000000ll / 1) chunks = 2000000000ll;
+    return chunks;
+}
+
+// Carves the workspace; with base == nullptr only sizes it.
+static size_t carve(Workspace* w, char* base, int64_t N, const petar_params* p) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) -> char* { char* r = base ? base + off : nullptr; off += align_up(bytes); return r; };
+    const size_t n = (size_t)N;
+    const int nblk = (int)((N + 2047) / 2048) + 1;
+    const int ntile = (int)((N + 1023) / 1024) + 1;
+    Workspace tmp; Workspace* W = w ? w : &tmp;
+    W->hdr = (DevHeader*)take(sizeof(DevHeader));
+    W->key = (unsigned long long*)take(n * 8); W->key_alt = (unsigned long long*)take(n * 8);
+    W->idx = (unsigned*)take(n * 4); W->idx_alt = (unsigned*)take(n * 4);
+    W->sort_hist = (unsigned*)take(8 * 256 * 4);
+    W->sort_blk = (unsigned*)take((size_t)256 * nblk * 4);
+    W->xs = (double*)take(n * 8); W->ys = (double*)take(n * 8); W->zs = (double*)take(n * 8);
+    W->ms = (double*)take(n * 8); W->routs = (double*)take(n * 8); W->rss = (double*)take(n * 8);
+    W->pa = (float4*)take(n * 16); W->pb = (float4*)take(n * 16);
+    W->D = (signed char*)take(n + 1); W->depth = (signed char*)take(n); W->glevel = (signed char*)take(n);
+    W->gflag = (int*)take((2 * (n + 1)) * 4);
+    W->tile_cnt = (int*)take((size_t)PETAR_NLEVELS * ntile * 4);
+    W->scan_tmp = (int*)take((size_t)(n / 4096 + 8) * 8);
+    W->node_cap = node_capacity(N, p);
+    W->nint = (NodeInt*)take((size_t)W->node_cap * sizeof(NodeInt));
+    W->nmac = (NodeMac*)take((size_t)W->node_cap * sizeof(NodeMac));
+    W->nmom = (NodeMom*)take((size_t)W->node_cap * sizeof(NodeMom));
+    W->nsp = (NodeSp*)take((size_t)W->node_cap * sizeof(NodeSp));
+    W->group_cap = (int)N + 1;
+    W->grp = (GroupRec*)take((size_t)W->group_cap * sizeof(GroupRec));
+    W->nb_cnt = (int*)take(n * 4);
+    W->exp_scratch = (int*)take((10 * (n + 1) + 8) * 4);
+    long long chunks = arena_chunks_for(N, p);
+    W->arena_chunks = (int)chunks;
+    W->arena = (int*)take((size_t)chunks * PETAR_CHUNK * 4);
+    return off;
+}
+
+extern "C" size_t petar_workspace_bytes(int64_t N, const petar_params* p) {
+    if (N < 0 || N > 2000000000ll || !params_ok(p)) return 0;
+    return carve(nullptr, nullptr, N, p) + 256;
+}
+
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_last_cuda = e_; return PETAR_ECUDA; } } while (0)
+
+extern "C" int petar_tree_build(const double* x, const double* y, const double* z, const double* m, const double* r_out,
+                                const double* r_search, int64_t N, const petar_params* p, void* workspace,
+                                size_t workspace_bytes, void* cuda_stream, petar_tree** tree_out) {
+    if (!tree_out) return PETAR_EINVAL;
+    *tree_out = nullptr;
+    if (N < 0 || N > 2000000000ll || !params_ok(p)) return PETAR_EINVAL;
+    if (N > 0 && (!x || !y || !z || !m || !r_out)) return PETAR_EINVAL;
+    size_t need = petar_workspace_bytes(N, p);
+    if (N > 0 && (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 255u))) return PETAR_EWORKSPACE;
+    petar_tree* t = new (std::nothrow) petar_tree();
+    if (!t) return PETAR_EINVAL;
+    memset(t, 0, sizeof(*t));
+    t->magic = PETAR_MAGIC; t->N = N; t->p = *p;
+    t->x = x; t->y = y; t->z = z; t->m = m; t->r_out = r_out; t->r_search = r_search;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&t->pinned, 64 * sizeof(long long));
+    if (e != cudaSuccess) { g_last_cuda = e; delete t; return PETAR_ECUDA; }
+    if (N > 0) {
+        carve(&t->w, (char*)workspace, N, p);
+        e = launch_keys_sort_gather(t, s);
+        if (e == cudaSuccess) e = launch_tree(t, s);
+        if (e != cudaSuccess) { g_last_cuda = e; cudaFreeHost(t->pinned); delete t; return PETAR_ECUDA; }
+    }
+    t->built = true; t->walked = false;
+    *tree_out = t;
+    return PETAR_OK;
+}
+
+static int check_tree(petar_tree* t) { return (t && t->magic == PETAR_MAGIC && t->built) ? PETAR_OK : PETAR_ENOTBUILT; }
+
+static int ensure_walk(petar_tree* t, cudaStream_t s) {
+    if (t->walked) return PETAR_OK;
+    CK(launch_walk(t, s));
+    t->walked = true;
+    return PETAR_OK;
+}
+
+// reads the device header into t->pinned (as DevHeader) and synchronises
+static int read_header(petar_tree* t, cudaStream_t s, DevHeader* out) {
+    CK(cudaMemcpyAsync(out, t->w.hdr, sizeof(DevHeader), cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    return PETAR_OK;
+}
+
+extern "C" int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_y, double* acc_z, double* pot,
+                                      petar_counts* counts, void* cuda_stream) {
+    int rc = check_tree(t);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (t->N == 0) { if (counts) memset(counts, 0, sizeof(*counts)); return PETAR_OK; }
+    rc = ensure_walk(t, s);
+    if (rc) return rc;
+    CK(launch_force(t, acc_x, acc_y, acc_z, pot, s));
+    if (counts) {
+        DevHeader hh;
+        rc = read_header(t, s, &hh);
+        if (rc) return rc;
+        counts->n_groups = hh.n_groups; counts->n_nodes = hh.n_nodes;
+        counts->n_epep = (int64_t)hh.n_epep; counts->n_epsp = (int64_t)hh.n_epsp; counts->n_epep_near = (int64_t)hh.n_epep_near;
+        counts->n_ep_list = (int64_t)hh.n_ep_list; counts->n_sp_list = (int64_t)hh.n_sp_list;
+        counts->list_entries_used = (int64_t)hh.arena_top * PETAR_CHUNK;
+        if (hh.status) return PETAR_ESTATUS;
+    }
+    return PETAR_OK;
+}
+
+extern "C" int petar_neighbor_list(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity, int32_t* status_dev,
+                                   void* cuda_stream) {
+    int rc = check_tree(t);
+    if (rc) return rc;
+    if (!offsets || capacity < 0) return PETAR_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (t->N == 0) {
+        CK(cudaMemsetAsync(offsets, 0, 8, s));
+        if (status_dev) CK(cudaMemsetAsync(status_dev, 0, 4, s));
+        return PETAR_OK;
+    }
+    rc = ensure_walk(t, s);
+    if (rc) return rc;
+    CK(launch_neighbors(t, offsets, indices, capacity, status_dev, s));
+    return PETAR_OK;
+}
+
+extern "C" int petar_tree_status(petar_tree* t, int32_t* status_host, void* cuda_stream) {
+    int rc = check_tree(t);
+    if (rc) return rc;
+    if (!status_host) return PETAR_EINVAL;
+    if (t->N == 0) { *status_host = 0; return PETAR_OK; }
+    DevHeader hh;
+    rc = read_header(t, (cudaStream_t)cuda_stream, &hh);
+    if (rc) return rc;
+    *status_host = hh.status;
+    return PETAR_OK;
+}
+
+extern "C" int petar_tree_destroy(petar_tree* t) {
+    if (!t) return PETAR_OK;
+    if (t->magic != PETAR_MAGIC) return PETAR_ENOTBUILT;
+    t->magic = 0; t->built = false;
+    if (t->pinned) cudaFreeHost(t->pinned);
+    delete t;
+    return PETAR_OK;
+}
+
+extern "C" const char* petar_strerror(int code) {
+    switch (code) {
+        case PETAR_OK: return "ok";
+        case PETAR_EINVAL: return "invalid argument";
+        case PETAR_EWORKSPACE: return "workspace too small or misaligned";
+        case PETAR_ECUDA: return cudaGetErrorString(g_last_cuda);
+        case PETAR_ENOTBUILT: return "no tree built / handle destroyed";
+        case PETAR_ESTATUS: return "device status word non-zero (see petar_tree_status)";
+        default: return "unknown error";
+    }
+}
+
+extern "C" int petar_debug_export(petar_tree* t, int what, void* dst, size_t dst_bytes, void* cuda_stream) {
+    int rc = check_tree(t);
+    if (rc) return rc;
+    if (!dst) return PETAR_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (t->N == 0) return PETAR_OK;
+    DevHeader hh;
+    rc = read_header(t, s, &hh);
+    if (rc) return rc;
+    t->pinned[0] = hh.n_nodes; t->pinned[1] = hh.n_groups;
+    const size_t n = (size_t)t->N;
+    const Workspace& w = t->w;
+    auto copy = [&](const void* src, size_t bytes) -> int {
+        if (dst_bytes < bytes) return PETAR_EINVAL;
+        CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, s));
+        return PETAR_OK;
+    };
+    switch (what) {
+        case PETAR_DBG_HEADER: {
+            long long v[8] = {hh.n_nodes, hh.n_groups, hh.status, (long long)hh.arena_top * PETAR_CHUNK, 0, 0, 0, 0};
+            if (dst_bytes < sizeof(v)) return PETAR_EINVAL;
+            CK(cudaMemcpyAsync(dst, v, sizeof(v), cudaMemcpyHostToDevice, s));
+            break;
+        }
+        case PETAR_DBG_ROOT: {
+            double v[4] = {hh.c[0], hh.c[1], hh.c[2], hh.h};
+            if (dst_bytes < sizeof(v)) return PETAR_EINVAL;
+            CK(cudaMemcpyAsync(dst, v, sizeof(v), cudaMemcpyHostToDevice, s));
+            break;
+        }
+        case PETAR_DBG_KEYS: rc = copy(w.key, n * 8); break;
+        case PETAR_DBG_PERM: rc = copy(w.idx, n * 4); break;
+        case PETAR_DBG_NODE_INT: rc = copy(w.nint, (size_t)hh.n_nodes * sizeof(NodeInt)); break;
+        case PETAR_DBG_NODE_DBL: case PETAR_DBG_GROUP_INT: case PETAR_DBG_GROUP_DBL: case PETAR_DBG_GROUP_CNT:
+        case PETAR_DBG_LIST_OFFS: case PETAR_DBG_LISTS: {
+            if ((what == PETAR_DBG_GROUP_CNT || what == PETAR_DBG_LIST_OFFS || what == PETAR_DBG_LISTS) && !t->walked) return PETAR_ENOTBUILT;
+            cudaError_t e = launch_export_lists(t, what, dst, dst_bytes, s);
+            if (e == cudaErrorInvalidValue) return PETAR_EINVAL;
+            CK(e);
+            break;
+        }
+        default: return PETAR_EINVAL;
+    }
+    if (rc) return rc;
+    CK(cudaStreamSynchronize(s));
+    return PETAR_OK;
+}
+
+extern "C" int petar_set_profiling(int on) { g_profiling = on ? 1 : 0; return PETAR_OK; }
+extern "C" int petar_stage_times(petar_tree* t, float* stage_ms) {
+    int rc = check_tree(t);
+    if (rc) return rc;
+    if (!stage_ms) return PETAR_EINVAL;
+    memcpy(stage_ms, t->stage_ms, sizeof(t->stage_ms));
+    return PETAR_OK;
+}
+extern "C" int64_t petar_launch_count(void) { return (int64_t)g_launches.load(); }

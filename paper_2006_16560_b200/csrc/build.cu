@@ -1,0 +1,758 @@
+// build.cu -- steps S0-S6: bounding cube, Morton keys, stable LSD radix sort, sorted SoA gather,
+// octree from sorted keys (no level loop: nodes are enumerated per key boundary), bottom-up
+// moments, i-groups.   Compiled with -fmad=false: every fp64 operation below is exactly the one
+// written (fma only where rule O5 says so), because key, permutation, node and group tables must be
+// bit-identical to an independent fp64 implementation of DESIGN.md's rules O1-O6.
+#include <cooperative_groups.h>
+#include "internal.cuh"
+namespace cg = cooperative_groups;
+
+// ------------------------------------------------------------------------------------------------
+// small device helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long enc_f64(double d) {
+    unsigned long long b = (unsigned long long)__double_as_longlong(d);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double dec_f64(unsigned long long e) {
+    unsigned long long b = (e >> 63) ? (e & 0x7fffffffffffffffull) : ~e;
+    return __longlong_as_double((long long)b);
+}
+__device__ __forceinline__ unsigned long long spread21(unsigned long long x) {
+    x &= 0x1fffffull;
+    x = (x | x << 32) & 0x1f00000000ffffull;
+    x = (x | x << 16) & 0x1f0000ff0000ffull;
+    x = (x | x << 8) & 0x100f00f00f00f00full;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ull;
+    x = (x | x << 2) & 0x1249249249249249ull;
+    return x;
+}
+__device__ __forceinline__ unsigned compact21(unsigned long long x) {   // inverse of spread21
+    x &= 0x1249249249249249ull;
+    x = (x | x >> 2) & 0x10c30c30c30c30c3ull;
+    x = (x | x >> 4) & 0x100f00f00f00f00full;
+    x = (x | x >> 8) & 0x1f0000ff0000ffull;
+    x = (x | x >> 16) & 0x1f00000000ffffull;
+    x = (x | x >> 32) & 0x1fffffull;
+    return (unsigned)x;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S0: header reset + bounding box
+// ------------------------------------------------------------------------------------------------
+__global__ void k_reset_header(DevHeader* h) {
+    if (threadIdx.x == 0) {
+        for (int k = 0; k < 3; ++k) { h->bbox[k] = ~0ull; h->bbox[3 + k] = 0ull; }
+        h->n_nodes = 0; h->n_groups = 0; h->status = 0; h->arena_top = 0;
+        h->group_ticket = 0; h->group_ticket2 = 0; h->group_ticket3 = 0;
+        h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = 0ull; h->nb_total = 0ull;
+        for (int l = 0; l < PETAR_NLEVELS + 2; ++l) h->level_off[l] = 0;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_bbox(const double* __restrict__ x, const double* __restrict__ y,
+                                              const double* __restrict__ z, const double* __restrict__ m,
+                                              const double* __restrict__ ro, const double* __restrict__ rs,
+                                              long long n, DevHeader* h) {
+    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    bool bad = false;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        double v[3] = {x[i], y[i], z[i]};
+        double mi = m[i], r = ro[i];
+        bad |= !(isfinite(v[0]) && isfinite(v[1]) && isfinite(v[2]) && isfinite(mi) && isfinite(r) && r > 0.0);
+        if (rs) { double q = rs[i]; bad |= !(isfinite(q) && q >= r); }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { lo[k] = fmin(lo[k], v[k]); hi[k] = fmax(hi[k], v[k]); }
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        for (int o = 16; o; o >>= 1) {
+            lo[k] = fmin(lo[k], __shfl_xor_sync(0xffffffffu, lo[k], o));
+            hi[k] = fmax(hi[k], __shfl_xor_sync(0xffffffffu, hi[k], o));
+        }
+    bad = __any_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            if (lo[k] <= hi[k]) { atomicMin(&h->bbox[k], enc_f64(lo[k])); atomicMax(&h->bbox[3 + k], enc_f64(hi[k])); }
+        }
+        if (bad) atomicOr(&h->status, PETAR_ST_NONFINITE);
+    }
+}
+
+// O1: root cube.  c = 0.5 (lo + hi); L = max extent; v = 0.5 L (1 + 2^-20); h = 2^e with frexp(v) = (f, e).
+__global__ void k_root(DevHeader* h) {
+    if (threadIdx.x != 0) return;
+    double L = 0.0;
+    for (int k = 0; k < 3; ++k) {
+        double lo = dec_f64(h->bbox[k]), hi = dec_f64(h->bbox[3 + k]);
+        h->c[k] = 0.5 * (lo + hi);
+        double e = hi - lo;
+        if (e > L) L = e;
+    }
+    double hh;
+    if (!(L > 0.0) || !isfinite(L)) hh = 1.0;
+    else {
+        double v = 0.5 * L * (1.0 + 9.5367431640625e-07);   // 2^-20
+        int e; (void)frexp(v, &e);
+        hh = ldexp(1.0, e);
+    }
+    h->h = hh;
+    for (int k = 0; k < 3; ++k) h->o[k] = h->c[k] - hh;
+    h->inv_s = ldexp(1.0, PETAR_MAXLEVEL) / (2.0 * hh);     // exact: power of two
+}
+
+// O2 + O3: keys.
+__global__ void __launch_bounds__(256) k_keys(const double* __restrict__ x, const double* __restrict__ y,
+                                              const double* __restrict__ z, long long n, const DevHeader* __restrict__ h,
+                                              unsigned long long* __restrict__ key, unsigned* __restrict__ idx) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double inv_s = h->inv_s;
+    double v[3] = {x[i], y[i], z[i]};
+    unsigned long long q[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        double g = floor((v[k] - h->o[k]) * inv_s);
+        long long qi = (g >= 0.0) ? ((g < 2097152.0) ? (long long)g : 2097151ll) : 0ll;   // NaN -> 0
+        q[k] = (unsigned long long)qi;
+    }
+    key[i] = (spread21(q[0]) << 2) | (spread21(q[1]) << 1) | spread21(q[2]);
+    idx[i] = (unsigned)i;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S2: stable LSD radix sort of (key, idx), 8 passes x 8 bits.  Tile = 2048 elements per CTA.
+// ------------------------------------------------------------------------------------------------
+#define SORT_TILE 2048
+#define SORT_THREADS 256
+#define SORT_ITEMS 8
+
+// per-block digit counts of the current pass:  blk[d * nblk + b]
+__global__ void __launch_bounds__(SORT_THREADS) k_sort_count(const unsigned long long* __restrict__ key, long long n, int shift,
+                                                             unsigned* __restrict__ blk, int nblk, unsigned* __restrict__ tot) {
+    __shared__ unsigned cnt[256];
+    cnt[threadIdx.x] = 0;
+    __syncthreads();
+    long long base = (long long)blockIdx.x * SORT_TILE;
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        long long i = base + r * SORT_THREADS + threadIdx.x;
+        if (i < n) atomicAdd(&cnt[(unsigned)(key[i] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    blk[threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
+    if (cnt[threadIdx.x]) atomicAdd(&tot[threadIdx.x], cnt[threadIdx.x]);      // digit totals of this pass
+}
+
+// one CTA per digit d: blk[d][b] <- (number of keys with smaller digit) + (same digit in earlier blocks)
+__global__ void __launch_bounds__(256) k_sort_scan(unsigned* __restrict__ blk, int nblk, const unsigned* __restrict__ tot) {
+    __shared__ unsigned red[256];
+    __shared__ unsigned carry_s;
+    const int d = blockIdx.x, t = threadIdx.x;
+    // total of every digit e < d (from the pass's digit totals; the rows of other digits are being
+    // rewritten concurrently by their own CTAs and must not be read here)
+    red[t] = (t < d) ? tot[t] : 0u;
+    __syncthreads();
+    for (int o = 128; o; o >>= 1) { if (t < o) red[t] += red[t + o]; __syncthreads(); }
+    if (t == 0) carry_s = red[0];
+    __syncthreads();
+    unsigned* row = blk + (size_t)d * nblk;
+    for (int b0 = 0; b0 < nblk; b0 += 256) {
+        int b = b0 + t;
+        unsigned v = (b < nblk) ? row[b] : 0u;
+        // block inclusive scan (Hillis-Steele in smem)
+        __syncthreads();
+        red[t] = v;
+        __syncthreads();
+        for (int o = 1; o < 256; o <<= 1) {
+            unsigned a = (t >= o) ? red[t - o] : 0u;
+            __syncthreads();
+            red[t] += a;
+            __syncthreads();
+        }
+        unsigned incl = red[t], carry = carry_s;
+        if (b < nblk) row[b] = carry + incl - v;
+        __syncthreads();
+        if (t == 255) carry_s = carry + incl;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(SORT_THREADS) k_sort_scatter(const unsigned long long* __restrict__ kin, const unsigned* __restrict__ vin,
+                                                               unsigned long long* __restrict__ kout, unsigned* __restrict__ vout,
+                                                               const unsigned* __restrict__ blk, int nblk, long long n, int shift) {
+    __shared__ unsigned wcnt[SORT_THREADS / 32][256];
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    for (int k = t; k < (SORT_THREADS / 32) * 256; k += SORT_THREADS) (&wcnt[0][0])[k] = 0;
+    __syncthreads();
+    const long long base = (long long)blockIdx.x * SORT_TILE + (long long)w * (SORT_TILE / (SORT_THREADS / 32));
+    unsigned long long k[SORT_ITEMS];
+    unsigned v[SORT_ITEMS], rank[SORT_ITEMS];
+    const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        long long i = base + r * 32 + lane;
+        bool ok = i < n;
+        k[r] = ok ? kin[i] : ~0ull;
+        v[r] = ok ? vin[i] : 0u;
+        unsigned d = ok ? ((unsigned)(k[r] >> shift) & 255u) : 255u;
+        unsigned peers = __match_any_sync(0xffffffffu, d);
+        int leader = __ffs(peers) - 1;
+        unsigned prev = 0;
+        if (lane == leader) { prev = wcnt[w][d]; wcnt[w][d] = prev + __popc(peers); }
+        prev = __shfl_sync(0xffffffffu, prev, leader);
+        rank[r] = prev + __popc(peers & lt);
+        __syncwarp();
+    }
+    __syncthreads();
+    {   // per digit (thread t = digit): exclusive scan over warps, seeded with the global block offset
+        unsigned run = blk[(size_t)t * nblk + blockIdx.x];
+#pragma unroll
+        for (int ww = 0; ww < SORT_THREADS / 32; ++ww) { unsigned c = wcnt[ww][t]; wcnt[ww][t] = run; run += c; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < SORT_ITEMS; ++r) {
+        long long i = base + r * 32 + lane;
+        if (i < n) {
+            unsigned d = (unsigned)(k[r] >> shift) & 255u;
+            unsigned pos = wcnt[w][d] + rank[r];
+            kout[pos] = k[r];
+            vout[pos] = v[r];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S3: gather into sorted order + fp32 float-float records relative to the root centre
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_gather(const unsigned* __restrict__ idx, long long n, const DevHeader* __restrict__ h,
+                                                const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
+                                                const double* __restrict__ m, const double* __restrict__ ro, const double* __restrict__ rs,
+                                                double* __restrict__ xs, double* __restrict__ ys, double* __restrict__ zs,
+                                                double* __restrict__ ms, double* __restrict__ ros, double* __restrict__ rss,
+                                                float4* __restrict__ pa, float4* __restrict__ pb) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    unsigned o = idx[i];
+    double vx = x[o], vy = y[o], vz = z[o], vm = m[o], vr = ro[o];
+    xs[i] = vx; ys[i] = vy; zs[i] = vz; ms[i] = vm; ros[i] = vr;
+    if (rs) rss[i] = rs[o];
+    double dx = vx - h->c[0], dy = vy - h->c[1], dz = vz - h->c[2];
+    float xh = (float)dx, yh = (float)dy, zh = (float)dz;
+    float xl = (float)(dx - (double)xh), yl = (float)(dy - (double)yh), zl = (float)(dz - (double)zh);
+    pa[i] = make_float4(xh, yh, zh, (float)vm);
+    pb[i] = make_float4(xl, yl, zl, (float)(1.0 / vr));
+}
+
+// ------------------------------------------------------------------------------------------------
+// S4: octree from sorted keys.
+//   D[i]  (i = 0..N) = number of leading octal digits keys i-1 and i share (-1 at both array ends).
+//   Keys i-1 and i lie in the same level-l cell iff D[i] >= l.
+//   depth[i]  = leaf level of particle i  = smallest l whose cell holds <= n_leaf particles (cap 21)
+//   glevel[i] = group level               = same with n_group, capped by depth
+//   A level-l node starts at boundary i  iff  D[i] < l <= depth[i].
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_diverge(const unsigned long long* __restrict__ key, long long n, signed char* __restrict__ D) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i > n) return;
+    int d = -1;
+    if (i > 0 && i < n) {
+        unsigned long long xr = key[i - 1] ^ key[i];
+        d = xr ? (__clzll((long long)xr) - 1) / 3 : PETAR_MAXLEVEL;     // bit 62 is the top key bit
+    }
+    D[i] = (signed char)d;
+}
+
+// smallest level l such that the level-l cell containing particle i holds <= L particles, using the
+// window D[i-L+1 .. i+L] held in shared memory `sd` (index 0 <-> boundary `w0`).  Returns up to 22
+// (22 = even the level-21 cell is over-full).
+__device__ __forceinline__ int level_for_limit(const signed char* sd, long long w0, long long i, long long n, int L) {
+    int best = 127, run = 127;
+    for (int k = 1; k <= L; ++k) {
+        long long e = i + k;
+        int de = (e <= n) ? (int)sd[e - w0] : -1;
+        run = min(run, de);
+        long long b = i - L + k;
+        if (b >= 0) best = min(best, max((int)sd[b - w0], run));
+    }
+    return best + 1;
+}
+
+#define DEPTH_THREADS 256
+__global__ void __launch_bounds__(DEPTH_THREADS) k_depth(const unsigned long long* __restrict__ key, const signed char* __restrict__ D,
+                                                         long long n, int n_leaf, int n_group,
+                                                         signed char* __restrict__ depth, signed char* __restrict__ glevel,
+                                                         int* __restrict__ gflag) {
+    extern __shared__ signed char sd[];
+    const long long i0 = (long long)blockIdx.x * DEPTH_THREADS;
+    const int halo = n_group;
+    const long long w0 = i0 - halo;
+    const int wn = DEPTH_THREADS + 2 * halo + 1;
+    for (int k = threadIdx.x; k < wn; k += DEPTH_THREADS) {
+        long long b = w0 + k;
+        sd[k] = (b >= 0 && b <= n) ? D[b] : (signed char)-1;
+    }
+    __syncthreads();
+    long long i = i0 + threadIdx.x;
+    if (i >= n) return;
+    int dl = min(level_for_limit(sd, w0, i, n, n_leaf), PETAR_MAXLEVEL);
+    int gl_raw = level_for_limit(sd, w0, i, n, n_group);
+    int gl = min(min(gl_raw, PETAR_MAXLEVEL), dl);
+    depth[i] = (signed char)dl;
+    glevel[i] = (signed char)gl;
+    int flag;
+    if (gl_raw > PETAR_MAXLEVEL) {
+        // over-full level-21 cell: cut into consecutive chunks of n_group from the cell's first particle
+        unsigned long long kk = key[i];
+        long long lo = 0, hi = i;                 // first index with key == kk
+        while (lo < hi) { long long mid = (lo + hi) >> 1; if (key[mid] < kk) lo = mid + 1; else hi = mid; }
+        flag = ((i - lo) % n_group) == 0;
+    } else {
+        flag = (int)sd[i - w0] < gl;
+    }
+    gflag[i] = flag;
+}
+
+// ---- node ranking: id(i, l) = level_off[l] + (#level-l nodes starting before boundary i) ----------
+#define RANK_THREADS 1024
+__global__ void __launch_bounds__(RANK_THREADS) k_rank_count(const signed char* __restrict__ D, const signed char* __restrict__ depth,
+                                                             long long n, int* __restrict__ tile_cnt, int ntile) {
+    __shared__ int cnt[PETAR_NLEVELS];
+    if (threadIdx.x < PETAR_NLEVELS) cnt[threadIdx.x] = 0;
+    __syncthreads();
+    long long i = (long long)blockIdx.x * RANK_THREADS + threadIdx.x;
+    if (i < n) {
+        int lo = D[i] + 1, hi = depth[i];
+        for (int l = lo; l <= hi; ++l) atomicAdd(&cnt[l], 1);
+    }
+    __syncthreads();
+    if (threadIdx.x < PETAR_NLEVELS) tile_cnt[threadIdx.x * ntile + blockIdx.x] = cnt[threadIdx.x];
+}
+
+// single CTA: per level exclusive scan over tiles; level offsets; node count and capacity check
+__global__ void __launch_bounds__(1024) k_rank_scan(int* __restrict__ tile_cnt, int ntile, DevHeader* __restrict__ h, int node_cap) {
+    __shared__ int buf[1024];
+    __shared__ int carry_s;
+    __shared__ int tot[PETAR_NLEVELS];
+    const int t = threadIdx.x;
+    for (int l = 0; l < PETAR_NLEVELS; ++l) {
+        if (t == 0) carry_s = 0;
+        __syncthreads();
+        int* row = tile_cnt + (size_t)l * ntile;
+        for (int b0 = 0; b0 < ntile; b0 += 1024) {
+            int b = b0 + t;
+            int v = (b < ntile) ? row[b] : 0;
+            buf[t] = v;
+            __syncthreads();
+            for (int o = 1; o < 1024; o <<= 1) {
+                int a = (t >= o) ? buf[t - o] : 0;
+                __syncthreads();
+                buf[t] += a;
+                __syncthreads();
+            }
+            int incl = buf[t], carry = carry_s;
+            if (b < ntile) row[b] = carry + incl - v;
+            __syncthreads();
+            if (t == 1023) carry_s = carry + incl;
+            __syncthreads();
+        }
+        if (t == 0) tot[l] = carry_s;
+        __syncthreads();
+    }
+    if (t == 0) {
+        int run = 0;
+        for (int l = 0; l < PETAR_NLEVELS; ++l) { h->level_off[l] = run; run += tot[l]; }
+        h->level_off[PETAR_NLEVELS] = run; h->level_off[PETAR_NLEVELS + 1] = run;
+        h->n_nodes = run;
+        if (run > node_cap) { atomicOr(&h->status, PETAR_ST_NODE_CAP); }
+    }
+}
+
+__global__ void __launch_bounds__(RANK_THREADS) k_nodes_write(const unsigned long long* __restrict__ key, const signed char* __restrict__ D,
+                                                              const signed char* __restrict__ depth, long long n,
+                                                              const int* __restrict__ tile_off, int ntile, const DevHeader* __restrict__ h,
+                                                              NodeInt* __restrict__ nint, int node_cap) {
+    __shared__ unsigned s_bal[RANK_THREADS / 32][PETAR_NLEVELS];
+    __shared__ int s_woff[RANK_THREADS / 32][PETAR_NLEVELS];
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const long long i = (long long)blockIdx.x * RANK_THREADS + t;
+    int lo = 1, hi = 0;
+    if (i < n) { lo = D[i] + 1; hi = depth[i]; }
+#pragma unroll
+    for (int l = 0; l < PETAR_NLEVELS; ++l) {
+        unsigned bal = __ballot_sync(0xffffffffu, l >= lo && l <= hi);
+        if (lane == 0) s_bal[w][l] = bal;
+    }
+    __syncthreads();
+    if (t < PETAR_NLEVELS) {
+        int run = h->level_off[t] + tile_off[(size_t)t * ntile + blockIdx.x];
+        for (int ww = 0; ww < RANK_THREADS / 32; ++ww) { s_woff[ww][t] = run; run += __popc(s_bal[ww][t]); }
+    }
+    __syncthreads();
+    if (h->n_nodes > node_cap) return;            // capacity exceeded: status already set
+    if (i >= n || lo > hi) return;
+    const unsigned lt = (1u << lane) - 1u;
+    const unsigned long long ki = key[i];
+    for (int l = lo; l <= hi; ++l) {
+        int id = s_woff[w][l] + __popc(s_bal[w][l] & lt);
+        int child = (l < hi) ? (s_woff[w][l + 1] + __popc(s_bal[w][l + 1] & lt)) : -1;
+        // end of the cell: first j > i whose level-l prefix differs (galloping + binary search)
+        long long end;
+        if (l == 0) end = n;
+        else {
+            const int shift = 3 * (PETAR_MAXLEVEL - l);
+            const unsigned long long pref = ki >> shift;
+            long long a = i, step = 1;
+            while (a + step < n && (key[a + step] >> shift) == pref) { a += step; step <<= 1; }
+            long long b = min(n, a + step);        // key[a] matches, key[b] differs or b == n
+            while (b - a > 1) { long long mid = (a + b) >> 1; if ((key[mid] >> shift) == pref) a = mid; else b = mid; }
+            end = b;
+        }
+        NodeInt r;
+        r.begin = (int)i; r.end = (int)end; r.first_child = child;
+        r.meta = l | ((l == hi) ? (1 << 16) : 0) | ((l > lo) ? (1 << 17) : 0);
+        nint[id] = r;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S5: bottom-up moments, one level per grid-wide phase (cooperative launch).  Summation order is
+// rule O5: leaf = members in sorted order with S = fma(m, x, S); internal = children ascending.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_moments(const DevHeader* __restrict__ h, NodeInt* __restrict__ nint, NodeMac* __restrict__ nmac,
+                                                 NodeMom* __restrict__ nmom, NodeSp* __restrict__ nsp,
+                                                 const unsigned long long* __restrict__ key,
+                                                 const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
+                                                 const double* __restrict__ ms, const double* __restrict__ rss, int node_cap, int multipole) {
+    cg::grid_group grid = cg::this_grid();
+    if (h->n_nodes > node_cap) return;            // uniform across the grid
+    const long long gsz = (long long)gridDim.x * blockDim.x;
+    const long long gtid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const double cx = h->c[0], cy = h->c[1], cz = h->c[2];
+    for (int l = PETAR_MAXLEVEL; l >= 0; --l) {
+        const int n0 = h->level_off[l], n1 = h->level_off[l + 1], n2 = h->level_off[l + 2];
+        for (long long id = n0 + gtid; id < n1; id += gsz) {
+            NodeInt r = nint[id];
+            double M = 0, S0 = 0, S1 = 0, S2 = 0, rmax = 0;
+            double lo0 = INFINITY, lo1 = INFINITY, lo2 = INFINITY, hi0 = -INFINITY, hi1 = -INFINITY, hi2 = -INFINITY;
+            double Q[6] = {0, 0, 0, 0, 0, 0};
+            double com0, com1, com2;
+            const bool leaf = (r.meta >> 16) & 1;
+            int nchild = 0;
+            if (leaf) {
+                for (int p = r.begin; p < r.end; ++p) {
+                    double m = ms[p], x = xs[p], y = ys[p], z = zs[p];
+                    M = M + m;
+                    S0 = fma(m, x, S0); S1 = fma(m, y, S1); S2 = fma(m, z, S2);
+                    lo0 = fmin(lo0, x); lo1 = fmin(lo1, y); lo2 = fmin(lo2, z);
+                    hi0 = fmax(hi0, x); hi1 = fmax(hi1, y); hi2 = fmax(hi2, z);
+                    rmax = fmax(rmax, rss[p]);
+                }
+            } else {
+                int c = r.first_child;
+                do {
+                    NodeMom cm = nmom[c];
+                    NodeMac cc = nmac[c];
+                    M = M + cm.M; S0 = S0 + cm.S[0]; S1 = S1 + cm.S[1]; S2 = S2 + cm.S[2];
+                    lo0 = fmin(lo0, cc.lo[0]); lo1 = fmin(lo1, cc.lo[1]); lo2 = fmin(lo2, cc.lo[2]);
+                    hi0 = fmax(hi0, cc.hi[0]); hi1 = fmax(hi1, cc.hi[1]); hi2 = fmax(hi2, cc.hi[2]);
+                    rmax = fmax(rmax, cc.rmax);
+                    ++c; ++nchild;
+                } while (nchild < 8 && c < n2 && !((nint[c].meta >> 17) & 1));
+            }
+            if (M != 0.0) { com0 = S0 / M; com1 = S1 / M; com2 = S2 / M; }
+            else {
+                // massless cell: centre of its cube
+                unsigned long long pref = l ? (key[r.begin] >> (3 * (PETAR_MAXLEVEL - l))) << (3 * (PETAR_MAXLEVEL - l)) : 0ull;
+                double edge = ldexp(2.0 * h->h, -l);
+                int sh = PETAR_MAXLEVEL - l;
+                double q0 = (double)(compact21(pref >> 2) >> sh), q1 = (double)(compact21(pref >> 1) >> sh), q2 = (double)(compact21(pref) >> sh);
+                com0 = h->o[0] + (q0 + 0.5) * edge; com1 = h->o[1] + (q1 + 0.5) * edge; com2 = h->o[2] + (q2 + 0.5) * edge;
+            }
+            // quadrupole about com (Eq. 30): any summation order is allowed (tolerance-compared only)
+            if (leaf) {
+                for (int p = r.begin; p < r.end; ++p) {
+                    double m = ms[p], dx = xs[p] - com0, dy = ys[p] - com1, dz = zs[p] - com2;
+                    Q[0] += m * dx * dx; Q[1] += m * dy * dy; Q[2] += m * dz * dz;
+                    Q[3] += m * dx * dy; Q[4] += m * dx * dz; Q[5] += m * dy * dz;
+                }
+            } else {
+                for (int k = 0; k < nchild; ++k) {        // parallel-axis rule
+                    int c = r.first_child + k;
+                    NodeMom cm = nmom[c];
+                    NodeMac cc = nmac[c];
+                    double dx = cc.com[0] - com0, dy = cc.com[1] - com1, dz = cc.com[2] - com2;
+                    Q[0] += cm.Q[0] + cm.M * dx * dx; Q[1] += cm.Q[1] + cm.M * dy * dy; Q[2] += cm.Q[2] + cm.M * dz * dz;
+                    Q[3] += cm.Q[3] + cm.M * dx * dy; Q[4] += cm.Q[4] + cm.M * dx * dz; Q[5] += cm.Q[5] + cm.M * dy * dz;
+                }
+                nint[id].meta = r.meta | (nchild << 8);
+            }
+            NodeMac mac;
+            mac.lo[0] = lo0; mac.lo[1] = lo1; mac.lo[2] = lo2; mac.hi[0] = hi0; mac.hi[1] = hi1; mac.hi[2] = hi2;
+            mac.com[0] = com0; mac.com[1] = com1; mac.com[2] = com2; mac.rmax = rmax;
+            nmac[id] = mac;
+            NodeMom mom;
+            mom.M = M; mom.S[0] = S0; mom.S[1] = S1; mom.S[2] = S2;
+            for (int k = 0; k < 6; ++k) mom.Q[k] = Q[k];
+            nmom[id] = mom;
+            // fp32 super-particle record: float-float position relative to the root centre, traceless A'
+            double dx = com0 - cx, dy = com1 - cy, dz = com2 - cz;
+            float xh = (float)dx, yh = (float)dy, zh = (float)dz;
+            float xl = (float)(dx - (double)xh), yl = (float)(dy - (double)yh), zl = (float)(dz - (double)zh);
+            double tr = Q[0] + Q[1] + Q[2];
+            NodeSp sp;
+            sp.q0 = make_float4(xh, yh, zh, (float)M);
+            if (multipole >= 2) {
+                sp.q1 = make_float4(xl, yl, zl, (float)(1.5 * Q[0] - 0.5 * tr));
+                sp.q2 = make_float4((float)(1.5 * Q[1] - 0.5 * tr), (float)(1.5 * Q[3]), (float)(1.5 * Q[4]), (float)(1.5 * Q[5]));
+            } else {
+                sp.q1 = make_float4(xl, yl, zl, 0.f);
+                sp.q2 = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+            nsp[id] = sp;
+        }
+        grid.sync();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S6: i-groups from the scanned start flags
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_groups_begin(const int* __restrict__ gflag, const int* __restrict__ gscan, long long n,
+                                                      GroupRec* __restrict__ grp, DevHeader* __restrict__ h) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i == 0) h->n_groups = gscan[n];
+    if (i >= n) return;
+    if (gflag[i]) grp[gscan[i]].begin = (int)i;
+}
+
+// one warp per group: end, tight box, rmax; list heads reset
+__global__ void __launch_bounds__(256) k_groups_finish(GroupRec* __restrict__ grp, const DevHeader* __restrict__ h, long long n,
+                                                       const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
+                                                       const double* __restrict__ rss) {
+    const int lane = threadIdx.x & 31;
+    const int ng = h->n_groups;
+    for (long long g = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5; g < ng; g += ((long long)gridDim.x * blockDim.x) >> 5) {
+        int b = grp[g].begin;
+        int e = (g + 1 < ng) ? grp[g + 1].begin : (int)n;
+        double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY}, rmax = 0;
+        for (int p = b + lane; p < e; p += 32) {
+            double v[3] = {xs[p], ys[p], zs[p]};
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { lo[k] = fmin(lo[k], v[k]); hi[k] = fmax(hi[k], v[k]); }
+            rmax = fmax(rmax, rss[p]);
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                lo[k] = fmin(lo[k], __shfl_xor_sync(0xffffffffu, lo[k], o));
+                hi[k] = fmax(hi[k], __shfl_xor_sync(0xffffffffu, hi[k], o));
+            }
+            rmax = fmax(rmax, __shfl_xor_sync(0xffffffffu, rmax, o));
+        }
+        __syncwarp();
+        if (lane == 0) {          // (begin is left alone: the neighbouring warp reads it)
+            GroupRec* r = &grp[g];
+            r->end = e; r->head_sp = r->head_epn = r->head_epf = -1;
+            r->n_sp = r->n_epn = r->n_epf = 0; r->n_ep_part = r->n_epn_part = 0; r->pad0 = r->pad1 = 0;
+            for (int k = 0; k < 3; ++k) { r->lo[k] = lo[k]; r->hi[k] = hi[k]; }
+            r->rmax = rmax; r->pad2 = 0;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// device-wide exclusive scans (reduce -> scan of partials -> scan + add), 4096 elements per CTA
+// ------------------------------------------------------------------------------------------------
+#define SCAN_THREADS 1024
+#define SCAN_ITEMS 4
+template <typename T>
+__device__ __forceinline__ T block_excl_scan(T v, T* total_out, T* sbuf /* 32 */) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    T incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { T a = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += a; }
+    if (lane == 31) sbuf[w] = incl;
+    __syncthreads();
+    if (w == 0) {
+        T x = (lane < (int)(blockDim.x >> 5)) ? sbuf[lane] : (T)0;
+        T xi = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { T a = __shfl_up_sync(0xffffffffu, xi, o); if (lane >= o) xi += a; }
+        sbuf[lane] = xi - x;
+        if (lane == 31) *total_out = xi;
+    }
+    __syncthreads();
+    T r = sbuf[w] + incl - v;
+    __syncthreads();
+    return r;
+}
+
+template <typename TO>
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_reduce(const int* __restrict__ in, long long n, TO* __restrict__ part) {
+    __shared__ TO sbuf[32];
+    __shared__ TO tot;
+    long long base = (long long)blockIdx.x * SCAN_THREADS * SCAN_ITEMS + (long long)threadIdx.x * SCAN_ITEMS;
+    TO s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) if (base + k < n) s += (TO)in[base + k];
+    (void)block_excl_scan<TO>(s, &tot, sbuf);
+    if (threadIdx.x == 0) part[blockIdx.x] = tot;
+}
+template <typename TO>
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_partials(TO* __restrict__ part, int nblk) {
+    __shared__ TO sbuf[32];
+    __shared__ TO tot;
+    __shared__ TO carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < nblk; b0 += SCAN_THREADS) {
+        int b = b0 + threadIdx.x;
+        TO v = (b < nblk) ? part[b] : (TO)0;
+        TO ex = block_excl_scan<TO>(v, &tot, sbuf);
+        TO carry = carry_s;
+        if (b < nblk) part[b] = carry + ex;
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s = carry + tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[nblk] = carry_s;
+}
+template <typename TO>
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_final(const int* __restrict__ in, long long n, const TO* __restrict__ part,
+                                                             int nblk, TO* __restrict__ out) {
+    __shared__ TO sbuf[32];
+    __shared__ TO tot;
+    long long base = (long long)blockIdx.x * SCAN_THREADS * SCAN_ITEMS + (long long)threadIdx.x * SCAN_ITEMS;
+    int v[SCAN_ITEMS];
+    TO s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (base + k < n) ? in[base + k] : 0; s += (TO)v[k]; }
+    TO ex = block_excl_scan<TO>(s, &tot, sbuf) + part[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { if (base + k < n) out[base + k] = ex; ex += (TO)v[k]; }
+    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = part[nblk];
+}
+
+template <typename TO>
+static cudaError_t scan_impl(const int* in, TO* out, long long n, TO* tmp, cudaStream_t s) {
+    int nblk = cdiv(n, SCAN_THREADS * SCAN_ITEMS);
+    if (nblk < 1) nblk = 1;
+    k_scan_reduce<TO><<<nblk, SCAN_THREADS, 0, s>>>(in, n, tmp);
+    KCHECK(s, "k_scan_reduce");
+    k_scan_partials<TO><<<1, SCAN_THREADS, 0, s>>>(tmp, nblk);
+    KCHECK(s, "k_scan_partials");
+    k_scan_final<TO><<<nblk, SCAN_THREADS, 0, s>>>(in, n, tmp, nblk, out);
+    KCHECK(s, "k_scan_final");
+    petar_count_launch(3);
+    return cudaGetLastError();
+}
+cudaError_t launch_scan_i32(const int* in, int* out, int n, int* tmp, cudaStream_t s) { return scan_impl<int>(in, out, n, tmp, s); }
+cudaError_t launch_scan_i32_to_i64(const int* in, long long* out, long long n, long long* tmp, cudaStream_t s) {
+    return scan_impl<long long>(in, out, n, tmp, s);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host-side launch sequences
+// ------------------------------------------------------------------------------------------------
+cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s) {
+    Workspace& w = t->w;
+    const long long n = t->N;
+    stage_begin(t, s);
+    k_reset_header<<<1, 32, 0, s>>>(w.hdr);
+    KCHECK(s, "k_reset_header");
+    int g = min(cdiv(n, 256), t->sm_count * 8);
+    k_bbox<<<g, 256, 0, s>>>(t->x, t->y, t->z, t->m, t->r_out, t->r_search, n, w.hdr);
+    KCHECK(s, "k_bbox");
+    k_root<<<1, 32, 0, s>>>(w.hdr);
+    KCHECK(s, "k_root");
+    k_keys<<<cdiv(n, 256), 256, 0, s>>>(t->x, t->y, t->z, n, w.hdr, w.key, w.idx);
+    KCHECK(s, "k_keys");
+    petar_count_launch(4);
+    stage_end(t, PETAR_STAGE_BBOX_KEYS, s);
+
+    stage_begin(t, s);
+    const int nblk = cdiv(n, SORT_TILE);
+    {
+        cudaError_t e = cudaMemsetAsync(w.sort_hist, 0, 8 * 256 * sizeof(unsigned), s);
+        if (e != cudaSuccess) return e;
+    }
+    unsigned long long *kin = w.key, *kout = w.key_alt;
+    unsigned *vin = w.idx, *vout = w.idx_alt;
+    for (int pass = 0; pass < 8; ++pass) {
+        int shift = 8 * pass;
+        k_sort_count<<<nblk, SORT_THREADS, 0, s>>>(kin, n, shift, w.sort_blk, nblk, w.sort_hist + 256 * pass);
+        KCHECK(s, "k_sort_count");
+        k_sort_scan<<<256, 256, 0, s>>>(w.sort_blk, nblk, w.sort_hist + 256 * pass);
+        KCHECK(s, "k_sort_scan");
+        k_sort_scatter<<<nblk, SORT_THREADS, 0, s>>>(kin, vin, kout, vout, w.sort_blk, nblk, n, shift);
+        KCHECK(s, "k_sort_scatter");
+        unsigned long long* tk = kin; kin = kout; kout = tk;
+        unsigned* tv = vin; vin = vout; vout = tv;
+    }
+    petar_count_launch(24);
+    // 8 passes: the sorted data is back in (key, idx)
+    stage_end(t, PETAR_STAGE_SORT, s);
+
+    stage_begin(t, s);
+    k_gather<<<cdiv(n, 256), 256, 0, s>>>(w.idx, n, w.hdr, t->x, t->y, t->z, t->m, t->r_out, t->r_search,
+                                          w.xs, w.ys, w.zs, w.ms, w.routs, t->r_search ? w.rss : nullptr, w.pa, w.pb);
+    KCHECK(s, "k_gather");
+    petar_count_launch(1);
+    stage_end(t, PETAR_STAGE_GATHER, s);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_tree(petar_tree* t, cudaStream_t s) {
+    Workspace& w = t->w;
+    const long long n = t->N;
+    const int ntile = cdiv(n, RANK_THREADS);
+    stage_begin(t, s);
+    k_diverge<<<cdiv(n + 1, 256), 256, 0, s>>>(w.key, n, w.D);
+    KCHECK(s, "k_diverge");
+    size_t sh = DEPTH_THREADS + 2 * t->p.n_group_limit + 1;
+    k_depth<<<cdiv(n, DEPTH_THREADS), DEPTH_THREADS, sh, s>>>(w.key, w.D, n, t->p.n_leaf_limit, t->p.n_group_limit, w.depth, w.glevel, w.gflag);
+    KCHECK(s, "k_depth");
+    k_rank_count<<<ntile, RANK_THREADS, 0, s>>>(w.D, w.depth, n, w.tile_cnt, ntile);
+    KCHECK(s, "k_rank_count");
+    k_rank_scan<<<1, 1024, 0, s>>>(w.tile_cnt, ntile, w.hdr, w.node_cap);
+    KCHECK(s, "k_rank_scan");
+    k_nodes_write<<<ntile, RANK_THREADS, 0, s>>>(w.key, w.D, w.depth, n, w.tile_cnt, ntile, w.hdr, w.nint, w.node_cap);
+    KCHECK(s, "k_nodes_write");
+    petar_count_launch(5);
+    stage_end(t, PETAR_STAGE_TREE, s);
+
+    stage_begin(t, s);
+    {
+        int per_sm = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moments, 256, 0);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) per_sm = 1;
+        if (per_sm > 4) per_sm = 4;
+        int grid = t->sm_count * per_sm;
+        const DevHeader* hdr = w.hdr;
+        const double* rss = t->r_search ? w.rss : w.routs;
+        int cap = w.node_cap, mult = t->p.multipole;
+        void* args[] = {(void*)&hdr, (void*)&w.nint, (void*)&w.nmac, (void*)&w.nmom, (void*)&w.nsp, (void*)&w.key,
+                        (void*)&w.xs, (void*)&w.ys, (void*)&w.zs, (void*)&w.ms, (void*)&rss, (void*)&cap, (void*)&mult};
+        e = cudaLaunchCooperativeKernel((void*)k_moments, dim3(grid), dim3(256), args, 0, s);
+        if (e != cudaSuccess) return e;
+        KCHECK(s, "k_moments");
+        petar_count_launch(1);
+    }
+    stage_end(t, PETAR_STAGE_MOMENTS, s);
+
+    stage_begin(t, s);
+    cudaError_t e = launch_scan_i32(w.gflag, w.gflag + (n + 1), (int)n, w.scan_tmp, s);
+    if (e != cudaSuccess) return e;
+    k_groups_begin<<<cdiv(n, 256), 256, 0, s>>>(w.gflag, w.gflag + (n + 1), n, w.grp, w.hdr);
+    KCHECK(s, "k_groups_begin");
+    k_groups_finish<<<min(cdiv(n, 8), t->sm_count * 16), 256, 0, s>>>(w.grp, w.hdr, n, w.xs, w.ys, w.zs, t->r_search ? w.rss : w.routs);
+    KCHECK(s, "k_groups_finish");
+    petar_count_launch(2);
+    stage_end(t, PETAR_STAGE_GROUPS, s);
+    return cudaGetLastError();
+}

@@ -1,0 +1,288 @@
+// force.cu -- step S8: fp32 pairwise force + potential over the walk's lists (rule O8), with the
+// changeover weights 1-K (Eq. 17) and 1-W (Eq. 15) on near EP pairs.
+//
+// One CTA (128 threads) per i-group, groups pulled from a device ticket (persistent CTAs).
+// Thread mapping: the group's n_i particles are taken two per thread ("pair slot" p = t % P,
+// P = ceil(n_i/2)); the remaining factor of the CTA, S = 128 / P, splits every j-tile into S
+// interleaved slices (slice s = t / P handles j = s, s+S, ...).  This keeps >= 80 % of the lanes busy
+// for any n_i in 1..64 and halves the shared-memory reads per interaction.
+//
+// Precision: positions are float-float (hi + lo) relative to the root-cube centre; a pair's
+// displacement is (xjh - xih) + (xjl - xil), which is the pair-relative coordinate to ~1e-7
+// relative accuracy whatever the distance from the origin.  fp32
+// partial sums live only across one tile slice and are flushed into fp64 accumulators per tile.
+#include "internal.cuh"
+
+#define FT 128                 // threads per CTA
+#define SP_TILE 256            // cells per staged tile
+#define EP_TILE 512            // particles per staged tile
+#define EP_BATCH FT            // EP ranges expanded per batch (one per thread)
+
+struct ForceConst {
+    float c1, c0;              // x = r * inv_R * c1 - c0,  c1 = 1/(1-rho), c0 = rho/(1-rho)
+    float lam, one_plus_lam;   // Lambda = (1-rho)/(1+rho) (Eq. 16), 1 + Lambda
+    float b0, b1, b2, b3, b4;  // 1-K = x^4 (b0 + b1 x + b2 x^2 + b3 x^3 + b4 x^4)   (form B, x < 1/2)
+    float a4;                  // 35 Lambda: K = (1-x)^4 (1 + 4x + 10x^2 + 20x^3 + a4 x^4) (form A, x >= 1/2)
+};
+
+struct IPart {
+    float xh, yh, zh, xl, yl, zl, inv_ro;
+    float ax, ay, az, pot;     // fp32 partial sums of the current tile slice
+};
+
+__device__ __forceinline__ void sp_interact(IPart& p, const float4 a, const float4 b, const float4 c, const bool quad) {
+    // d = com - x_i  (points to the source)
+    const float dx = (a.x - p.xh) + (b.x - p.xl);
+    const float dy = (a.y - p.yh) + (b.y - p.yl);
+    const float dz = (a.z - p.zh) + (b.z - p.zl);
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const float rinv = rsqrtf(r2);
+    const float rinv2 = rinv * rinv;
+    const float mr = a.w * rinv;
+    if (!quad) {
+        const float f = mr * rinv2;
+        p.pot -= mr;
+        p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
+    } else {
+        // A = traceless quadrupole: (Axx, Ayy, Azz = -(Axx+Ayy), Axy, Axz, Ayz) = (b.w, c.x, -, c.y, c.z, c.w)
+        const float azz = -(b.w + c.x);
+        const float adx = fmaf(b.w, dx, fmaf(c.y, dy, c.z * dz));
+        const float ady = fmaf(c.y, dx, fmaf(c.x, dy, c.w * dz));
+        const float adz = fmaf(c.z, dx, fmaf(c.w, dy, azz * dz));
+        const float dad = fmaf(dx, adx, fmaf(dy, ady, dz * adz));
+        const float rinv3 = rinv * rinv2, rinv5 = rinv3 * rinv2;
+        const float q5 = dad * rinv5;                  // d^T A d / r^5
+        p.pot -= mr + q5;                              // phi = -[M/r + d^T A d / r^5]
+        const float f = fmaf(5.0f * q5, rinv2, mr * rinv2);   // M/r^3 + 5 dAd / r^7
+        const float g = -2.0f * rinv5;
+        p.ax = fmaf(f, dx, fmaf(g, adx, p.ax));
+        p.ay = fmaf(f, dy, fmaf(g, ady, p.ay));
+        p.az = fmaf(f, dz, fmaf(g, adz, p.az));
+    }
+}
+
+template <bool NEAR>
+__device__ __forceinline__ void ep_interact(IPart& p, const float4 a, const float4 b, const ForceConst& k) {
+    const float dx = (a.x - p.xh) + (b.x - p.xl);
+    const float dy = (a.y - p.yh) + (b.y - p.yl);
+    const float dz = (a.z - p.zh) + (b.z - p.zl);
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const float rinv = (r2 > 0.0f) ? rsqrtf(r2) : 0.0f;     // self / coincident pair: no force
+    const float rinv2 = rinv * rinv;
+    if (!NEAR) {
+        const float mr = a.w * rinv;
+        const float f = mr * rinv2;
+        p.pot -= mr;
+        p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
+    } else {
+        const float inv_R = fminf(p.inv_ro, b.w);           // 1 / max(r_out,i, r_out,j)
+        const float r = r2 * rinv;
+        const float x = fmaf(r * inv_R, k.c1, -k.c0);
+        const float xc = __saturatef(x);
+        const float x2 = xc * xc, x4 = x2 * x2;
+        // 1 - K: form B below 1/2 (no cancellation at small x), form A above (K itself is small there)
+        const float qb = fmaf(fmaf(fmaf(fmaf(k.b4, xc, k.b3), xc, k.b2), xc, k.b1), xc, k.b0);
+        const float wb = x4 * qb;
+        const float y = 1.0f - xc, y2 = y * y, y4 = y2 * y2;
+        const float pa = fmaf(fmaf(fmaf(fmaf(k.a4, xc, 20.0f), xc, 10.0f), xc, 4.0f), xc, 1.0f);
+        const float wa = fmaf(-y4, pa, 1.0f);
+        const float wk = (xc < 0.5f) ? wb : wa;
+        // (1 - W)/r = (1+Lambda)/R - Lambda x^5 (14 - 28x + 20x^2 - 5x^3)/r  for r < R, 1/r beyond
+        const float gp = x4 * xc * fmaf(fmaf(fmaf(-5.0f, xc, 20.0f), xc, -28.0f), xc, 14.0f);
+        const float pw = (x < 1.0f) ? fmaf(-k.lam * gp, rinv, k.one_plus_lam * inv_R) : rinv;
+        p.pot = fmaf(-a.w, pw, p.pot);
+        const float f = a.w * wk * rinv * rinv2;
+        p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
+    }
+}
+
+struct Acc64 { double ax, ay, az, pot; };
+__device__ __forceinline__ void flush(IPart& p, Acc64& a) {
+    a.ax += (double)p.ax; a.ay += (double)p.ay; a.az += (double)p.az; a.pot += (double)p.pot;
+    p.ax = p.ay = p.az = p.pot = 0.0f;
+}
+
+union __align__(16) ForceSmem {
+    struct { float4 q0[SP_TILE], q1[SP_TILE], q2[SP_TILE]; } sp;      // 12 KB
+    struct { float4 a[EP_TILE], b[EP_TILE]; } ep;                      // 16 KB
+    double red[FT * 8];                                                // 8 KB
+};
+
+template <bool QUAD>
+__global__ void __launch_bounds__(FT) k_force(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
+                                              const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
+                                              const unsigned* __restrict__ perm, const double* __restrict__ ms, const double* __restrict__ routs,
+                                              double* __restrict__ oax, double* __restrict__ oay, double* __restrict__ oaz, double* __restrict__ opot,
+                                              ForceConst fc, double G, double one_plus_lam64) {
+    __shared__ ForceSmem sm;
+    __shared__ int s_g;
+    __shared__ int s_scan[FT / 32 + 1];
+    const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
+    const int ng = h->n_groups;
+    for (;;) {
+        __syncthreads();
+        if (t == 0) s_g = atomicAdd(&h->group_ticket2, 1);
+        __syncthreads();
+        const int g = s_g;
+        if (g >= ng) break;
+        const GroupRec* gr = &grp[g];
+        const int gb = gr->begin, n_i = gr->end - gb;
+        const int P = (n_i + 1) >> 1;
+        const int S = FT / P;
+        const int pslot = t % P, slice = t / P;
+        const bool active = slice < S;
+        IPart ip[2];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            int i = gb + 2 * pslot + q;
+            if (i >= gb + n_i) i = gb + n_i - 1;         // odd n_i: duplicate the last particle (result dropped)
+            float4 a = pa[i], b = pb[i];
+            ip[q].xh = a.x; ip[q].yh = a.y; ip[q].zh = a.z; ip[q].xl = b.x; ip[q].yl = b.y; ip[q].zl = b.z; ip[q].inv_ro = b.w;
+            ip[q].ax = ip[q].ay = ip[q].az = ip[q].pot = 0.0f;
+        }
+        Acc64 acc[2] = {{0, 0, 0, 0}, {0, 0, 0, 0}};
+
+        // ---- super-particles -----------------------------------------------------------------
+        {
+            int chunk = gr->head_sp, remaining = gr->n_sp;
+            while (chunk >= 0 && remaining > 0) {
+                const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
+                const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+                for (int off = 0; off < ne; off += SP_TILE) {
+                    const int tn = min(SP_TILE, ne - off);
+                    __syncthreads();
+                    for (int k = t; k < tn; k += FT) {
+                        const int id = cp[PETAR_CHUNK_HDR + off + k];
+                        const NodeSp* s = &nsp[id];
+                        sm.sp.q0[k] = s->q0; sm.sp.q1[k] = s->q1;
+                        if (QUAD) sm.sp.q2[k] = s->q2;
+                    }
+                    __syncthreads();
+                    if (active) {
+                        for (int j = slice; j < tn; j += S) {
+                            const float4 a = sm.sp.q0[j], b = sm.sp.q1[j];
+                            float4 c = make_float4(0.f, 0.f, 0.f, 0.f);
+                            if (QUAD) c = sm.sp.q2[j];
+                            sp_interact(ip[0], a, b, c, QUAD);
+                            sp_interact(ip[1], a, b, c, QUAD);
+                        }
+                        flush(ip[0], acc[0]); flush(ip[1], acc[1]);
+                    }
+                }
+                remaining -= ne;
+                chunk = cp[0];
+            }
+        }
+        // ---- particles: near ranges (changeover) then far ranges (plain Newtonian) ----------------
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            int chunk = pass == 0 ? gr->head_epn : gr->head_epf;
+            int remaining = 2 * (pass == 0 ? gr->n_epn : gr->n_epf);
+            while (chunk >= 0 && remaining > 0) {
+                const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
+                const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+                for (int off = 0; off < ne; off += 2 * EP_BATCH) {
+                    // one range per thread, block scan of the range sizes
+                    int jb = 0, cnt = 0;
+                    if (off + 2 * t < ne) { jb = cp[PETAR_CHUNK_HDR + off + 2 * t]; cnt = cp[PETAR_CHUNK_HDR + off + 2 * t + 1] - jb; }
+                    int incl = cnt;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
+                    __syncthreads();                       // previous tile consumed; s_scan free
+                    if (lane == 31) s_scan[wrp] = incl;
+                    __syncthreads();
+                    int woff = 0, total = 0;
+#pragma unroll
+                    for (int ww = 0; ww < FT / 32; ++ww) { int v = s_scan[ww]; if (ww < wrp) woff += v; total += v; }
+                    const int my0 = woff + incl - cnt;     // exclusive offset of my range
+                    for (int w0 = 0; w0 < total; w0 += EP_TILE) {
+                        if (w0) __syncthreads();
+                        const int lo = max(my0, w0), hi = min(my0 + cnt, w0 + EP_TILE);
+                        for (int q = lo; q < hi; ++q) {
+                            const int j = jb + (q - my0);
+                            sm.ep.a[q - w0] = pa[j]; sm.ep.b[q - w0] = pb[j];
+                        }
+                        __syncthreads();
+                        const int tn = min(EP_TILE, total - w0);
+                        if (active) {
+                            if (pass == 0) {
+                                for (int j = slice; j < tn; j += S) {
+                                    const float4 a = sm.ep.a[j], b = sm.ep.b[j];
+                                    ep_interact<true>(ip[0], a, b, fc);
+                                    ep_interact<true>(ip[1], a, b, fc);
+                                }
+                            } else {
+                                for (int j = slice; j < tn; j += S) {
+                                    const float4 a = sm.ep.a[j], b = sm.ep.b[j];
+                                    ep_interact<false>(ip[0], a, b, fc);
+                                    ep_interact<false>(ip[1], a, b, fc);
+                                }
+                            }
+                            flush(ip[0], acc[0]); flush(ip[1], acc[1]);
+                        }
+                    }
+                }
+                remaining -= ne;
+                chunk = cp[0];
+            }
+        }
+        // ---- ordered reduction over slices, then scatter to the caller's order --------------------
+        __syncthreads();
+        if (active) {
+            double* r = &sm.red[(size_t)(slice * (2 * P) + 2 * pslot) * 4];
+            r[0] = acc[0].ax; r[1] = acc[0].ay; r[2] = acc[0].az; r[3] = acc[0].pot;
+            r[4] = acc[1].ax; r[5] = acc[1].ay; r[6] = acc[1].az; r[7] = acc[1].pot;
+        }
+        __syncthreads();
+        for (int k = t; k < n_i * 4; k += FT) {
+            const int i = k >> 2, comp = k & 3;
+            double s = 0.0;
+            for (int sl = 0; sl < S; ++sl) s += sm.red[(size_t)(sl * (2 * P) + i) * 4 + comp];
+            const int ig = gb + i;
+            const unsigned o = perm[ig];
+            if (comp == 3) {
+                // the list contains the particle itself: remove its constant self term (reading P4)
+                s += ms[ig] * one_plus_lam64 / routs[ig];
+                if (opot) opot[o] = G * s;
+            } else {
+                double* dst = comp == 0 ? oax : comp == 1 ? oay : oaz;
+                if (dst) dst[o] = G * s;
+            }
+        }
+    }
+}
+
+__global__ void k_reset_ticket2(DevHeader* h) { if (threadIdx.x == 0) h->group_ticket2 = 0; }
+
+cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s) {
+    Workspace& w = t->w;
+    const double rho = t->p.r_in_over_r_out;
+    const double lam = (1.0 - rho) / (1.0 + rho);
+    ForceConst fc;
+    fc.c1 = (float)(1.0 / (1.0 - rho)); fc.c0 = (float)(rho / (1.0 - rho));
+    fc.lam = (float)lam; fc.one_plus_lam = (float)(1.0 + lam);
+    fc.b0 = (float)(35.0 * (1.0 - lam));
+    fc.b1 = (float)(56.0 * lam - 84.0 * (1.0 - lam));
+    fc.b2 = (float)(70.0 * (1.0 - lam) - 140.0 * lam);
+    fc.b3 = (float)(120.0 * lam - 20.0 * (1.0 - lam));
+    fc.b4 = (float)(-35.0 * lam);
+    fc.a4 = (float)(35.0 * lam);
+    stage_begin(t, s);
+    k_reset_ticket2<<<1, 32, 0, s>>>(w.hdr);
+    KCHECK(s, "k_reset_ticket2");
+    int per_sm = 0;
+    cudaError_t e;
+    if (t->p.multipole >= 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<true>, FT, 0);
+    else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<false>, FT, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    const int grid = t->sm_count * per_sm;
+    if (t->p.multipole >= 2)
+        k_force<true><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.ms, w.routs, ax, ay, az, pot, fc, t->p.G, 1.0 + lam);
+    else
+        k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.ms, w.routs, ax, ay, az, pot, fc, t->p.G, 1.0 + lam);
+    KCHECK(s, "k_force");
+    petar_count_launch(2);
+    stage_end(t, PETAR_STAGE_FORCE, s);
+    return cudaGetLastError();
+}

@@ -1,0 +1,117 @@
+// internal.cuh -- shared declarations of the CUDA path (host handle, HBM layout, launch wrappers).
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/petar.h"
+
+#define PETAR_MAXLEVEL 21
+#define PETAR_NLEVELS 22           // levels 0..21
+#define PETAR_CHUNK 1024           // list arena chunk, in 4-byte entries; [0] = next chunk (or -1), [1] unused
+#define PETAR_CHUNK_HDR 2
+#define PETAR_CHUNK_PAYLOAD (PETAR_CHUNK - PETAR_CHUNK_HDR)   // 1022 entries (even: EP ranges are pairs)
+
+// ---- device-resident header (one per tree, lives at the start of the workspace) -----------------
+struct DevHeader {
+    // encoded bounding box (ordered-uint encoding of doubles) : min x,y,z ; max x,y,z
+    unsigned long long bbox[6];
+    double c[3];        // root cube centre (O1)
+    double h;           // half edge, power of two
+    double o[3];        // origin c - h
+    double inv_s;       // 2^21 / (2h)
+    int n_nodes;
+    int n_groups;
+    int status;         // PETAR_ST_* bits
+    int arena_top;      // next free chunk index
+    int level_off[PETAR_NLEVELS + 2];   // node id range of level l: [level_off[l], level_off[l+1])
+    int group_ticket;   // dynamic scheduling counters (reset before each consumer kernel)
+    int group_ticket2;
+    int group_ticket3;
+    int pad_;
+    unsigned long long n_epep, n_epsp, n_epep_near, n_ep_list, n_sp_list;
+    unsigned long long nb_total;
+};
+
+// node integer record: begin, end, first_child, meta = level | nchild<<8 | leaf<<16 | firstflag<<17
+struct __align__(16) NodeInt { int begin, end, first_child, meta; };
+// MAC record (fp64, exact decisions): lo[3], hi[3], com[3], rmax  -> 10 doubles = 80 B
+struct __align__(16) NodeMac { double lo[3]; double hi[3]; double com[3]; double rmax; };
+// moments kept for the bottom-up pass / export
+struct __align__(16) NodeMom { double M; double S[3]; double Q[6]; };
+// fp32 super-particle record for the force kernel: 12 floats = 48 B
+//  q0 = (xh, yh, zh, M) ; q1 = (xl, yl, zl, Axx) ; q2 = (Ayy, Axy, Axz, Ayz) ;  Azz = -(Axx + Ayy)
+//  (xh + xl) = com - c_root in float-float; A = 1.5 Q - 0.5 tr(Q) I  (Eq. 31, traceless)
+struct __align__(16) NodeSp { float4 q0, q1, q2; };
+
+struct __align__(16) GroupRec {
+    int begin, end;
+    int head_sp, head_epn, head_epf;   // first chunk of each list (-1 = empty)
+    int n_sp, n_epn, n_epf;            // entries: cells, near ranges, far ranges
+    int n_ep_part, n_epn_part;         // particles in all EP ranges / in near ranges
+    int pad0, pad1;
+    double lo[3], hi[3], rmax;
+    double pad2;
+};
+
+struct Workspace {
+    DevHeader* hdr;
+    // sort buffers
+    unsigned long long *key, *key_alt;
+    unsigned int *idx, *idx_alt;
+    unsigned int *sort_hist;       // [8][256] global digit totals, then per-pass block counts
+    unsigned int *sort_blk;        // [256][nblk]
+    // sorted particle data
+    double *xs, *ys, *zs, *ms, *routs, *rss;
+    float4 *pa, *pb;               // (xh,yh,zh,m) , (xl,yl,zl,1/r_out)
+    signed char *D;                // [N+1] shared leading octal digits of keys i-1, i
+    signed char *depth;            // [N] leaf level of particle i
+    signed char *glevel;           // [N] group level
+    int *gflag;                    // [N] group-start flags -> scanned
+    int *tile_cnt;                 // [22][ntile]
+    int *scan_tmp;                 // scan partials
+    // nodes
+    NodeInt* nint; NodeMac* nmac; NodeMom* nmom; NodeSp* nsp;
+    int node_cap;
+    // groups
+    GroupRec* grp; int group_cap;
+    // list arena
+    int* arena; int arena_chunks;
+    // neighbour temporaries
+    int* nb_cnt;                   // [N] counts in caller's order
+    int* exp_scratch;              // [10 (N+1) + 8] list-export scratch (tests)
+};
+
+struct petar_tree {
+    uint32_t magic;
+    int64_t N;
+    petar_params p;
+    Workspace w;
+    const double *x, *y, *z, *m, *r_out, *r_search;
+    bool built, walked;
+    float stage_ms[PETAR_N_STAGES];
+    int sm_count;
+    int* pinned;                   // small pinned host buffer for header read-back
+};
+
+#define PETAR_MAGIC 0x50335431u
+
+// launch wrappers (each returns cudaError_t of the launch)
+cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s);
+cudaError_t launch_tree(petar_tree* t, cudaStream_t s);
+cudaError_t launch_walk(petar_tree* t, cudaStream_t s);
+cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s);
+cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity,
+                             int32_t* status_dev, cudaStream_t s);
+cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_bytes, cudaStream_t s);
+// device-wide exclusive scan: out[i] = sum_{j<i} in[j], out has n+1 entries (out[n] = total)
+cudaError_t launch_scan_i32(const int* in, int* out, int n, int* tmp, cudaStream_t s);
+cudaError_t launch_scan_i32_to_i64(const int* in, long long* out, long long n, long long* tmp, cudaStream_t s);
+
+void petar_count_launch(int n);
+// PETAR_DEBUG_SYNC=1 in the environment: synchronise after every kernel and report the first failing one
+void petar_debug_check(cudaStream_t s, const char* name);
+#define KCHECK(s, name) petar_debug_check(s, name)
+void stage_begin(petar_tree* t, cudaStream_t s);
+void stage_end(petar_tree* t, int stage, cudaStream_t s);
+
+static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }

@@ -1,0 +1,349 @@
+// walk.cu -- step S7 (per-group interaction-list walk, rule O7), step S9 (neighbour-list writer,
+// rule O9) and the list export used by the tests.  Compiled with -fmad=false: the MAC and the
+// neighbour test are fp64 with exactly the operation order of DESIGN.md O7 / O9 (fma where written).
+#include "internal.cuh"
+
+#define WALK_WARPS 8
+#define WALK_STACK 1536          // frontier entries per warp (shared memory)
+
+// warp-uniform cursor of one chunked list
+struct ListCursor {
+    int head;      // first chunk or -1
+    int chunk;     // current chunk or -1
+    int pos;       // payload entries used in the current chunk
+    int dead;      // arena exhausted
+};
+
+// Appends `per` entries (1 or 2) for every lane with `take` set.  v0/v1 are the lane's entries.
+__device__ __forceinline__ void list_append(ListCursor& c, bool take, int per, int v0, int v1, int* __restrict__ arena,
+                                            int arena_chunks, DevHeader* __restrict__ h, int lane) {
+    const unsigned mask = __ballot_sync(0xffffffffu, take);
+    if (mask == 0u || c.dead) return;
+    const int n = __popc(mask);
+    int off = __popc(mask & ((1u << lane) - 1u)) * per;        // my first slot relative to c.pos
+    int space = (c.chunk >= 0) ? (PETAR_CHUNK_PAYLOAD - c.pos) : 0;
+    // part 1: what fits into the current chunk
+    if (take && off < space) {
+        int* p = arena + (size_t)c.chunk * PETAR_CHUNK + PETAR_CHUNK_HDR + c.pos + off;
+        p[0] = v0;
+        if (per == 2) p[1] = v1;
+    }
+    if (n * per <= space) { c.pos += n * per; return; }
+    // part 2: new chunk for the rest
+    int nc = 0;
+    if (lane == 0) {
+        nc = atomicAdd(&h->arena_top, 1);
+        if (nc >= arena_chunks) { atomicOr(&h->status, PETAR_ST_LIST_CAP); nc = -1; }
+        else {
+            arena[(size_t)nc * PETAR_CHUNK] = -1;
+            if (c.chunk >= 0) arena[(size_t)c.chunk * PETAR_CHUNK] = nc;
+        }
+    }
+    nc = __shfl_sync(0xffffffffu, nc, 0);
+    if (nc < 0) { c.dead = 1; return; }
+    if (c.chunk < 0) c.head = nc;
+    c.chunk = nc;
+    if (take && off >= space) {
+        int* p = arena + (size_t)nc * PETAR_CHUNK + PETAR_CHUNK_HDR + (off - space);
+        p[0] = v0;
+        if (per == 2) p[1] = v1;
+    }
+    c.pos = n * per - space;
+}
+
+__global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict__ h, const NodeInt* __restrict__ nint,
+                                                          const NodeMac* __restrict__ nmac, GroupRec* __restrict__ grp,
+                                                          int* __restrict__ arena, int arena_chunks, double theta, int node_cap) {
+    __shared__ int s_stack[WALK_WARPS][WALK_STACK];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int* stack = s_stack[w];
+    const int ng = h->n_groups;
+    if (h->n_nodes > node_cap || h->n_nodes <= 0) return;
+    const double theta2 = theta * theta;
+    const double twoh = 2.0 * h->h;
+    unsigned long long t_epep = 0, t_epsp = 0, t_near = 0, t_eplist = 0, t_splist = 0;
+    for (;;) {
+        int g = 0;
+        if (lane == 0) g = atomicAdd(&h->group_ticket, 1);
+        g = __shfl_sync(0xffffffffu, g, 0);
+        if (g >= ng) break;
+        const GroupRec* gr = &grp[g];
+        const double glo0 = gr->lo[0], glo1 = gr->lo[1], glo2 = gr->lo[2];
+        const double ghi0 = gr->hi[0], ghi1 = gr->hi[1], ghi2 = gr->hi[2];
+        const double grmax = gr->rmax;
+        const int n_i = gr->end - gr->begin;
+        ListCursor lsp = {-1, -1, 0, 0}, lepn = {-1, -1, 0, 0}, lepf = {-1, -1, 0, 0};
+        int n_sp = 0, n_epn = 0, n_epf = 0, n_ep_part = 0, n_epn_part = 0;
+        int top = 1;
+        if (lane == 0) stack[0] = 0;
+        __syncwarp();
+        while (top > 0) {
+            int p = min(32, top);
+            if (top - p + 8 * p > WALK_STACK) p = max(1, (WALK_STACK - top) / 7);
+            const int node = (lane < p) ? stack[top - p + lane] : -1;
+            top -= p;
+            __syncwarp();
+            int act = -1;                      // 0 SP, 1 EP near, 2 EP far, 3 open
+            int nb = 0, ne = 0, fc = 0, nch = 0;
+            if (node >= 0) {
+                const NodeInt ni = nint[node];
+                const NodeMac c = nmac[node];
+                const int level = ni.meta & 255;
+                const bool leaf = (ni.meta >> 16) & 1;
+                // O7, exactly this operation order
+                double gx = fmax(0.0, fmax(c.lo[0] - ghi0, glo0 - c.hi[0]));
+                double gy = fmax(0.0, fmax(c.lo[1] - ghi1, glo1 - c.hi[1]));
+                double gz = fmax(0.0, fmax(c.lo[2] - ghi2, glo2 - c.hi[2]));
+                double d2box = fma(gz, gz, fma(gy, gy, gx * gx));
+                double R = fmax(grmax, c.rmax);
+                bool nearb = d2box < R * R;
+                double px = fmax(0.0, fmax(glo0 - c.com[0], c.com[0] - ghi0));
+                double py = fmax(0.0, fmax(glo1 - c.com[1], c.com[1] - ghi1));
+                double pz = fmax(0.0, fmax(glo2 - c.com[2], c.com[2] - ghi2));
+                double d2com = fma(pz, pz, fma(py, py, px * px));
+                double edge = ldexp(twoh, -level);
+                bool farb = (edge * edge) < theta2 * d2com;
+                nb = ni.begin; ne = ni.end; fc = ni.first_child; nch = (ni.meta >> 8) & 15;
+                if (!nearb && farb) act = 0;
+                else if (leaf) act = nearb ? 1 : 2;
+                else act = 3;
+            }
+            // outputs
+            list_append(lsp, act == 0, 1, node, 0, arena, arena_chunks, h, lane);
+            list_append(lepn, act == 1, 2, nb, ne, arena, arena_chunks, h, lane);
+            list_append(lepf, act == 2, 2, nb, ne, arena, arena_chunks, h, lane);
+            n_sp += __popc(__ballot_sync(0xffffffffu, act == 0));
+            n_epn += __popc(__ballot_sync(0xffffffffu, act == 1));
+            n_epf += __popc(__ballot_sync(0xffffffffu, act == 2));
+            int cn = (act == 1) ? (ne - nb) : 0, cf = (act == 2) ? (ne - nb) : 0;
+            int push = (act == 3) ? nch : 0;
+            int pref = push;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                cn += __shfl_xor_sync(0xffffffffu, cn, o);
+                cf += __shfl_xor_sync(0xffffffffu, cf, o);
+                int a = __shfl_up_sync(0xffffffffu, pref, o);
+                if (lane >= o) pref += a;
+            }
+            n_epn_part += cn; n_ep_part += cn + cf;
+            const int total_push = __shfl_sync(0xffffffffu, pref, 31);
+            if (top + total_push > WALK_STACK) {                 // never expected
+                if (lane == 0) atomicOr(&h->status, PETAR_ST_STACK);
+                top = 0;
+                break;
+            }
+            const int at = top + pref - push;
+            for (int k = 0; k < push; ++k) stack[at + k] = fc + k;
+            top += total_push;
+            __syncwarp();
+        }
+        if (lane == 0) {
+            GroupRec* go = &grp[g];
+            go->head_sp = lsp.head; go->head_epn = lepn.head; go->head_epf = lepf.head;
+            go->n_sp = n_sp; go->n_epn = n_epn; go->n_epf = n_epf;
+            go->n_ep_part = n_ep_part; go->n_epn_part = n_epn_part;
+        }
+        t_epep += (unsigned long long)n_i * (unsigned long long)n_ep_part;
+        t_near += (unsigned long long)n_i * (unsigned long long)n_epn_part;
+        t_epsp += (unsigned long long)n_i * (unsigned long long)n_sp;
+        t_eplist += (unsigned long long)(n_epn + n_epf);
+        t_splist += (unsigned long long)n_sp;
+    }
+    if (lane == 0) {
+        atomicAdd(&h->n_epep, t_epep); atomicAdd(&h->n_epsp, t_epsp); atomicAdd(&h->n_epep_near, t_near);
+        atomicAdd(&h->n_ep_list, t_eplist); atomicAdd(&h->n_sp_list, t_splist);
+    }
+}
+
+__global__ void k_reset_ticket(DevHeader* h, int which) {
+    if (threadIdx.x == 0) { if (which == 0) { h->group_ticket = 0; h->arena_top = 0; h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = 0ull; } else h->group_ticket3 = 0; }
+}
+
+cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
+    Workspace& w = t->w;
+    stage_begin(t, s);
+    k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 0);
+    KCHECK(s, "k_reset_ticket");
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_walk, WALK_WARPS * 32, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    k_walk<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nint, w.nmac, w.grp, w.arena, w.arena_chunks, t->p.theta, w.node_cap);
+    KCHECK(s, "k_walk");
+    petar_count_launch(2);
+    stage_end(t, PETAR_STAGE_WALK, s);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// S9: neighbours.  One warp per group; lanes own i-particles; j runs over the NEAR EP ranges only
+// (a leaf that is not near has every pair at r >= R_ij, rule O7), fp64 test of rule O9.
+// Pass 1 counts into cnt[original index]; pass 2 (after the scan) fills.
+// ------------------------------------------------------------------------------------------------
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
+                                                   const unsigned* __restrict__ perm,
+                                                   const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
+                                                   const double* __restrict__ rss, int* __restrict__ cnt,
+                                                   const long long* __restrict__ offsets, int* __restrict__ indices, long long capacity) {
+    const int lane = threadIdx.x & 31;
+    const int ng = h->n_groups;
+    for (;;) {
+        int g = 0;
+        if (lane == 0) g = atomicAdd(&h->group_ticket3, 1);
+        g = __shfl_sync(0xffffffffu, g, 0);
+        if (g >= ng) break;
+        const GroupRec gr = grp[g];
+        for (int ib = gr.begin; ib < gr.end; ib += 32) {
+            const int i = ib + lane;
+            const bool vi = i < gr.end;
+            double xi = 0, yi = 0, zi = 0, ri = 0;
+            unsigned oi = 0;
+            long long o = 0;
+            if (vi) { xi = xs[i]; yi = ys[i]; zi = zs[i]; ri = rss[i]; oi = perm[i]; if (FILL) o = offsets[oi]; }
+            int c = 0;
+            int chunk = gr.head_epn;
+            int remaining = gr.n_epn * 2;       // entries
+            while (chunk >= 0 && remaining > 0) {
+                const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
+                const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+                for (int e = 0; e < ne; e += 2) {
+                    const int jb = cp[PETAR_CHUNK_HDR + e], je = cp[PETAR_CHUNK_HDR + e + 1];
+                    for (int j = jb; j < je; ++j) {
+                        double xj = xs[j], yj = ys[j], zj = zs[j], rj = rss[j];   // warp-uniform loads
+                        double dx = xi - xj, dy = yi - yj, dz = zi - zj;
+                        double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                        double R = fmax(ri, rj);
+                        if (vi && j != i && r2 < R * R) {
+                            if (FILL) { if (o + c < capacity) indices[o + c] = (int)perm[j]; }
+                            ++c;
+                        }
+                    }
+                }
+                remaining -= ne;
+                chunk = cp[0];
+            }
+            if (!FILL && vi) cnt[oi] = c;
+        }
+    }
+}
+
+__global__ void k_nb_status(const long long* __restrict__ offsets, long long n, long long capacity, int* __restrict__ status_dev,
+                            DevHeader* __restrict__ h, int have_indices) {
+    if (threadIdx.x == 0) {
+        long long tot = offsets[n];
+        h->nb_total = (unsigned long long)tot;
+        int over = (have_indices && tot > capacity) ? 1 : 0;
+        if (status_dev) *status_dev = over;
+        if (over) atomicOr(&h->status, PETAR_ST_NB_CAP);
+    }
+}
+
+cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity, int32_t* status_dev, cudaStream_t s) {
+    Workspace& w = t->w;
+    const long long n = t->N;
+    const double* rss = t->r_search ? w.rss : w.routs;
+    stage_begin(t, s);
+    int grid = t->sm_count * 8;
+    k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 1);
+    KCHECK(s, "k_reset_ticket");
+    k_neighbors<false><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, nullptr, nullptr, 0);
+    KCHECK(s, "k_neighbors");
+    petar_count_launch(2);
+    cudaError_t e = launch_scan_i32_to_i64(w.nb_cnt, (long long*)offsets, n, (long long*)w.scan_tmp, s);
+    if (e != cudaSuccess) return e;
+    if (indices) {
+        k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 1);
+        KCHECK(s, "k_reset_ticket");
+        k_neighbors<true><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, (const long long*)offsets, indices, capacity);
+        KCHECK(s, "k_neighbors");
+        petar_count_launch(2);
+    }
+    k_nb_status<<<1, 32, 0, s>>>((const long long*)offsets, n, capacity, status_dev, w.hdr, indices ? 1 : 0);
+    KCHECK(s, "k_nb_status");
+    petar_count_launch(1);
+    stage_end(t, PETAR_STAGE_NEIGHBOR, s);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// list export (tests): flatten the chunk chains.
+// ------------------------------------------------------------------------------------------------
+__global__ void k_list_sizes(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, int* __restrict__ sizes) {
+    int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= h->n_groups) return;
+    sizes[3 * g] = grp[g].n_sp; sizes[3 * g + 1] = 2 * grp[g].n_epn; sizes[3 * g + 2] = 2 * grp[g].n_epf;
+}
+__global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
+                               const long long* __restrict__ offs, int* __restrict__ out, long long out_entries) {
+    const int lane = threadIdx.x & 31;
+    long long wid = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (wid >= 3ll * h->n_groups) return;
+    int g = (int)(wid / 3), which = (int)(wid % 3);
+    int chunk = which == 0 ? grp[g].head_sp : which == 1 ? grp[g].head_epn : grp[g].head_epf;
+    int remaining = which == 0 ? grp[g].n_sp : which == 1 ? 2 * grp[g].n_epn : 2 * grp[g].n_epf;
+    long long o = offs[wid];
+    while (chunk >= 0 && remaining > 0) {
+        const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
+        int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+        for (int e = lane; e < ne; e += 32) if (o + e < out_entries) out[o + e] = cp[PETAR_CHUNK_HDR + e];
+        o += ne; remaining -= ne; chunk = cp[0];
+    }
+}
+__global__ void k_group_cnt(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, int* __restrict__ out, int what) {
+    int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= h->n_groups) return;
+    if (what == PETAR_DBG_GROUP_CNT) { out[4 * g] = grp[g].n_sp; out[4 * g + 1] = grp[g].n_epn; out[4 * g + 2] = grp[g].n_epf; out[4 * g + 3] = grp[g].n_ep_part; }
+    else { out[2 * g] = grp[g].begin; out[2 * g + 1] = grp[g].end; }
+}
+__global__ void k_group_dbl(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, double* __restrict__ out) {
+    int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= h->n_groups) return;
+    for (int k = 0; k < 3; ++k) { out[7 * g + k] = grp[g].lo[k]; out[7 * g + 3 + k] = grp[g].hi[k]; }
+    out[7 * g + 6] = grp[g].rmax;
+}
+__global__ void k_node_dbl(const DevHeader* __restrict__ h, const NodeMac* __restrict__ nmac, const NodeMom* __restrict__ nmom, double* __restrict__ out) {
+    int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= h->n_nodes) return;
+    double* D = out + 17ll * n;
+    D[0] = nmom[n].M;
+    for (int k = 0; k < 3; ++k) { D[1 + k] = nmac[n].com[k]; D[4 + k] = nmac[n].lo[k]; D[7 + k] = nmac[n].hi[k]; }
+    D[10] = nmac[n].rmax;
+    for (int k = 0; k < 6; ++k) D[11 + k] = nmom[n].Q[k];
+}
+
+// n_groups / n_nodes are passed by the caller (api.cu reads the header back first)
+cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_bytes, cudaStream_t s) {
+    Workspace& w = t->w;
+    int ng = t->pinned[1], nn = t->pinned[0];
+    if (what == PETAR_DBG_GROUP_CNT || what == PETAR_DBG_GROUP_INT) {
+        size_t need = (size_t)ng * (what == PETAR_DBG_GROUP_CNT ? 16 : 8);
+        if (dst_bytes < need) return cudaErrorInvalidValue;
+        if (ng) k_group_cnt<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, (int*)dst, what);
+        KCHECK(s, "k_group_cnt");
+    } else if (what == PETAR_DBG_GROUP_DBL) {
+        if (dst_bytes < (size_t)ng * 56) return cudaErrorInvalidValue;
+        if (ng) k_group_dbl<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, (double*)dst);
+        KCHECK(s, "k_group_dbl");
+    } else if (what == PETAR_DBG_NODE_DBL) {
+        if (dst_bytes < (size_t)nn * 136) return cudaErrorInvalidValue;
+        if (nn) k_node_dbl<<<cdiv(nn, 256), 256, 0, s>>>(w.hdr, w.nmac, w.nmom, (double*)dst);
+        KCHECK(s, "k_node_dbl");
+    } else if (what == PETAR_DBG_LIST_OFFS || what == PETAR_DBG_LISTS) {
+        // sizes -> scan -> flatten
+        if (!ng) return cudaSuccess;
+        int* sizes = w.exp_scratch;                                       // 3 ng ints
+        long long* offs = (long long*)(w.exp_scratch + 4ll * (ng + 1));   // 3 ng + 1 int64 (16-byte aligned)
+        k_list_sizes<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, sizes);
+        KCHECK(s, "k_list_sizes");
+        cudaError_t e = launch_scan_i32_to_i64(sizes, offs, 3ll * ng, (long long*)w.scan_tmp, s);
+        if (e != cudaSuccess) return e;
+        if (what == PETAR_DBG_LIST_OFFS) {
+            if (dst_bytes < (size_t)(3ll * ng + 1) * 8) return cudaErrorInvalidValue;
+            return cudaMemcpyAsync(dst, offs, (size_t)(3ll * ng + 1) * 8, cudaMemcpyDeviceToDevice, s);
+        }
+        k_list_flatten<<<cdiv(3ll * ng * 32, 256), 256, 0, s>>>(w.hdr, w.grp, w.arena, offs, (int*)dst, (long long)(dst_bytes / 4));
+        KCHECK(s, "k_list_flatten");
+    }
+    return cudaGetLastError();
+}
