@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py -- long-range P3T force step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3]
+
+One "step" = the whole hot path on one batch of synthetic input:
+petar_tree_build + petar_long_range_force + petar_neighbor_list (count phase and fill phase).
+Workload: BASELINE.json configs[2] (N = 1,048,576 Plummer sphere, Kroupa IMF, 100 % binaries,
+r_out = 0.003, theta = 0.3, quadrupole), the configuration the metric is quoted on.
+
+Prints ONE JSON line (rank 0).  `value` = long-range interactions per second of the whole job,
+interactions = sum over i-groups of n_i * (n_ep + n_sp) as counted by the walk (rule O7),
+inputs resident in HBM.  `e2e` = the same metric through the C-ABI with HOST buffers (pinned
+host inputs copied in, accelerations/potentials/neighbour lists copied out, every step).
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+Multi-GPU: the path is single-GPU by design ("replicas only"): N ranks run N
+independent replicas, no data-path collective; value = total interactions / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FLOP_NEWTON, FLOP_CUT, FLOP_QUAD = 20, 49, 53      # fixed flops-per-interaction convention
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--N", type=int, default=None, help="override the particle count (debugging only)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-groups", type=int, default=3000, help="i-groups in the oracle's timed sample")
+    return ap.parse_args()
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return json.load(fh), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2]))
+            except Exception:
+                continue
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            for nme, v in zip(names, r[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def cpu_oracle_sample(w, n_groups_sample: int, seed: int = 1):
+    """Times the oracle as it stands on a bounded sample: full tree build + walk + force of sampled i-groups."""
+    import oracle
+    op = oracle.OracleParams.from_workload(w)
+    t0 = time.perf_counter()
+    T = oracle.OracleTree(w.x, w.y, w.z, w.m, w.r_out, op)
+    t_build = time.perf_counter() - t0
+    ng = T.n_groups
+    sel = np.sort(np.random.default_rng(seed).choice(ng, size=min(n_groups_sample, ng), replace=False)).astype(np.int64)
+    t0 = time.perf_counter()
+    T.force(sel)
+    t_force = time.perf_counter() - t0
+    # interactions of the sample (counted by a second, untimed walk of the same groups)
+    n_int = 0
+    gb, ge, *_ = T.groups()
+    for g in sel[:: max(1, len(sel) // 200)]:
+        sp, ep = T.walk_lists(int(g))
+        n_int += (ge[g] - gb[g]) * (len(sp) + int((ep[:, 1] - ep[:, 0]).sum()))
+    n_int = n_int * len(sel) / len(sel[:: max(1, len(sel) // 200)])
+    return dict(value=n_int / t_force, unit="interactions/s", cores=oracle.num_threads(), kind="oracle",
+                sample=f"fp64 oracle (oracle/petar_oracle.c, OpenMP): tree build of all N={w.N} particles ({t_build:.2f} s, untimed in value) "
+                       f"+ walk and force of {len(sel)} of {ng} i-groups ({t_force:.2f} s, ~{n_int:.3g} interactions, "
+                       f"counted on a 1/{max(1, len(sel) // 200)} subsample)",
+                seconds=t_force, build_seconds=t_build)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from workloads import make_workload
+    w = make_workload(args.config, N=args.N)
+    vals = []
+    per_step = max(50, args.cpu_groups // max(1, args.steps + args.warmup))
+    base = None
+    for s in range(args.warmup + args.steps):
+        r = cpu_oracle_sample(w, per_step, seed=s)
+        if s >= args.warmup:
+            vals.append(r)
+        base = r
+    v = float(np.mean([r["value"] for r in vals]))
+    ms = float(np.mean([r["seconds"] for r in vals])) * 1e3
+    out = dict(metric="long-range interactions/sec", value=v, unit="interactions/s", n_gpus=args.gpus, steps=args.steps,
+               warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+               data="synthetic", impl="reference",
+               config={"workload": f"BASELINE.json configs[{args.config - 1}] (N={w.N}); each step = oracle walk+force of "
+                                   f"{per_step} sampled i-groups on the host CPU"},
+               cpu_baseline=dict(value=v, unit="interactions/s", cores=base["cores"], kind="oracle", sample=base["sample"]),
+               e2e=dict(value=v, unit="interactions/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import torch
+    import paper_2006_16560_b200 as P
+    from workloads import make_workload
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product has no CPU path)")
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist_.init_process_group("nccl", device_id=dev)
+        dist = dist_
+    W = max(3, args.warmup)
+    K = args.steps
+    cfg = args.config
+    # weak scaling: every rank holds its own replica of the workload (different seed per rank)
+    from workloads.generators import SEED_BASE
+    w = make_workload(cfg, N=args.N, seed=SEED_BASE + cfg + 1000 * rank if rank else None)
+    N = w.N
+    params = P.PetarParams.from_workload(w)
+    P.petar_set_profiling(True)
+    tree = P.Tree(N, params, device=dev)
+    stream = torch.cuda.current_stream()
+    # pinned host inputs (e2e) and their device copies (device-resident measurement)
+    host_in = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (w.x, w.y, w.z, w.m, w.r_out)]
+    dev_in = [torch.empty(N, dtype=torch.float64, device=dev) for _ in range(5)]
+    for d, h in zip(dev_in, host_in):
+        d.copy_(h, non_blocking=True)
+    tree.inputs = tuple(dev_in) + (None,)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def step_device(capacity_holder):
+        tree.build(stream)
+        P.petar_long_range_force(tree.handle, tree.acc_x, tree.acc_y, tree.acc_z, tree.pot, False, stream)
+        P.petar_neighbor_list(tree.handle, tree.offsets, None, 0, None, stream)                  # count + scan
+        P.petar_neighbor_list(tree.handle, tree.offsets, capacity_holder[0], capacity_holder[0].numel(), tree.nb_status, stream)
+
+    # one untimed pass to size the neighbour index buffer (two-phase output) and to read the counters
+    tree.build(stream)
+    counts = P.petar_long_range_force(tree.handle, tree.acc_x, tree.acc_y, tree.acc_z, tree.pot, True, stream)
+    off, idx = tree.neighbors(stream)
+    nb_total = int(off[-1].item())
+    cap = [torch.empty(int(nb_total * 1.1) + 1024, dtype=torch.int32, device=dev)]
+    n_inter = counts.n_epep + counts.n_epsp
+    quad = params.multipole >= 2
+    flops_step = (FLOP_CUT * counts.n_epep_near + FLOP_NEWTON * (counts.n_epep - counts.n_epep_near)
+                  + (FLOP_QUAD if quad else FLOP_NEWTON) * counts.n_epsp)
+
+    for _ in range(W):
+        flush.fill_(1)
+        step_device(cap)
+    torch.cuda.synchronize()
+    if dist: dist.barrier()
+    sampler = ClockSampler(local); sampler.start()
+    launches0 = P.petar_launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    stage_sum = {k: 0.0 for k in P.STAGE_NAMES}
+    torch.cuda.synchronize()
+    t_wall0 = time.perf_counter()
+    for k in range(K):
+        flush.fill_(k & 255)                     # L2 flush between timed iterations (outside the events)
+        ev[k][0].record(stream)
+        step_device(cap)
+        ev[k][1].record(stream)
+        ev[k][1].synchronize()
+        st = P.petar_stage_times(tree.handle)
+        for name, v in st.items():
+            stage_sum[name] += v
+    torch.cuda.synchronize()
+    t_wall = time.perf_counter() - t_wall0
+    launches = P.petar_launch_count() - launches0
+    clocks = sampler.stop()
+    if dist: dist.barrier()
+    ms_total = sum(a.elapsed_time(b) for a, b in ev)
+    status = P.petar_tree_status(tree.handle)
+
+    # ---- e2e: HOST buffers through the C-ABI, copies inside the timed region ---------------------------
+    host_out = [torch.empty(N, dtype=torch.float64).pin_memory() for _ in range(4)]
+    host_off = torch.empty(N + 1, dtype=torch.int64).pin_memory()
+    host_idx = torch.empty(cap[0].numel(), dtype=torch.int32).pin_memory()
+    e2e_ms, d2h_bytes = 0.0, 0
+
+    def step_e2e():
+        nonlocal d2h_bytes
+        for d, h in zip(dev_in, host_in):
+            d.copy_(h, non_blocking=True)
+        tree.build(stream)
+        P.petar_long_range_force(tree.handle, tree.acc_x, tree.acc_y, tree.acc_z, tree.pot, False, stream)
+        P.petar_neighbor_list(tree.handle, tree.offsets, None, 0, None, stream)
+        total = int(tree.offsets[-1].item())                 # the caller reads the total, then asks for the rows
+        if total > cap[0].numel():
+            cap[0] = torch.empty(int(total * 1.1), dtype=torch.int32, device=dev)
+        P.petar_neighbor_list(tree.handle, tree.offsets, cap[0], cap[0].numel(), tree.nb_status, stream)
+        for h, d in zip(host_out, (tree.acc_x, tree.acc_y, tree.acc_z, tree.pot)):
+            h.copy_(d, non_blocking=True)
+        host_off.copy_(tree.offsets, non_blocking=True)
+        host_idx[:total].copy_(cap[0][:total], non_blocking=True)
+        stream.synchronize()
+        d2h_bytes = 4 * 8 * N + 8 * (N + 1) + 4 * total + 8
+
+    step_e2e()
+    torch.cuda.synchronize()
+    Ke = max(3, min(K, 10))
+    if dist: dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        step_e2e()
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / Ke
+    h2d_bytes = 5 * 8 * N
+
+    # ---- FP32 peak probe (FFMA only), timed alone ------------------------------------------------------
+    scratch = torch.zeros(1, dtype=torch.float32, device=dev)
+    P.petar_probe_fp32(20000, scratch, stream)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream); fl = P.petar_probe_fp32(400000, scratch, stream); b.record(stream); b.synchronize()
+    probe_tflops = fl / (a.elapsed_time(b) * 1e-3) / 1e12
+
+    # ---- aggregate over ranks --------------------------------------------------------------------------
+    ms_step = ms_total / K
+    tot_inter = float(n_inter)
+    if dist:
+        t = torch.tensor([ms_step, e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step, e2e_ms = float(t[0]), float(t[1])
+        s = torch.tensor([tot_inter], dtype=torch.float64, device=dev)
+        dist.all_reduce(s, op=dist.ReduceOp.SUM)
+        tot_inter = float(s[0])
+    value = tot_inter / (ms_step * 1e-3)
+    e2e_value = tot_inter / (e2e_ms * 1e-3)
+
+    pk, pk_kind = peaks()
+    sm_max = float(pk.get("sm_max_mhz", 1965.0))
+    nominal_fp32 = 2 * 128 * 148 * sm_max * 1e6 / 1e12
+    force_ms = stage_sum["force"] / K
+    achieved = flops_step / (force_ms * 1e-3) / 1e12
+    stage_ms = {k: v / K for k, v in stage_sum.items()}
+
+    if rank == 0:
+        out = dict(
+            metric="long-range interactions/sec", value=value, unit="interactions/s", n_gpus=world, steps=K, warmup=W,
+            ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+            config={"workload": f"BASELINE.json configs[{cfg - 1}]: N={N} Plummer (Henon units), "
+                                f"{w.meta['masses']} masses, {2 * w.meta['n_pairs']} stars in binaries, r_out_ref={w.r_out_ref}, "
+                                f"theta={w.theta}, multipole={params.multipole}, leaf<=8, group<=64",
+                    "step": "petar_tree_build + petar_long_range_force + petar_neighbor_list (count phase + fill phase)",
+                    "l2": "256 MB buffer written between timed iterations (L2 flush), outside the per-step CUDA events",
+                    "interactions_per_step": int(n_inter), "n_epep": int(counts.n_epep), "n_epsp": int(counts.n_epsp),
+                    "n_epep_changeover": int(counts.n_epep_near), "neighbours": nb_total, "n_groups": int(counts.n_groups),
+                    "n_nodes": int(counts.n_nodes), "status": status, "multi_gpu": "replicas only (no data-path collective)"},
+            stage_ms=stage_ms,
+            e2e=dict(value=e2e_value, unit="interactions/s", ms_per_step=e2e_ms, h2d_bytes_per_step=h2d_bytes,
+                     d2h_bytes_per_step=d2h_bytes, steps=Ke),
+            gpu_launches=int(launches),
+            clocks=clocks,
+            roofline=dict(bound="alu", kernel="k_force", achieved=achieved, peak=nominal_fp32, unit="TFLOP/s",
+                          frac=achieved / nominal_fp32, traffic=None,
+                          peak_kind=f"nominal CUDA-core FP32: 2 x 128 lanes x 148 SMs x {sm_max:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {pk_kind})",
+                          peak_measured_ffma_probe=probe_tflops, frac_of_probe=achieved / probe_tflops,
+                          flops_convention=f"{FLOP_NEWTON}/{FLOP_CUT}/{FLOP_QUAD} flops per Newtonian / changeover / quadrupole interaction",
+                          flops_per_launch=float(flops_step), kernel_ms=force_ms, kernel_share_of_step=force_ms / ms_step,
+                          hbm_peak_gbs=pk.get("hbm_gbs")),
+            wall_s_timed_region=t_wall,
+        )
+        if not args.no_cpu_baseline and world == 1:
+            cb = cpu_oracle_sample(w, args.cpu_groups)
+            out["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        print(json.dumps(out), flush=True)
+    if dist:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -158,7 +158,7 @@ int petar_debug_export(petar_tree* t, int what, void* dst, size_t dst_bytes, voi
 
 /* Per-stage device times of the last build / force / neighbour call on this tree, in ms, measured
  * with CUDA events when profiling was switched on with petar_set_profiling(1) (HOST; default off;
- * switching it on makes the calls synchronise).  stage_ms: HOST float[PETAR_N_STAGES].             */
+ * it must be set before petar_tree_build; events are recorded asynchronously and petar_stage_times synchronises on them).  stage_ms: HOST float[PETAR_N_STAGES].             */
 #define PETAR_STAGE_BBOX_KEYS 0
 #define PETAR_STAGE_SORT 1
 #define PETAR_STAGE_GATHER 2
@@ -173,6 +173,12 @@ int petar_set_profiling(int on);
 int petar_stage_times(petar_tree* t, float* stage_ms /* HOST */);
 /* Number of kernel launches the library has enqueued since process start (HOST counter).           */
 int64_t petar_launch_count(void);
+
+/* Measurement hook (not part of the path): enqueues an FFMA-only kernel (16 independent chains per
+ * thread, 8 CTAs x 256 threads per SM) and returns the flops it executes in *flops_out_host (HOST);
+ * the caller times it with CUDA events to obtain this GPU's CUDA-core FP32 peak.
+ * scratch_dev: DEVICE float[1].                                                                      */
+int petar_probe_fp32(int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -11,7 +11,7 @@ _LIB = None
 EXPORTS = [
     "petar_workspace_bytes", "petar_tree_build", "petar_long_range_force", "petar_neighbor_list",
     "petar_tree_status", "petar_tree_destroy", "petar_strerror", "petar_debug_export",
-    "petar_set_profiling", "petar_stage_times", "petar_launch_count",
+    "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32",
 ]
 STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor"]
 DBG = dict(HEADER=0, ROOT=1, KEYS=2, PERM=3, NODE_INT=4, NODE_DBL=5, GROUP_INT=6, GROUP_DBL=7, GROUP_CNT=8,
@@ -82,6 +82,8 @@ def lib():
         L.petar_stage_times.restype = C.c_int
         L.petar_stage_times.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
         L.petar_launch_count.restype = C.c_int64
+        L.petar_probe_fp32.restype = C.c_int
+        L.petar_probe_fp32.argtypes = [C.c_int64, C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
         _LIB = L
     return _LIB
 
@@ -165,6 +167,15 @@ def petar_stage_times(tree):
     if rc:
         raise PetarError(rc, "petar_stage_times")
     return {n: float(arr[i]) for i, n in enumerate(STAGE_NAMES)}
+
+
+def petar_probe_fp32(iters: int, scratch, stream=None) -> float:
+    """Enqueues the FFMA probe kernel; returns the flops it executes (time it with CUDA events)."""
+    fl = C.c_double(0.0)
+    rc = lib().petar_probe_fp32(C.c_int64(iters), C.byref(fl), _ptr(scratch), _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_probe_fp32")
+    return float(fl.value)
 
 
 def petar_launch_count() -> int:

@@ -9,7 +9,6 @@
 static thread_local cudaError_t g_last_cuda = cudaSuccess;
 static std::atomic<long long> g_launches{0};
 static int g_profiling = 0;
-static cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
 
 void petar_count_launch(int n) { g_launches += n; }
 void petar_debug_check(cudaStream_t s, const char* name) {
@@ -20,19 +19,20 @@ void petar_debug_check(cudaStream_t s, const char* name) {
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) fprintf(stderr, "[petar] kernel %s failed: %s\n", name, cudaGetErrorString(e));
 }
+// Stage timing: events are only RECORDED here (asynchronously, on the caller's stream);
+// petar_stage_times synchronises on them later.  No effect unless petar_set_profiling(1)
+// was called before petar_tree_build.
 void stage_begin(petar_tree* t, cudaStream_t s) {
-    (void)t;
-    if (!g_profiling) return;
-    if (!g_ev0) { cudaEventCreate(&g_ev0); cudaEventCreate(&g_ev1); }
-    cudaEventRecord(g_ev0, s);
+    if (!t->ev) return;
+    cudaEventRecord(t->ev[2 * PETAR_N_STAGES], s);      // scratch slot
 }
 void stage_end(petar_tree* t, int stage, cudaStream_t s) {
-    if (!g_profiling) return;
-    cudaEventRecord(g_ev1, s);
-    cudaEventSynchronize(g_ev1);
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, g_ev0, g_ev1);
-    t->stage_ms[stage] = ms;
+    if (!t->ev) return;
+    cudaEvent_t b = t->ev[2 * PETAR_N_STAGES];          // swap the begin event into the stage's slot
+    t->ev[2 * PETAR_N_STAGES] = t->ev[2 * stage];
+    t->ev[2 * stage] = b;
+    cudaEventRecord(t->ev[2 * stage + 1], s);
+    t->stage_rec[stage] = 1;
 }
 
 static inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
@@ -118,6 +118,10 @@ extern "C" int petar_tree_build(const double* x, const double* y, const double* 
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&t->pinned, 64 * sizeof(long long));
+    if (e == cudaSuccess && g_profiling) {
+        t->ev = new (std::nothrow) cudaEvent_t[2 * PETAR_N_STAGES + 1];
+        for (int k = 0; t->ev && k < 2 * PETAR_N_STAGES + 1 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);
+    }
     if (e != cudaSuccess) { g_last_cuda = e; delete t; return PETAR_ECUDA; }
     if (N > 0) {
         carve(&t->w, (char*)workspace, N, p);
@@ -202,6 +206,7 @@ extern "C" int petar_tree_destroy(petar_tree* t) {
     if (t->magic != PETAR_MAGIC) return PETAR_ENOTBUILT;
     t->magic = 0; t->built = false;
     if (t->pinned) cudaFreeHost(t->pinned);
+    if (t->ev) { for (int k = 0; k < 2 * PETAR_N_STAGES + 1; ++k) cudaEventDestroy(t->ev[k]); delete[] t->ev; }
     delete t;
     return PETAR_OK;
 }
@@ -271,7 +276,13 @@ extern "C" int petar_stage_times(petar_tree* t, float* stage_ms) {
     int rc = check_tree(t);
     if (rc) return rc;
     if (!stage_ms) return PETAR_EINVAL;
-    memcpy(stage_ms, t->stage_ms, sizeof(t->stage_ms));
+    for (int k = 0; k < PETAR_N_STAGES; ++k) {
+        stage_ms[k] = 0.f;
+        if (t->ev && t->stage_rec[k]) {
+            CK(cudaEventSynchronize(t->ev[2 * k + 1]));
+            CK(cudaEventElapsedTime(&stage_ms[k], t->ev[2 * k], t->ev[2 * k + 1]));
+        }
+    }
     return PETAR_OK;
 }
 extern "C" int64_t petar_launch_count(void) { return (int64_t)g_launches.load(); }

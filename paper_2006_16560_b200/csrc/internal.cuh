@@ -88,7 +88,8 @@ struct petar_tree {
     Workspace w;
     const double *x, *y, *z, *m, *r_out, *r_search;
     bool built, walked;
-    float stage_ms[PETAR_N_STAGES];
+    cudaEvent_t* ev;               // [2*PETAR_N_STAGES + 1] stage begin/end events (profiling only)
+    int stage_rec[PETAR_N_STAGES];
     int sm_count;
     int* pinned;                   // small pinned host buffer for header read-back
 };
