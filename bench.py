@@ -43,7 +43,7 @@ def parse():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--N", type=int, default=None, help="override the particle count (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-groups", type=int, default=3000, help="i-groups in the oracle's timed sample")
+    ap.add_argument("--cpu-groups", type=int, default=40000, help="i-groups in the oracle's timed sample")
     return ap.parse_args()
 
 

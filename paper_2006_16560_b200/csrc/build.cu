@@ -505,8 +505,9 @@ __global__ void __launch_bounds__(256) k_moments(const DevHeader* __restrict__ h
             NodeSp sp;
             sp.q0 = make_float4(xh, yh, zh, (float)M);
             if (multipole >= 2) {
-                sp.q1 = make_float4(xl, yl, zl, (float)(1.5 * Q[0] - 0.5 * tr));
-                sp.q2 = make_float4((float)(1.5 * Q[1] - 0.5 * tr), (float)(1.5 * Q[3]), (float)(1.5 * Q[4]), (float)(1.5 * Q[5]));
+                // B = -2 A' with A' = 1.5 Q - 0.5 tr(Q) I  (the force kernel works with B, see force.cu)
+                sp.q1 = make_float4(xl, yl, zl, (float)(-2.0 * (1.5 * Q[0] - 0.5 * tr)));
+                sp.q2 = make_float4((float)(-2.0 * (1.5 * Q[1] - 0.5 * tr)), (float)(-3.0 * Q[3]), (float)(-3.0 * Q[4]), (float)(-3.0 * Q[5]));
             } else {
                 sp.q1 = make_float4(xl, yl, zl, 0.f);
                 sp.q2 = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -557,7 +558,7 @@ __global__ void __launch_bounds__(256) k_groups_finish(GroupRec* __restrict__ gr
         if (lane == 0) {          // (begin is left alone: the neighbouring warp reads it)
             GroupRec* r = &grp[g];
             r->end = e; r->head_sp = r->head_epn = r->head_epf = -1;
-            r->n_sp = r->n_epn = r->n_epf = 0; r->n_ep_part = r->n_epn_part = 0; r->pad0 = r->pad1 = 0;
+            r->n_sp = r->n_epn = r->n_epf = 0; r->n_ep_part = r->n_epn_part = 0; r->head_spp = -1; r->n_spp = 0;
             for (int k = 0; k < 3; ++k) { r->lo[k] = lo[k]; r->hi[k] = hi[k]; }
             r->rmax = rmax; r->pad2 = 0;
         }

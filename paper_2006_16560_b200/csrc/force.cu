@@ -3,20 +3,29 @@
 //
 // One CTA (128 threads) per i-group, groups pulled from a device ticket (persistent CTAs).
 // Thread mapping: the group's n_i particles are taken two per thread ("pair slot" p = t % P,
-// P = ceil(n_i/2)); the remaining factor of the CTA, S = 128 / P, splits every j-tile into S
-// interleaved slices (slice s = t / P handles j = s, s+S, ...).  This keeps >= 80 % of the lanes busy
-// for any n_i in 1..64 and halves the shared-memory reads per interaction.
+// P = ceil(n_i/2)); S = 128 / P slices split every staged j-tile (slice s handles j = s, s+S, ...),
+// so >= 80 % of the lanes are busy for any n_i in 1..64 and every shared-memory j-record feeds two
+// interactions.
 //
-// Precision: positions are float-float (hi + lo) relative to the root-cube centre; a pair's
-// displacement is (xjh - xih) + (xjl - xil), which is the pair-relative coordinate to ~1e-7
-// relative accuracy whatever the distance from the origin.  fp32
-// partial sums live only across one tile slice and are flushed into fp64 accumulators per tile.
+// The kernel is ISSUE-bound ("force kernel"): on B200 scalar FFMA/FADD/FMUL issue at one
+// warp instruction per clock per sub-partition, the packed fp32x2 forms measured slower per flop for
+// distinct operands, so the design minimises instructions per interaction:
+//   * cells farther from the group than the group's own size (the bulk) are evaluated with
+//     GROUP-RELATIVE single floats: the j-record is translated to the group centre once when its tile
+//     is staged, the displacement is then one FADD per axis (33 fp32 instructions + 1 MUFU per
+//     quadrupole interaction);
+//   * cells closer than that, and all particles, keep float-float coordinates (hi + lo, relative to
+//     the root-cube centre): displacement (xjh - xih) + (xjl - xil), exact to ~1e-7 of the
+//     separation whatever the distance from the origin (needed for tight binaries in sparse groups).
+// Super-particle tiles are gathered through a 3-stage software pipeline (ids two tiles ahead,
+// 48-byte records one tile ahead in registers, current tile in double-buffered shared memory), so
+// the dependent id -> record loads overlap the arithmetic and there is one barrier per tile.
+// fp32 partial sums live only across one tile slice and are flushed into fp64 accumulators per tile.
 #include "internal.cuh"
 
 #define FT 128                 // threads per CTA
-#define SP_TILE 256            // cells per staged tile
+#define SP_TILE 256            // cells per staged tile (two per thread)
 #define EP_TILE 512            // particles per staged tile
-#define EP_BATCH FT            // EP ranges expanded per batch (one per thread)
 
 struct ForceConst {
     float c1, c0;              // x = r * inv_R * c1 - c0,  c1 = 1/(1-rho), c0 = rho/(1-rho)
@@ -25,101 +34,220 @@ struct ForceConst {
     float a4;                  // 35 Lambda: K = (1-x)^4 (1 + 4x + 10x^2 + 20x^3 + a4 x^4) (form A, x >= 1/2)
 };
 
-struct IPart {
-    float xh, yh, zh, xl, yl, zl, inv_ro;
-    float ax, ay, az, pot;     // fp32 partial sums of the current tile slice
-};
+__device__ __forceinline__ float rsqrt_ftz(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
-__device__ __forceinline__ void sp_interact(IPart& p, const float4 a, const float4 b, const float4 c, const bool quad) {
-    // d = com - x_i  (points to the source)
-    const float dx = (a.x - p.xh) + (b.x - p.xl);
-    const float dy = (a.y - p.yh) + (b.y - p.yl);
-    const float dz = (a.z - p.zh) + (b.z - p.zl);
-    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const float rinv = rsqrtf(r2);
-    const float rinv2 = rinv * rinv;
-    const float mr = a.w * rinv;
-    if (!quad) {
-        const float f = mr * rinv2;
-        p.pot -= mr;
-        p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
-    } else {
-        // A = traceless quadrupole: (Axx, Ayy, Azz = -(Axx+Ayy), Axy, Axz, Ayz) = (b.w, c.x, -, c.y, c.z, c.w)
-        const float azz = -(b.w + c.x);
-        const float adx = fmaf(b.w, dx, fmaf(c.y, dy, c.z * dz));
-        const float ady = fmaf(c.y, dx, fmaf(c.x, dy, c.w * dz));
-        const float adz = fmaf(c.z, dx, fmaf(c.w, dy, azz * dz));
-        const float dad = fmaf(dx, adx, fmaf(dy, ady, dz * adz));
-        const float rinv3 = rinv * rinv2, rinv5 = rinv3 * rinv2;
-        const float q5 = dad * rinv5;                  // d^T A d / r^5
-        p.pot -= mr + q5;                              // phi = -[M/r + d^T A d / r^5]
-        const float f = fmaf(5.0f * q5, rinv2, mr * rinv2);   // M/r^3 + 5 dAd / r^7
-        const float g = -2.0f * rinv5;
-        p.ax = fmaf(f, dx, fmaf(g, adx, p.ax));
-        p.ay = fmaf(f, dy, fmaf(g, ady, p.ay));
-        p.az = fmaf(f, dz, fmaf(g, adz, p.az));
-    }
-}
-
-template <bool NEAR>
-__device__ __forceinline__ void ep_interact(IPart& p, const float4 a, const float4 b, const ForceConst& k, const bool self) {
-    const float dx = (a.x - p.xh) + (b.x - p.xl);
-    const float dy = (a.y - p.yh) + (b.y - p.yl);
-    const float dz = (a.z - p.zh) + (b.z - p.zl);
-    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const float rinv = (r2 > 0.0f) ? rsqrtf(r2) : 0.0f;     // self / coincident pair: no force
-    const float rinv2 = rinv * rinv;
-    if (!NEAR) {
-        const float mr = a.w * rinv;
-        const float f = mr * rinv2;
-        p.pot -= mr;
-        p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
-    } else {
-        const float inv_R = fminf(p.inv_ro, b.w);           // 1 / max(r_out,i, r_out,j)
-        const float r = r2 * rinv;
-        const float x = fmaf(r * inv_R, k.c1, -k.c0);
-        const float xc = __saturatef(x);
-        const float x2 = xc * xc, x4 = x2 * x2;
-        // 1 - K: form B below 1/2 (no cancellation at small x), form A above (K itself is small there)
-        const float qb = fmaf(fmaf(fmaf(fmaf(k.b4, xc, k.b3), xc, k.b2), xc, k.b1), xc, k.b0);
-        const float wb = x4 * qb;
-        const float y = 1.0f - xc, y2 = y * y, y4 = y2 * y2;
-        const float pa = fmaf(fmaf(fmaf(fmaf(k.a4, xc, 20.0f), xc, 10.0f), xc, 4.0f), xc, 1.0f);
-        const float wa = fmaf(-y4, pa, 1.0f);
-        const float wk = (xc < 0.5f) ? wb : wa;
-        // (1 - W)/r = (1+Lambda)/R - Lambda x^5 (14 - 28x + 20x^2 - 5x^3)/r  for r < R, 1/r beyond
-        const float gp = x4 * xc * fmaf(fmaf(fmaf(-5.0f, xc, 20.0f), xc, -28.0f), xc, 14.0f);
-        float pw = (x < 1.0f) ? fmaf(-k.lam * gp, rinv, k.one_plus_lam * inv_R) : rinv;
-        if (self) pw = 0.0f;                                 // the list holds the particle itself (j == i)
-        p.pot = fmaf(-a.w, pw, p.pot);
-        const float f = a.w * wk * rinv * rinv2;
-        p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
-    }
-}
-
+struct Acc32 { float ax, ay, az, pot; };      // pot accumulates +sum m (1-W)/r; sign applied at the end
 struct Acc64 { double ax, ay, az, pot; };
-__device__ __forceinline__ void flush(IPart& p, Acc64& a) {
+__device__ __forceinline__ void flush(Acc32& p, Acc64& a) {
     a.ax += (double)p.ax; a.ay += (double)p.ay; a.az += (double)p.az; a.pot += (double)p.pot;
     p.ax = p.ay = p.az = p.pot = 0.0f;
 }
 
+// Cell term from the displacement d = com - x_i.  With B = -2A (stored by the moments kernel):
+//   bd = B d,  u = (d.bd)/r^5 = -2 dAd/r^5
+//   phi = -[M/r + dAd/r^5]                    ->  pot += M/r - u/2
+//   a   = (M/r^3 + 5 dAd/r^7) d - 2 A d/r^5   =   (M/r - 2.5 u)/r^2 * d + bd/r^5
+template <bool QUAD>
+__device__ __forceinline__ void cell_term(Acc32& p, const float dx, const float dy, const float dz, const float M,
+                                          const float bxx, const float byy, const float bzz, const float bxy, const float bxz, const float byz) {
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const float rinv = rsqrt_ftz(r2);
+    const float rinv2 = rinv * rinv;
+    const float mr = M * rinv;
+    if (!QUAD) {
+        const float f = mr * rinv2;
+        p.pot += mr;
+        p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
+    } else {
+        const float bdx = fmaf(bxx, dx, fmaf(bxy, dy, bxz * dz));
+        const float bdy = fmaf(bxy, dx, fmaf(byy, dy, byz * dz));
+        const float bdz = fmaf(bxz, dx, fmaf(byz, dy, bzz * dz));
+        const float dbd = fmaf(dx, bdx, fmaf(dy, bdy, dz * bdz));
+        const float rinv4 = rinv2 * rinv2;
+        const float rinv5 = rinv4 * rinv;
+        const float u = dbd * rinv5;
+        p.pot = fmaf(u, -0.5f, p.pot + mr);
+        const float f = fmaf(u, -2.5f, mr) * rinv2;
+        p.ax = fmaf(f, dx, fmaf(rinv5, bdx, p.ax));
+        p.ay = fmaf(f, dy, fmaf(rinv5, bdy, p.ay));
+        p.az = fmaf(f, dz, fmaf(rinv5, bdz, p.az));
+    }
+}
+
+struct IFF { float nxh, nyh, nzh, nxl, nyl, nzl, inv_ro; };     // negated float-float position of an i-particle
+
+// one far particle: plain Newtonian (every pair of a far leaf has r >= R_ij > 0, rule O7)
+__device__ __forceinline__ void ep_far_one(Acc32& p, const IFF& i, const float4 a, const float4 b) {
+    const float dx = (a.x + i.nxh) + (b.x + i.nxl);
+    const float dy = (a.y + i.nyh) + (b.y + i.nyl);
+    const float dz = (a.z + i.nzh) + (b.z + i.nzl);
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const float rinv = rsqrt_ftz(r2);
+    const float mr = a.w * rinv;
+    const float f = mr * (rinv * rinv);
+    p.pot += mr;
+    p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
+}
+
+// one near particle: changeover weights (Eq. 15-17).  self = the list entry is the i-particle itself.
+__device__ __forceinline__ void ep_near_one(Acc32& p, const IFF& i, const float4 a, const float4 b, const ForceConst& k, const bool self) {
+    const float dx = (a.x + i.nxh) + (b.x + i.nxl);
+    const float dy = (a.y + i.nyh) + (b.y + i.nyl);
+    const float dz = (a.z + i.nzh) + (b.z + i.nzl);
+    const float m = a.w;
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const float rinv = (r2 > 0.0f) ? rsqrt_ftz(r2) : 0.0f;      // self / coincident pair: no force
+    const float rinv2 = rinv * rinv;
+    const float inv_R = fminf(i.inv_ro, b.w);                   // 1 / max(r_out,i, r_out,j)
+    const float r = r2 * rinv;
+    const float x = fmaf(r * inv_R, k.c1, -k.c0);
+    const float xc = __saturatef(x);
+    const float x2 = xc * xc, x4 = x2 * x2;
+    // 1 - K: form B below 1/2 (no cancellation at small x), form A above (K itself is small there)
+    const float qb = fmaf(fmaf(fmaf(fmaf(k.b4, xc, k.b3), xc, k.b2), xc, k.b1), xc, k.b0);
+    const float wb = x4 * qb;
+    const float y = 1.0f - xc, y2 = y * y, y4 = y2 * y2;
+    const float pa = fmaf(fmaf(fmaf(fmaf(k.a4, xc, 20.0f), xc, 10.0f), xc, 4.0f), xc, 1.0f);
+    const float wa = fmaf(-y4, pa, 1.0f);
+    const float wk = (xc < 0.5f) ? wb : wa;
+    // (1 - W)/r = (1+Lambda)/R - Lambda x^5 (14 - 28x + 20x^2 - 5x^3)/r  for r < R, 1/r beyond
+    const float gp = x4 * xc * fmaf(fmaf(fmaf(-5.0f, xc, 20.0f), xc, -28.0f), xc, 14.0f);
+    float pw = (x < 1.0f) ? fmaf(-k.lam * gp, rinv, k.one_plus_lam * inv_R) : rinv;
+    if (self) pw = 0.0f;                                        // the list holds the particle itself
+    p.pot = fmaf(m, pw, p.pot);
+    const float f = m * wk * rinv * rinv2;
+    p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
+}
+
+// staged super-particle tile.  PLAIN:   q0 = (xr, yr, zr, M) group-relative, q1 = (Bxx, Byy, Bzz, Bxy), q2 = (Bxz, Byz, -, -)
+//                              PRECISE: q0 = (xh, yh, zh, M), q1 = (xl, yl, zl, Bxx), q2 = (Byy, Bzz, Bxy, Bxz), q3 = Byz
+struct SpBuf { float4 q0[SP_TILE], q1[SP_TILE], q2[SP_TILE]; float q3[SP_TILE]; };   // 13 KB
 union __align__(16) ForceSmem {
-    struct { float4 q0[SP_TILE], q1[SP_TILE], q2[SP_TILE]; } sp;      // 12 KB
-    struct { float4 a[EP_TILE], b[EP_TILE]; int j[EP_TILE]; } ep;      // 18 KB (j = sorted index, near pass)
+    SpBuf sp[2];                                                       // 26 KB
+    struct { float4 a[EP_TILE], b[EP_TILE]; int j[EP_TILE]; } ep;      // 18 KB
     double red[FT * 8];                                                // 8 KB
 };
 
+// uniform cursor over the tiles (<= SP_TILE entries, never straddling a chunk) of a chunked list
+struct TileCursor {
+    const int* cp; int chunk, nxt, off, remaining;
+    __device__ __forceinline__ void init(const int* arena, int head, int n) {
+        chunk = head; remaining = n; off = 0;
+        cp = arena + (size_t)(chunk >= 0 ? chunk : 0) * PETAR_CHUNK;
+        nxt = (chunk >= 0 && n > PETAR_CHUNK_PAYLOAD) ? cp[0] : -1;
+    }
+    __device__ __forceinline__ int count() const { return (chunk >= 0 && remaining > 0) ? min(SP_TILE, min(remaining, PETAR_CHUNK_PAYLOAD - off)) : 0; }
+    __device__ __forceinline__ void advance(const int* arena, int n) {
+        remaining -= n; off += n;
+        if (remaining > 0 && off >= PETAR_CHUNK_PAYLOAD) {
+            chunk = nxt; off = 0;
+            cp = arena + (size_t)(chunk >= 0 ? chunk : 0) * PETAR_CHUNK;
+            nxt = (chunk >= 0 && remaining > PETAR_CHUNK_PAYLOAD) ? cp[0] : -1;
+        }
+    }
+};
+
+// One super-particle list of the group (3-stage pipeline).  gh/gl: group centre (float-float, root-relative).
+template <bool QUAD, bool PRECISE>
+__device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ arena, const NodeSp* __restrict__ nsp,
+                                         const int head, const int n, const int t, const int slice, const int S, const bool active,
+                                         const float4 ia0, const float4 ib0, const float4 ia1, const float4 ib1,
+                                         const float3 gh, const float3 gl, Acc64& acc0, Acc64& acc1) {
+    if (n <= 0) return;             // uniform
+    // i-particles in the representation of this path
+    float ix0, iy0, iz0, ix1, iy1, iz1;                 // PLAIN: group-relative; PRECISE: -hi
+    float lx0 = 0.f, ly0 = 0.f, lz0 = 0.f, lx1 = 0.f, ly1 = 0.f, lz1 = 0.f;     // PRECISE: -lo
+    if (PRECISE) {
+        ix0 = -ia0.x; iy0 = -ia0.y; iz0 = -ia0.z; lx0 = -ib0.x; ly0 = -ib0.y; lz0 = -ib0.z;
+        ix1 = -ia1.x; iy1 = -ia1.y; iz1 = -ia1.z; lx1 = -ib1.x; ly1 = -ib1.y; lz1 = -ib1.z;
+    } else {
+        ix0 = (ia0.x - gh.x) + (ib0.x - gl.x); iy0 = (ia0.y - gh.y) + (ib0.y - gl.y); iz0 = (ia0.z - gh.z) + (ib0.z - gl.z);
+        ix1 = (ia1.x - gh.x) + (ib1.x - gl.x); iy1 = (ia1.y - gh.y) + (ib1.y - gl.y); iz1 = (ia1.z - gh.z) + (ib1.z - gl.z);
+    }
+    Acc32 p0 = {0.f, 0.f, 0.f, 0.f}, p1 = {0.f, 0.f, 0.f, 0.f};
+    TileCursor cur; cur.init(arena, head, n);
+    int tn0 = 0, tn1 = 0, tn2 = 0;
+    int id2[2] = {0, 0};
+    float4 q0[2], q1[2], q2[2];
+    auto load_ids = [&]() {
+        tn2 = cur.count();
+#pragma unroll
+        for (int r = 0; r < 2; ++r) if (t + r * FT < tn2) id2[r] = cur.cp[PETAR_CHUNK_HDR + cur.off + t + r * FT];
+        cur.advance(arena, tn2);
+    };
+    auto load_recs = [&]() {
+        tn1 = tn2;
+#pragma unroll
+        for (int r = 0; r < 2; ++r) if (t + r * FT < tn1) { const NodeSp* sp = &nsp[id2[r]]; q0[r] = sp->q0; q1[r] = sp->q1; if (QUAD) q2[r] = sp->q2; }
+    };
+    auto store_recs = [&](SpBuf& bf) {
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            const int k = t + r * FT;
+            if (k < tn1) {
+                const float bzz = -(q1[r].w + q2[r].x);
+                if (PRECISE) {
+                    bf.q0[k] = q0[r];
+                    bf.q1[k] = q1[r];
+                    if (QUAD) { bf.q2[k] = make_float4(q2[r].x, bzz, q2[r].y, q2[r].z); bf.q3[k] = q2[r].w; }
+                } else {
+                    bf.q0[k] = make_float4((q0[r].x - gh.x) + (q1[r].x - gl.x), (q0[r].y - gh.y) + (q1[r].y - gl.y),
+                                           (q0[r].z - gh.z) + (q1[r].z - gl.z), q0[r].w);
+                    if (QUAD) { bf.q1[k] = make_float4(q1[r].w, q2[r].x, bzz, q2[r].y); bf.q2[k] = make_float4(q2[r].z, q2[r].w, 0.f, 0.f); }
+                }
+            }
+        }
+    };
+    __syncthreads();            // shared memory free (previous phase consumed)
+    load_ids();                 // tile 0 ids
+    load_recs();                // tile 0 records
+    load_ids();                 // tile 1 ids
+    store_recs(sm.sp[0]); tn0 = tn1;
+    load_recs();                // tile 1 records
+    load_ids();                 // tile 2 ids
+    __syncthreads();
+    int cb = 0;
+    while (tn0 > 0) {
+        if (active) {
+            const SpBuf& bf = sm.sp[cb];
+#pragma unroll 2
+            for (int j = slice; j < tn0; j += S) {
+                const float4 a = bf.q0[j];
+                if (PRECISE) {
+                    const float4 b = bf.q1[j];
+                    float4 c = make_float4(0.f, 0.f, 0.f, 0.f); float byz = 0.f;
+                    if (QUAD) { c = bf.q2[j]; byz = bf.q3[j]; }
+                    cell_term<QUAD>(p0, (a.x + ix0) + (b.x + lx0), (a.y + iy0) + (b.y + ly0), (a.z + iz0) + (b.z + lz0), a.w, b.w, c.x, c.y, c.z, c.w, byz);
+                    cell_term<QUAD>(p1, (a.x + ix1) + (b.x + lx1), (a.y + iy1) + (b.y + ly1), (a.z + iz1) + (b.z + lz1), a.w, b.w, c.x, c.y, c.z, c.w, byz);
+                } else {
+                    float4 b = make_float4(0.f, 0.f, 0.f, 0.f); float2 c = make_float2(0.f, 0.f);
+                    if (QUAD) { b = bf.q1[j]; c = *reinterpret_cast<const float2*>(&bf.q2[j]); }
+                    cell_term<QUAD>(p0, a.x - ix0, a.y - iy0, a.z - iz0, a.w, b.x, b.y, b.z, b.w, c.x, c.y);
+                    cell_term<QUAD>(p1, a.x - ix1, a.y - iy1, a.z - iz1, a.w, b.x, b.y, b.z, b.w, c.x, c.y);
+                }
+            }
+            flush(p0, acc0); flush(p1, acc1);
+        }
+        store_recs(sm.sp[cb ^ 1]); tn0 = tn1;    // tile k+1 (its loads overlapped the loop above)
+        load_recs();                             // tile k+2 records (their ids arrived a tile ago)
+        load_ids();                              // tile k+3 ids
+        cb ^= 1;
+        __syncthreads();
+    }
+}
+
 template <bool QUAD>
-__global__ void __launch_bounds__(FT) k_force(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
-                                              const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
-                                              const unsigned* __restrict__ perm, const double* __restrict__ ms, const double* __restrict__ routs,
-                                              double* __restrict__ oax, double* __restrict__ oay, double* __restrict__ oaz, double* __restrict__ opot,
-                                              ForceConst fc, double G, double one_plus_lam64) {
+__global__ void __launch_bounds__(FT, 4) k_force(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
+                                                 const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
+                                                 const unsigned* __restrict__ perm,
+                                                 double* __restrict__ oax, double* __restrict__ oay, double* __restrict__ oaz, double* __restrict__ opot,
+                                                 ForceConst fc, double G) {
     __shared__ ForceSmem sm;
     __shared__ int s_g;
-    __shared__ int s_scan[FT / 32 + 1];
+    __shared__ int s_scan[FT / 32];
     const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
     const int ng = h->n_groups;
+    const double rcx = h->c[0], rcy = h->c[1], rcz = h->c[2];
     for (;;) {
         __syncthreads();
         if (t == 0) s_g = atomicAdd(&h->group_ticket2, 1);
@@ -132,121 +260,97 @@ __global__ void __launch_bounds__(FT) k_force(DevHeader* __restrict__ h, const G
         const int S = FT / P;
         const int pslot = t % P, slice = t / P;
         const bool active = slice < S;
-        IPart ip[2];
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
-            int i = gb + 2 * pslot + q;
-            if (i >= gb + n_i) i = gb + n_i - 1;         // odd n_i: duplicate the last particle (result dropped)
-            float4 a = pa[i], b = pb[i];
-            ip[q].xh = a.x; ip[q].yh = a.y; ip[q].zh = a.z; ip[q].xl = b.x; ip[q].yl = b.y; ip[q].zl = b.z; ip[q].inv_ro = b.w;
-            ip[q].ax = ip[q].ay = ip[q].az = ip[q].pot = 0.0f;
-        }
-        Acc64 acc[2] = {{0, 0, 0, 0}, {0, 0, 0, 0}};
         const int ig0 = gb + 2 * pslot;
-
-        // ---- super-particles -----------------------------------------------------------------
+        const int ig1 = min(ig0 + 1, gb + n_i - 1);          // odd n_i: the last slot duplicates a particle (result dropped)
+        const float4 ia0 = pa[ig0], ib0 = pb[ig0], ia1 = pa[ig1], ib1 = pb[ig1];
+        // group centre relative to the root centre, as float-float
+        float3 gh, gl;
         {
-            int chunk = gr->head_sp, remaining = gr->n_sp;
-            while (chunk >= 0 && remaining > 0) {
-                const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
-                const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
-                for (int off = 0; off < ne; off += SP_TILE) {
-                    const int tn = min(SP_TILE, ne - off);
-                    __syncthreads();
-                    for (int k = t; k < tn; k += FT) {
-                        const int id = cp[PETAR_CHUNK_HDR + off + k];
-                        const NodeSp* s = &nsp[id];
-                        sm.sp.q0[k] = s->q0; sm.sp.q1[k] = s->q1;
-                        if (QUAD) sm.sp.q2[k] = s->q2;
-                    }
-                    __syncthreads();
-                    if (active) {
-                        for (int j = slice; j < tn; j += S) {
-                            const float4 a = sm.sp.q0[j], b = sm.sp.q1[j];
-                            float4 c = make_float4(0.f, 0.f, 0.f, 0.f);
-                            if (QUAD) c = sm.sp.q2[j];
-                            sp_interact(ip[0], a, b, c, QUAD);
-                            sp_interact(ip[1], a, b, c, QUAD);
-                        }
-                        flush(ip[0], acc[0]); flush(ip[1], acc[1]);
-                    }
-                }
-                remaining -= ne;
-                chunk = cp[0];
-            }
+            const double cx = 0.5 * (gr->lo[0] + gr->hi[0]) - rcx, cy = 0.5 * (gr->lo[1] + gr->hi[1]) - rcy, cz = 0.5 * (gr->lo[2] + gr->hi[2]) - rcz;
+            gh = make_float3((float)cx, (float)cy, (float)cz);
+            gl = make_float3((float)(cx - (double)gh.x), (float)(cy - (double)gh.y), (float)(cz - (double)gh.z));
         }
-        // ---- particles: near ranges (changeover) then far ranges (plain Newtonian) ----------------
+        Acc64 acc0 = {0, 0, 0, 0}, acc1 = {0, 0, 0, 0};
+
+        sp_phase<QUAD, false>(sm, arena, nsp, gr->head_sp, gr->n_sp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
+        sp_phase<QUAD, true>(sm, arena, nsp, gr->head_spp, gr->n_spp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
+
+        // ---- particles: near ranges (changeover) then far ranges (plain Newtonian), float-float ----------
+        {
+            IFF i0 = {-ia0.x, -ia0.y, -ia0.z, -ib0.x, -ib0.y, -ib0.z, ib0.w};
+            IFF i1 = {-ia1.x, -ia1.y, -ia1.z, -ib1.x, -ib1.y, -ib1.z, ib1.w};
+            Acc32 p0 = {0.f, 0.f, 0.f, 0.f}, p1 = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll 1
-        for (int pass = 0; pass < 2; ++pass) {
-            int chunk = pass == 0 ? gr->head_epn : gr->head_epf;
-            int remaining = 2 * (pass == 0 ? gr->n_epn : gr->n_epf);
-            while (chunk >= 0 && remaining > 0) {
-                const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
-                const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
-                for (int off = 0; off < ne; off += 2 * EP_BATCH) {
-                    // one range per thread, block scan of the range sizes
-                    int jb = 0, cnt = 0;
-                    if (off + 2 * t < ne) { jb = cp[PETAR_CHUNK_HDR + off + 2 * t]; cnt = cp[PETAR_CHUNK_HDR + off + 2 * t + 1] - jb; }
-                    int incl = cnt;
+            for (int pass = 0; pass < 2; ++pass) {
+                int chunk = pass == 0 ? gr->head_epn : gr->head_epf;
+                int remaining = 2 * (pass == 0 ? gr->n_epn : gr->n_epf);
+                while (chunk >= 0 && remaining > 0) {
+                    const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
+                    const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+                    for (int off = 0; off < ne; off += 2 * FT) {
+                        // one range per thread, block scan of the range sizes
+                        int jb = 0, cnt = 0;
+                        if (off + 2 * t < ne) { jb = cp[PETAR_CHUNK_HDR + off + 2 * t]; cnt = cp[PETAR_CHUNK_HDR + off + 2 * t + 1] - jb; }
+                        int incl = cnt;
 #pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) { int v = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += v; }
-                    __syncthreads();                       // previous tile consumed; s_scan free
-                    if (lane == 31) s_scan[wrp] = incl;
-                    __syncthreads();
-                    int woff = 0, total = 0;
-#pragma unroll
-                    for (int ww = 0; ww < FT / 32; ++ww) { int v = s_scan[ww]; if (ww < wrp) woff += v; total += v; }
-                    const int my0 = woff + incl - cnt;     // exclusive offset of my range
-                    for (int w0 = 0; w0 < total; w0 += EP_TILE) {
-                        if (w0) __syncthreads();
-                        const int lo = max(my0, w0), hi = min(my0 + cnt, w0 + EP_TILE);
-                        for (int q = lo; q < hi; ++q) {
-                            const int j = jb + (q - my0);
-                            sm.ep.a[q - w0] = pa[j]; sm.ep.b[q - w0] = pb[j];
-                            if (pass == 0) sm.ep.j[q - w0] = j;
-                        }
+                        for (int o = 1; o < 32; o <<= 1) { int vv = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += vv; }
+                        __syncthreads();                       // previous tile consumed; s_scan free
+                        if (lane == 31) s_scan[wrp] = incl;
                         __syncthreads();
-                        const int tn = min(EP_TILE, total - w0);
-                        if (active) {
-                            if (pass == 0) {
-                                for (int j = slice; j < tn; j += S) {
-                                    const float4 a = sm.ep.a[j], b = sm.ep.b[j];
-                                    const int jg = sm.ep.j[j];
-                                    ep_interact<true>(ip[0], a, b, fc, jg == ig0);
-                                    ep_interact<true>(ip[1], a, b, fc, jg == ig0 + 1);
-                                }
-                            } else {
-                                for (int j = slice; j < tn; j += S) {
-                                    const float4 a = sm.ep.a[j], b = sm.ep.b[j];
-                                    ep_interact<false>(ip[0], a, b, fc, false);
-                                    ep_interact<false>(ip[1], a, b, fc, false);
-                                }
+                        int woff = 0, total = 0;
+#pragma unroll
+                        for (int ww = 0; ww < FT / 32; ++ww) { int vv = s_scan[ww]; if (ww < wrp) woff += vv; total += vv; }
+                        const int my0 = woff + incl - cnt;     // exclusive offset of my range
+                        for (int w0 = 0; w0 < total; w0 += EP_TILE) {
+                            if (w0) __syncthreads();
+                            const int lo = max(my0, w0), hi = min(my0 + cnt, w0 + EP_TILE);
+                            for (int q = lo; q < hi; ++q) {
+                                const int j = jb + (q - my0);
+                                sm.ep.a[q - w0] = pa[j]; sm.ep.b[q - w0] = pb[j];
+                                if (pass == 0) sm.ep.j[q - w0] = j;
                             }
-                            flush(ip[0], acc[0]); flush(ip[1], acc[1]);
+                            __syncthreads();
+                            const int tn = min(EP_TILE, total - w0);
+                            if (active) {
+                                if (pass == 0) {
+                                    for (int j = slice; j < tn; j += S) {
+                                        const float4 a = sm.ep.a[j], b = sm.ep.b[j];
+                                        const int jg = sm.ep.j[j];
+                                        ep_near_one(p0, i0, a, b, fc, jg == ig0);
+                                        ep_near_one(p1, i1, a, b, fc, jg == ig1);
+                                    }
+                                } else {
+#pragma unroll 2
+                                    for (int j = slice; j < tn; j += S) {
+                                        const float4 a = sm.ep.a[j], b = sm.ep.b[j];
+                                        ep_far_one(p0, i0, a, b);
+                                        ep_far_one(p1, i1, a, b);
+                                    }
+                                }
+                                flush(p0, acc0); flush(p1, acc1);
+                            }
                         }
                     }
+                    remaining -= ne;
+                    chunk = cp[0];
                 }
-                remaining -= ne;
-                chunk = cp[0];
             }
         }
         // ---- ordered reduction over slices, then scatter to the caller's order --------------------
         __syncthreads();
         if (active) {
             double* r = &sm.red[(size_t)(slice * (2 * P) + 2 * pslot) * 4];
-            r[0] = acc[0].ax; r[1] = acc[0].ay; r[2] = acc[0].az; r[3] = acc[0].pot;
-            r[4] = acc[1].ax; r[5] = acc[1].ay; r[6] = acc[1].az; r[7] = acc[1].pot;
+            r[0] = acc0.ax; r[1] = acc0.ay; r[2] = acc0.az; r[3] = acc0.pot;
+            r[4] = acc1.ax; r[5] = acc1.ay; r[6] = acc1.az; r[7] = acc1.pot;
         }
         __syncthreads();
         for (int k = t; k < n_i * 4; k += FT) {
             const int i = k >> 2, comp = k & 3;
             double s = 0.0;
             for (int sl = 0; sl < S; ++sl) s += sm.red[(size_t)(sl * (2 * P) + i) * 4 + comp];
-            const int ig = gb + i;
-            const unsigned o = perm[ig];
-            if (comp == 3) {
-                if (opot) opot[o] = G * s;
-            } else {
+            const unsigned o = perm[gb + i];
+            if (comp == 3) { if (opot) opot[o] = -G * s; }
+            else {
                 double* dst = comp == 0 ? oax : comp == 1 ? oay : oaz;
                 if (dst) dst[o] = G * s;
             }
@@ -280,9 +384,9 @@ cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, doub
     if (per_sm < 1) per_sm = 1;
     const int grid = t->sm_count * per_sm;
     if (t->p.multipole >= 2)
-        k_force<true><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.ms, w.routs, ax, ay, az, pot, fc, t->p.G, 1.0 + lam);
+        k_force<true><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, ax, ay, az, pot, fc, t->p.G);
     else
-        k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.ms, w.routs, ax, ay, az, pot, fc, t->p.G, 1.0 + lam);
+        k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, ax, ay, az, pot, fc, t->p.G);
     KCHECK(s, "k_force");
     petar_count_launch(2);
     stage_end(t, PETAR_STAGE_FORCE, s);

@@ -39,8 +39,8 @@ struct __align__(16) NodeMac { double lo[3]; double hi[3]; double com[3]; double
 // moments kept for the bottom-up pass / export
 struct __align__(16) NodeMom { double M; double S[3]; double Q[6]; };
 // fp32 super-particle record for the force kernel: 12 floats = 48 B
-//  q0 = (xh, yh, zh, M) ; q1 = (xl, yl, zl, Axx) ; q2 = (Ayy, Axy, Axz, Ayz) ;  Azz = -(Axx + Ayy)
-//  (xh + xl) = com - c_root in float-float; A = 1.5 Q - 0.5 tr(Q) I  (Eq. 31, traceless)
+//  q0 = (xh, yh, zh, M) ; q1 = (xl, yl, zl, Bxx) ; q2 = (Byy, Bxy, Bxz, Byz) ;  Bzz = -(Bxx + Byy)
+//  (xh + xl) = com - c_root in float-float; B = -2 A, A = 1.5 Q - 0.5 tr(Q) I  (Eq. 31, traceless)
 struct __align__(16) NodeSp { float4 q0, q1, q2; };
 
 struct __align__(16) GroupRec {
@@ -48,7 +48,7 @@ struct __align__(16) GroupRec {
     int head_sp, head_epn, head_epf;   // first chunk of each list (-1 = empty)
     int n_sp, n_epn, n_epf;            // entries: cells, near ranges, far ranges
     int n_ep_part, n_epn_part;         // particles in all EP ranges / in near ranges
-    int pad0, pad1;
+    int head_spp, n_spp;               // cells closer than the group's own size: float-float ("precise") path
     double lo[3], hi[3], rmax;
     double pad2;
 };

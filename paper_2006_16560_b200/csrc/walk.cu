@@ -72,8 +72,12 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
         const double ghi0 = gr->hi[0], ghi1 = gr->hi[1], ghi2 = gr->hi[2];
         const double grmax = gr->rmax;
         const int n_i = gr->end - gr->begin;
-        ListCursor lsp = {-1, -1, 0, 0}, lepn = {-1, -1, 0, 0}, lepf = {-1, -1, 0, 0};
-        int n_sp = 0, n_epn = 0, n_epf = 0, n_ep_part = 0, n_epn_part = 0;
+        ListCursor lsp = {-1, -1, 0, 0}, lspp = {-1, -1, 0, 0}, lepn = {-1, -1, 0, 0}, lepf = {-1, -1, 0, 0};
+        int n_sp = 0, n_spp = 0, n_epn = 0, n_epf = 0, n_ep_part = 0, n_epn_part = 0;
+        // cells closer to the group's box than the box's longest edge go to the "precise" list: the force
+        // kernel evaluates them with float-float coordinates, all others with group-relative floats
+        const double gedge = fmax(ghi0 - glo0, fmax(ghi1 - glo1, ghi2 - glo2));
+        const double gedge2 = gedge * gedge;
         int top = 1;
         if (lane == 0) stack[0] = 0;
         __syncwarp();
@@ -83,7 +87,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
             const int node = (lane < p) ? stack[top - p + lane] : -1;
             top -= p;
             __syncwarp();
-            int act = -1;                      // 0 SP, 1 EP near, 2 EP far, 3 open
+            int act = -1;                      // 0 SP, 1 EP near, 2 EP far, 3 open, 4 SP (precise list)
             int nb = 0, ne = 0, fc = 0, nch = 0;
             if (node >= 0) {
                 const NodeInt ni = nint[node];
@@ -104,15 +108,17 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
                 double edge = ldexp(twoh, -level);
                 bool farb = (edge * edge) < theta2 * d2com;
                 nb = ni.begin; ne = ni.end; fc = ni.first_child; nch = (ni.meta >> 8) & 15;
-                if (!nearb && farb) act = 0;
+                if (!nearb && farb) act = (d2box < gedge2) ? 4 : 0;
                 else if (leaf) act = nearb ? 1 : 2;
                 else act = 3;
             }
             // outputs
             list_append(lsp, act == 0, 1, node, 0, arena, arena_chunks, h, lane);
+            list_append(lspp, act == 4, 1, node, 0, arena, arena_chunks, h, lane);
             list_append(lepn, act == 1, 2, nb, ne, arena, arena_chunks, h, lane);
             list_append(lepf, act == 2, 2, nb, ne, arena, arena_chunks, h, lane);
             n_sp += __popc(__ballot_sync(0xffffffffu, act == 0));
+            n_spp += __popc(__ballot_sync(0xffffffffu, act == 4));
             n_epn += __popc(__ballot_sync(0xffffffffu, act == 1));
             n_epf += __popc(__ballot_sync(0xffffffffu, act == 2));
             int cn = (act == 1) ? (ne - nb) : 0, cf = (act == 2) ? (ne - nb) : 0;
@@ -141,13 +147,14 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
             GroupRec* go = &grp[g];
             go->head_sp = lsp.head; go->head_epn = lepn.head; go->head_epf = lepf.head;
             go->n_sp = n_sp; go->n_epn = n_epn; go->n_epf = n_epf;
+            go->head_spp = lspp.head; go->n_spp = n_spp;
             go->n_ep_part = n_ep_part; go->n_epn_part = n_epn_part;
         }
         t_epep += (unsigned long long)n_i * (unsigned long long)n_ep_part;
         t_near += (unsigned long long)n_i * (unsigned long long)n_epn_part;
-        t_epsp += (unsigned long long)n_i * (unsigned long long)n_sp;
+        t_epsp += (unsigned long long)n_i * (unsigned long long)(n_sp + n_spp);
         t_eplist += (unsigned long long)(n_epn + n_epf);
-        t_splist += (unsigned long long)n_sp;
+        t_splist += (unsigned long long)(n_sp + n_spp);
     }
     if (lane == 0) {
         atomicAdd(&h->n_epep, t_epep); atomicAdd(&h->n_epsp, t_epsp); atomicAdd(&h->n_epep_near, t_near);
@@ -272,7 +279,7 @@ cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, 
 __global__ void k_list_sizes(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, int* __restrict__ sizes) {
     int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= h->n_groups) return;
-    sizes[3 * g] = grp[g].n_sp; sizes[3 * g + 1] = 2 * grp[g].n_epn; sizes[3 * g + 2] = 2 * grp[g].n_epf;
+    sizes[3 * g] = grp[g].n_sp + grp[g].n_spp; sizes[3 * g + 1] = 2 * grp[g].n_epn; sizes[3 * g + 2] = 2 * grp[g].n_epf;
 }
 __global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
                                const long long* __restrict__ offs, int* __restrict__ out, long long out_entries) {
@@ -283,17 +290,21 @@ __global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* 
     int chunk = which == 0 ? grp[g].head_sp : which == 1 ? grp[g].head_epn : grp[g].head_epf;
     int remaining = which == 0 ? grp[g].n_sp : which == 1 ? 2 * grp[g].n_epn : 2 * grp[g].n_epf;
     long long o = offs[wid];
-    while (chunk >= 0 && remaining > 0) {
-        const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
-        int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
-        for (int e = lane; e < ne; e += 32) if (o + e < out_entries) out[o + e] = cp[PETAR_CHUNK_HDR + e];
-        o += ne; remaining -= ne; chunk = cp[0];
+    for (int part = 0; part < 2; ++part) {
+        while (chunk >= 0 && remaining > 0) {
+            const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
+            int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+            for (int e = lane; e < ne; e += 32) if (o + e < out_entries) out[o + e] = cp[PETAR_CHUNK_HDR + e];
+            o += ne; remaining -= ne; chunk = cp[0];
+        }
+        if (which != 0) break;
+        chunk = grp[g].head_spp; remaining = grp[g].n_spp;       // "SP" = plain cells, then precise cells
     }
 }
 __global__ void k_group_cnt(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, int* __restrict__ out, int what) {
     int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= h->n_groups) return;
-    if (what == PETAR_DBG_GROUP_CNT) { out[4 * g] = grp[g].n_sp; out[4 * g + 1] = grp[g].n_epn; out[4 * g + 2] = grp[g].n_epf; out[4 * g + 3] = grp[g].n_ep_part; }
+    if (what == PETAR_DBG_GROUP_CNT) { out[4 * g] = grp[g].n_sp + grp[g].n_spp; out[4 * g + 1] = grp[g].n_epn; out[4 * g + 2] = grp[g].n_epf; out[4 * g + 3] = grp[g].n_ep_part; }
     else { out[2 * g] = grp[g].begin; out[2 * g + 1] = grp[g].end; }
 }
 __global__ void k_group_dbl(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, double* __restrict__ out) {
