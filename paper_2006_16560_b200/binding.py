@@ -5,7 +5,7 @@ import ctypes as C
 import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(HERE, "libpetar_b200.so")
+_LIB_PATH = os.environ.get("PETAR_B200_LIB", os.path.join(HERE, "libpetar_b200.so"))   # override: tuning experiments only
 _LIB = None
 
 EXPORTS = [

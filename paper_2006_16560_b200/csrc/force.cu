@@ -24,7 +24,13 @@
 #include "internal.cuh"
 
 #define FT 128                 // threads per CTA
-#define SP_TILE 256            // cells per staged tile (two per thread)
+#ifndef SP_REC
+#define SP_REC 2               // staged cells per thread per tile
+#endif
+#define SP_TILE (SP_REC * FT)  // cells per staged tile
+#ifndef FORCE_MIN_CTAS
+#define FORCE_MIN_CTAS 4
+#endif
 #define EP_TILE 512            // particles per staged tile
 
 struct ForceConst {
@@ -167,22 +173,24 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
     Acc32 p0 = {0.f, 0.f, 0.f, 0.f}, p1 = {0.f, 0.f, 0.f, 0.f};
     TileCursor cur; cur.init(arena, head, n);
     int tn0 = 0, tn1 = 0, tn2 = 0;
-    int id2[2] = {0, 0};
-    float4 q0[2], q1[2], q2[2];
+    int id2[SP_REC];
+    float4 q0[SP_REC], q1[SP_REC], q2[SP_REC];
+#pragma unroll
+    for (int r = 0; r < SP_REC; ++r) id2[r] = 0;
     auto load_ids = [&]() {
         tn2 = cur.count();
 #pragma unroll
-        for (int r = 0; r < 2; ++r) if (t + r * FT < tn2) id2[r] = cur.cp[PETAR_CHUNK_HDR + cur.off + t + r * FT];
+        for (int r = 0; r < SP_REC; ++r) if (t + r * FT < tn2) id2[r] = cur.cp[PETAR_CHUNK_HDR + cur.off + t + r * FT];
         cur.advance(arena, tn2);
     };
     auto load_recs = [&]() {
         tn1 = tn2;
 #pragma unroll
-        for (int r = 0; r < 2; ++r) if (t + r * FT < tn1) { const NodeSp* sp = &nsp[id2[r]]; q0[r] = sp->q0; q1[r] = sp->q1; if (QUAD) q2[r] = sp->q2; }
+        for (int r = 0; r < SP_REC; ++r) if (t + r * FT < tn1) { const NodeSp* sp = &nsp[id2[r]]; q0[r] = sp->q0; q1[r] = sp->q1; if (QUAD) q2[r] = sp->q2; }
     };
     auto store_recs = [&](SpBuf& bf) {
 #pragma unroll
-        for (int r = 0; r < 2; ++r) {
+        for (int r = 0; r < SP_REC; ++r) {
             const int k = t + r * FT;
             if (k < tn1) {
                 const float bzz = -(q1[r].w + q2[r].x);
@@ -237,7 +245,7 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
 }
 
 template <bool QUAD>
-__global__ void __launch_bounds__(FT, 4) k_force(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
+__global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
                                                  const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
                                                  const unsigned* __restrict__ perm,
                                                  double* __restrict__ oax, double* __restrict__ oay, double* __restrict__ oaz, double* __restrict__ opot,
