@@ -82,6 +82,7 @@ static size_t carve(Workspace* w, char* base, int64_t N, const petar_params* p) 
     W->nmac = (NodeMac*)take((size_t)W->node_cap * sizeof(NodeMac));
     W->nmom = (NodeMom*)take((size_t)W->node_cap * sizeof(NodeMom));
     W->nsp = (NodeSp*)take((size_t)W->node_cap * sizeof(NodeSp));
+    W->nw = (NodeW*)take((size_t)W->node_cap * sizeof(NodeW));
     W->group_cap = (int)N + 1;
     W->grp = (GroupRec*)take((size_t)W->group_cap * sizeof(GroupRec));
     W->nb_cnt = (int*)take(n * 4);

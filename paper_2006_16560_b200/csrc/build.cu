@@ -422,7 +422,7 @@ __global__ void __launch_bounds__(RANK_THREADS) k_nodes_write(const unsigned lon
 // rule O5: leaf = members in sorted order with S = fma(m, x, S); internal = children ascending.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_moments(const DevHeader* __restrict__ h, NodeInt* __restrict__ nint, NodeMac* __restrict__ nmac,
-                                                 NodeMom* __restrict__ nmom, NodeSp* __restrict__ nsp,
+                                                 NodeMom* __restrict__ nmom, NodeSp* __restrict__ nsp, NodeW* __restrict__ nw,
                                                  const unsigned long long* __restrict__ key,
                                                  const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
                                                  const double* __restrict__ ms, const double* __restrict__ rss, int node_cap, int multipole) {
@@ -487,7 +487,8 @@ __global__ void __launch_bounds__(256) k_moments(const DevHeader* __restrict__ h
                     Q[0] += cm.Q[0] + cm.M * dx * dx; Q[1] += cm.Q[1] + cm.M * dy * dy; Q[2] += cm.Q[2] + cm.M * dz * dz;
                     Q[3] += cm.Q[3] + cm.M * dx * dy; Q[4] += cm.Q[4] + cm.M * dx * dz; Q[5] += cm.Q[5] + cm.M * dy * dz;
                 }
-                nint[id].meta = r.meta | (nchild << 8);
+                r.meta |= (nchild << 8);
+                nint[id].meta = r.meta;
             }
             NodeMac mac;
             mac.lo[0] = lo0; mac.lo[1] = lo1; mac.lo[2] = lo2; mac.hi[0] = hi0; mac.hi[1] = hi1; mac.hi[2] = hi2;
@@ -513,6 +514,18 @@ __global__ void __launch_bounds__(256) k_moments(const DevHeader* __restrict__ h
                 sp.q2 = make_float4(0.f, 0.f, 0.f, 0.f);
             }
             nsp[id] = sp;
+            // fp32 walk record: coordinates relative to the root centre, error bound eps
+            {
+                NodeW wr;
+                const float l0 = (float)(lo0 - cx), l1 = (float)(lo1 - cy), l2 = (float)(lo2 - cz);
+                const float h0 = (float)(hi0 - cx), h1 = (float)(hi1 - cy), h2 = (float)(hi2 - cz);
+                const float amax = fmaxf(fmaxf(fmaxf(fabsf(l0), fabsf(h0)), fmaxf(fabsf(l1), fabsf(h1))), fmaxf(fabsf(l2), fabsf(h2)));
+                wr.a = make_float4(l0, l1, l2, h0);
+                wr.b = make_float4(h1, h2, xh, yh);
+                wr.c = make_float4(zh, (float)rmax, amax * 4.8e-7f, 0.f);
+                wr.d = make_int4(r.begin, r.end, r.first_child, r.meta);
+                nw[id] = wr;
+            }
         }
         grid.sync();
     }
@@ -737,7 +750,7 @@ cudaError_t launch_tree(petar_tree* t, cudaStream_t s) {
         const DevHeader* hdr = w.hdr;
         const double* rss = t->r_search ? w.rss : w.routs;
         int cap = w.node_cap, mult = t->p.multipole;
-        void* args[] = {(void*)&hdr, (void*)&w.nint, (void*)&w.nmac, (void*)&w.nmom, (void*)&w.nsp, (void*)&w.key,
+        void* args[] = {(void*)&hdr, (void*)&w.nint, (void*)&w.nmac, (void*)&w.nmom, (void*)&w.nsp, (void*)&w.nw, (void*)&w.key,
                         (void*)&w.xs, (void*)&w.ys, (void*)&w.zs, (void*)&w.ms, (void*)&rss, (void*)&cap, (void*)&mult};
         e = cudaLaunchCooperativeKernel((void*)k_moments, dim3(grid), dim3(256), args, 0, s);
         if (e != cudaSuccess) return e;

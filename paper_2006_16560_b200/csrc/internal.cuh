@@ -36,6 +36,10 @@ struct DevHeader {
 struct __align__(16) NodeInt { int begin, end, first_child, meta; };
 // MAC record (fp64, exact decisions): lo[3], hi[3], com[3], rmax  -> 10 doubles = 80 B
 struct __align__(16) NodeMac { double lo[3]; double hi[3]; double com[3]; double rmax; };
+// fp32 walk record (64 B): conservative pre-test of the MAC; the fp64 NodeMac decides ambiguous cases.
+//  a = (lox, loy, loz, hix) ; b = (hiy, hiz, comx, comy) ; c = (comz, rmax, eps, 0) ; d = (begin, end, first_child, meta)
+//  coordinates relative to the root centre; eps = 2^-21 * max |box coordinate| bounds the fp32 error (walk.cu)
+struct __align__(16) NodeW { float4 a, b, c; int4 d; };
 // moments kept for the bottom-up pass / export
 struct __align__(16) NodeMom { double M; double S[3]; double Q[6]; };
 // fp32 super-particle record for the force kernel: 12 floats = 48 B
@@ -70,7 +74,7 @@ struct Workspace {
     int *tile_cnt;                 // [22][ntile]
     int *scan_tmp;                 // scan partials
     // nodes
-    NodeInt* nint; NodeMac* nmac; NodeMom* nmom; NodeSp* nsp;
+    NodeInt* nint; NodeMac* nmac; NodeMom* nmom; NodeSp* nsp; NodeW* nw;
     int node_cap;
     // groups
     GroupRec* grp; int group_cap;

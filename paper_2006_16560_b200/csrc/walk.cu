@@ -4,7 +4,7 @@
 #include "internal.cuh"
 
 #define WALK_WARPS 8
-#define WALK_STACK 1536          // frontier entries per warp (shared memory)
+#define WALK_STACK 1504          // frontier entries per warp (shared memory)
 
 // warp-uniform cursor of one chunked list
 struct ListCursor {
@@ -51,16 +51,50 @@ __device__ __forceinline__ void list_append(ListCursor& c, bool take, int per, i
     c.pos = n * per - space;
 }
 
-__global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict__ h, const NodeInt* __restrict__ nint,
+// fp64 MAC of rule O7 (exactly this operation order); returns act: 0 SP, 1 EP near, 2 EP far, 3 open
+__device__ __forceinline__ int mac_exact(const NodeMac& c, const int level, const bool leaf,
+                                         const double glo0, const double glo1, const double glo2,
+                                         const double ghi0, const double ghi1, const double ghi2,
+                                         const double grmax, const double theta2, const double twoh) {
+    double gx = fmax(0.0, fmax(c.lo[0] - ghi0, glo0 - c.hi[0]));
+    double gy = fmax(0.0, fmax(c.lo[1] - ghi1, glo1 - c.hi[1]));
+    double gz = fmax(0.0, fmax(c.lo[2] - ghi2, glo2 - c.hi[2]));
+    double d2box = fma(gz, gz, fma(gy, gy, gx * gx));
+    double R = fmax(grmax, c.rmax);
+    bool nearb = d2box < R * R;
+    double px = fmax(0.0, fmax(glo0 - c.com[0], c.com[0] - ghi0));
+    double py = fmax(0.0, fmax(glo1 - c.com[1], c.com[1] - ghi1));
+    double pz = fmax(0.0, fmax(glo2 - c.com[2], c.com[2] - ghi2));
+    double d2com = fma(pz, pz, fma(py, py, px * px));
+    double edge = ldexp(twoh, -level);
+    bool farb = (edge * edge) < theta2 * d2com;
+    if (!nearb && farb) return 0;
+    if (leaf) return nearb ? 1 : 2;
+    return 3;
+}
+
+// The walk decides every cell in fp32 first, with a rigorous error band, and falls back to the fp64
+// test of rule O7 only when the fp32 values cannot decide (so the decisions are exactly O7's).
+// fp32 coordinates q32 = fl32(q - c_root) carry |error| <= 2^-24 |q - c_root|.  With A_c, A_g the largest
+// |coordinate| of the cell's / group's box, a computed distance differs from the exact one by less than
+// 8 * 2^-24 (A_c + A_g) = eps_c + eps_g (component differences: 2(u_c+u_g) each; norm: 2 sqrt(3)(u_c+u_g);
+// rounding of the sum of squares: < 2.6 (u_c+u_g)); thresholds get a further relative 2^-22 for their own
+// rounding and the fp32 conversion of rmax and of the per-level edge/theta.
+#define WALK_RESERVE 160         // > 7 * 21: room for a pure depth-first descent from any state
+__global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
                                                           const NodeMac* __restrict__ nmac, GroupRec* __restrict__ grp,
                                                           int* __restrict__ arena, int arena_chunks, double theta, int node_cap) {
     __shared__ int s_stack[WALK_WARPS][WALK_STACK];
+    __shared__ float s_lt[PETAR_NLEVELS];          // edge(level) / theta  (inf when theta == 0: nothing is ever "far")
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     int* stack = s_stack[w];
     const int ng = h->n_groups;
     if (h->n_nodes > node_cap || h->n_nodes <= 0) return;
     const double theta2 = theta * theta;
     const double twoh = 2.0 * h->h;
+    const double rcx = h->c[0], rcy = h->c[1], rcz = h->c[2];
+    if (threadIdx.x < PETAR_NLEVELS) s_lt[threadIdx.x] = (theta > 0.0) ? (float)(ldexp(twoh, -(int)threadIdx.x) / theta) : INFINITY;
+    __syncthreads();
     unsigned long long t_epep = 0, t_epsp = 0, t_near = 0, t_eplist = 0, t_splist = 0;
     for (;;) {
         int g = 0;
@@ -72,45 +106,60 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
         const double ghi0 = gr->hi[0], ghi1 = gr->hi[1], ghi2 = gr->hi[2];
         const double grmax = gr->rmax;
         const int n_i = gr->end - gr->begin;
+        // fp32 copy of the group's box (relative to the root centre) and its error bound
+        const float fl0 = (float)(glo0 - rcx), fl1 = (float)(glo1 - rcy), fl2 = (float)(glo2 - rcz);
+        const float fh0 = (float)(ghi0 - rcx), fh1 = (float)(ghi1 - rcy), fh2 = (float)(ghi2 - rcz);
+        const float frm = (float)grmax;
+        const float geps = 4.8e-7f * fmaxf(fmaxf(fmaxf(fabsf(fl0), fabsf(fh0)), fmaxf(fabsf(fl1), fabsf(fh1))), fmaxf(fabsf(fl2), fabsf(fh2)));
         ListCursor lsp = {-1, -1, 0, 0}, lspp = {-1, -1, 0, 0}, lepn = {-1, -1, 0, 0}, lepf = {-1, -1, 0, 0};
         int n_sp = 0, n_spp = 0, n_epn = 0, n_epf = 0, n_ep_part = 0, n_epn_part = 0;
         // cells closer to the group's box than the box's longest edge go to the "precise" list: the force
         // kernel evaluates them with float-float coordinates, all others with group-relative floats
-        const double gedge = fmax(ghi0 - glo0, fmax(ghi1 - glo1, ghi2 - glo2));
-        const double gedge2 = gedge * gedge;
+        const float gedge = fmaxf(fh0 - fl0, fmaxf(fh1 - fl1, fh2 - fl2));
+        const float gedge2 = gedge * gedge;
         int top = 1;
         if (lane == 0) stack[0] = 0;
         __syncwarp();
         while (top > 0) {
+            // pop up to 32 nodes; throttle towards depth-first order when the frontier nears its capacity
+            // (a pure depth-first descent adds at most 7 entries per level, < WALK_RESERVE in total)
             int p = min(32, top);
-            if (top - p + 8 * p > WALK_STACK) p = max(1, (WALK_STACK - top) / 7);
+            if (top + 7 * p > WALK_STACK - WALK_RESERVE) p = max(1, min(p, (WALK_STACK - WALK_RESERVE - top) / 7));
             const int node = (lane < p) ? stack[top - p + lane] : -1;
             top -= p;
             __syncwarp();
             int act = -1;                      // 0 SP, 1 EP near, 2 EP far, 3 open, 4 SP (precise list)
             int nb = 0, ne = 0, fc = 0, nch = 0;
             if (node >= 0) {
-                const NodeInt ni = nint[node];
-                const NodeMac c = nmac[node];
-                const int level = ni.meta & 255;
-                const bool leaf = (ni.meta >> 16) & 1;
-                // O7, exactly this operation order
-                double gx = fmax(0.0, fmax(c.lo[0] - ghi0, glo0 - c.hi[0]));
-                double gy = fmax(0.0, fmax(c.lo[1] - ghi1, glo1 - c.hi[1]));
-                double gz = fmax(0.0, fmax(c.lo[2] - ghi2, glo2 - c.hi[2]));
-                double d2box = fma(gz, gz, fma(gy, gy, gx * gx));
-                double R = fmax(grmax, c.rmax);
-                bool nearb = d2box < R * R;
-                double px = fmax(0.0, fmax(glo0 - c.com[0], c.com[0] - ghi0));
-                double py = fmax(0.0, fmax(glo1 - c.com[1], c.com[1] - ghi1));
-                double pz = fmax(0.0, fmax(glo2 - c.com[2], c.com[2] - ghi2));
-                double d2com = fma(pz, pz, fma(py, py, px * px));
-                double edge = ldexp(twoh, -level);
-                bool farb = (edge * edge) < theta2 * d2com;
-                nb = ni.begin; ne = ni.end; fc = ni.first_child; nch = (ni.meta >> 8) & 15;
-                if (!nearb && farb) act = (d2box < gedge2) ? 4 : 0;
-                else if (leaf) act = nearb ? 1 : 2;
-                else act = 3;
+                const NodeW c = nw[node];
+                const int meta = c.d.w;
+                const int level = meta & 255;
+                const bool leaf = (meta >> 16) & 1;
+                nb = c.d.x; ne = c.d.y; fc = c.d.z; nch = (meta >> 8) & 15;
+                // ---- fp32 pre-test with error band --------------------------------------------------------
+                const float gx = fmaxf(0.f, fmaxf(c.a.x - fh0, fl0 - c.a.w));
+                const float gy = fmaxf(0.f, fmaxf(c.a.y - fh1, fl1 - c.b.x));
+                const float gz = fmaxf(0.f, fmaxf(c.a.z - fh2, fl2 - c.b.y));
+                const float d2b = fmaf(gz, gz, fmaf(gy, gy, gx * gx));
+                const float px = fmaxf(0.f, fmaxf(fl0 - c.b.z, c.b.z - fh0));
+                const float py = fmaxf(0.f, fmaxf(fl1 - c.b.w, c.b.w - fh1));
+                const float pz = fmaxf(0.f, fmaxf(fl2 - c.c.x, c.c.x - fh2));
+                const float d2c = fmaf(pz, pz, fmaf(py, py, px * px));
+                const float D = geps + c.c.z;
+                const float R = fmaxf(frm, c.c.y);
+                const float Dr = fmaf(R, 2.4e-7f, D);
+                const float Rm = fmaxf(R - Dr, 0.f), Rp = R + Dr;
+                const bool near_yes = d2b < Rm * Rm, near_no = d2b > Rp * Rp;
+                const float L = s_lt[level];
+                const float Dl = fmaf(L, 2.4e-7f, D);
+                const float Lm = fmaxf(L - Dl, 0.f), Lp = L + Dl;
+                const bool far_yes = d2c > Lp * Lp, far_no = d2c < Lm * Lm;      // L = inf: Lp*Lp = inf, never far
+                if (near_no && far_yes) act = 0;
+                else if (!leaf && (near_yes || far_no)) act = 3;
+                else if (leaf && near_yes) act = 1;
+                else if (leaf && near_no && far_no) act = 2;
+                else act = mac_exact(nmac[node], level, leaf, glo0, glo1, glo2, ghi0, ghi1, ghi2, grmax, theta2, twoh);
+                if (act == 0 && d2b < gedge2) act = 4;
             }
             // outputs
             list_append(lsp, act == 0, 1, node, 0, arena, arena_chunks, h, lane);
@@ -121,19 +170,18 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
             n_spp += __popc(__ballot_sync(0xffffffffu, act == 4));
             n_epn += __popc(__ballot_sync(0xffffffffu, act == 1));
             n_epf += __popc(__ballot_sync(0xffffffffu, act == 2));
-            int cn = (act == 1) ? (ne - nb) : 0, cf = (act == 2) ? (ne - nb) : 0;
-            int push = (act == 3) ? nch : 0;
+            const int cn = __reduce_add_sync(0xffffffffu, (act == 1) ? (ne - nb) : 0);
+            const int cf = __reduce_add_sync(0xffffffffu, (act == 2) ? (ne - nb) : 0);
+            const int push = (act == 3) ? nch : 0;
             int pref = push;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
-                cn += __shfl_xor_sync(0xffffffffu, cn, o);
-                cf += __shfl_xor_sync(0xffffffffu, cf, o);
                 int a = __shfl_up_sync(0xffffffffu, pref, o);
                 if (lane >= o) pref += a;
             }
             n_epn_part += cn; n_ep_part += cn + cf;
             const int total_push = __shfl_sync(0xffffffffu, pref, 31);
-            if (top + total_push > WALK_STACK) {                 // never expected
+            if (top + total_push > WALK_STACK) {                 // cannot happen (see the throttle above)
                 if (lane == 0) atomicOr(&h->status, PETAR_ST_STACK);
                 top = 0;
                 break;
@@ -175,7 +223,7 @@ cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_walk, WALK_WARPS * 32, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
-    k_walk<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nint, w.nmac, w.grp, w.arena, w.arena_chunks, t->p.theta, w.node_cap);
+    k_walk<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, w.nmac, w.grp, w.arena, w.arena_chunks, t->p.theta, w.node_cap);
     KCHECK(s, "k_walk");
     petar_count_launch(2);
     stage_end(t, PETAR_STAGE_WALK, s);
