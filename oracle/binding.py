@@ -203,11 +203,17 @@ class OracleTree:
                               C.c_int64(ep.shape[0]), _p(ep, C.c_int64), *[_p(o, C.c_double) for o in out])
         return tuple(out)
 
-    def neighbors(self):
+    def neighbors(self, groups=None):
+        """CSR neighbour list (rows ascending).  groups: only the particles of these i-groups get rows."""
         off = np.zeros(self.N + 1, dtype=np.int64)
         if self.N == 0:
             return off, np.zeros(0, dtype=np.int32)
-        _lib().ora_tree_neighbors(self._h, _p(off, C.c_int64), None)
+        if groups is None:
+            ns, sp = 0, None
+        else:
+            groups = np.ascontiguousarray(groups, dtype=np.int64)
+            ns, sp = groups.shape[0], _p(groups, C.c_int64)
+        _lib().ora_tree_neighbors_sel(self._h, C.c_int64(ns), sp, _p(off, C.c_int64), None)
         idx = np.zeros(max(int(off[-1]), 1), dtype=np.int32)
-        _lib().ora_tree_neighbors(self._h, _p(off, C.c_int64), _p(idx, C.c_int32))
+        _lib().ora_tree_neighbors_sel(self._h, C.c_int64(ns), sp, _p(off, C.c_int64), _p(idx, C.c_int32))
         return off, idx[: int(off[-1])]

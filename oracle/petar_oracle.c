@@ -564,11 +564,16 @@ void ora_eval_lists(const ora_tree *t, int64_t gb, int64_t ge, int64_t n_sp, con
 /* O9: neighbours from the walk's EP lists, fp64 test, ORIGINAL indices; rows sorted ascending.
  * Two-phase like the library: indices == NULL => offsets only.                                   */
 static int cmp_i32(const void *a, const void *b) { int32_t p = *(const int32_t *)a, q = *(const int32_t *)b; return (p > q) - (p < q); }
-void ora_tree_neighbors(const ora_tree *t, int64_t *offsets, int32_t *indices) {
+void ora_tree_neighbors_sel(const ora_tree *t, int64_t ns, const int64_t *sel, int64_t *offsets, int32_t *indices);
+void ora_tree_neighbors(const ora_tree *t, int64_t *offsets, int32_t *indices) { ora_tree_neighbors_sel(t, 0, NULL, offsets, indices); }
+/* Same for the particles of groups sel[0..ns) only (sel == NULL: all groups); other rows stay empty. */
+void ora_tree_neighbors_sel(const ora_tree *t, int64_t ns, const int64_t *sel, int64_t *offsets, int32_t *indices) {
     int64_t N = t->N;
+    int64_t ng = sel ? ns : t->n_grp;
     if (!indices) memset(offsets, 0, (size_t)(N + 1) * 8);
 #pragma omp parallel for schedule(dynamic, 4)
-    for (int64_t g = 0; g < t->n_grp; ++g) {
+    for (int64_t gs = 0; gs < ng; ++gs) {
+        int64_t g = sel ? sel[gs] : gs;
         ora_list l; memset(&l, 0, sizeof l); l.collect = 1;
         visit(t, &t->grp[g], 0, &l);
         for (int64_t i = t->grp[g].begin; i < t->grp[g].end; ++i) {

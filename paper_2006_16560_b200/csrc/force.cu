@@ -31,6 +31,12 @@
 #ifndef FORCE_MIN_CTAS
 #define FORCE_MIN_CTAS 4
 #endif
+#ifndef FORCE_UNROLL
+#define FORCE_UNROLL 2
+#endif
+#define PRAGMA_STR_(x) _Pragma(#x)
+#define PRAGMA_(x) PRAGMA_STR_(x)
+#define UNROLL_J PRAGMA_(unroll FORCE_UNROLL)
 #define EP_TILE 512            // particles per staged tile
 
 struct ForceConst {
@@ -134,13 +140,19 @@ union __align__(16) ForceSmem {
     double red[FT * 8];                                                // 8 KB
 };
 
-// uniform cursor over the tiles (<= SP_TILE entries, never straddling a chunk) of a chunked list
+// uniform cursor over the tiles (<= SP_TILE entries, never straddling a chunk) of TWO chunked lists in a
+// row (the super-group's common cells, then the group's own cells)
 struct TileCursor {
     const int* cp; int chunk, nxt, off, remaining;
-    __device__ __forceinline__ void init(const int* arena, int head, int n) {
+    int head_b, n_b;
+    __device__ __forceinline__ void start(const int* arena, int head, int n) {
         chunk = head; remaining = n; off = 0;
         cp = arena + (size_t)(chunk >= 0 ? chunk : 0) * PETAR_CHUNK;
         nxt = (chunk >= 0 && n > PETAR_CHUNK_PAYLOAD) ? cp[0] : -1;
+    }
+    __device__ __forceinline__ void init(const int* arena, int head1, int n1, int head2, int n2) {
+        if (n1 > 0) { head_b = head2; n_b = n2; start(arena, head1, n1); }
+        else { head_b = -1; n_b = 0; start(arena, head2, n2); }
     }
     __device__ __forceinline__ int count() const { return (chunk >= 0 && remaining > 0) ? min(SP_TILE, min(remaining, PETAR_CHUNK_PAYLOAD - off)) : 0; }
     __device__ __forceinline__ void advance(const int* arena, int n) {
@@ -149,6 +161,9 @@ struct TileCursor {
             chunk = nxt; off = 0;
             cp = arena + (size_t)(chunk >= 0 ? chunk : 0) * PETAR_CHUNK;
             nxt = (chunk >= 0 && remaining > PETAR_CHUNK_PAYLOAD) ? cp[0] : -1;
+        } else if (remaining <= 0 && n_b > 0) {
+            start(arena, head_b, n_b);
+            n_b = 0;
         }
     }
 };
@@ -156,10 +171,11 @@ struct TileCursor {
 // One super-particle list of the group (3-stage pipeline).  gh/gl: group centre (float-float, root-relative).
 template <bool QUAD, bool PRECISE>
 __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ arena, const NodeSp* __restrict__ nsp,
-                                         const int head, const int n, const int t, const int slice, const int S, const bool active,
+                                         const int head, const int n, const int head2, const int n2,
+                                         const int t, const int slice, const int S, const bool active,
                                          const float4 ia0, const float4 ib0, const float4 ia1, const float4 ib1,
                                          const float3 gh, const float3 gl, Acc64& acc0, Acc64& acc1) {
-    if (n <= 0) return;             // uniform
+    if (n + n2 <= 0) return;        // uniform
     // i-particles in the representation of this path
     float ix0, iy0, iz0, ix1, iy1, iz1;                 // PLAIN: group-relative; PRECISE: -hi
     float lx0 = 0.f, ly0 = 0.f, lz0 = 0.f, lx1 = 0.f, ly1 = 0.f, lz1 = 0.f;     // PRECISE: -lo
@@ -171,7 +187,7 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
         ix1 = (ia1.x - gh.x) + (ib1.x - gl.x); iy1 = (ia1.y - gh.y) + (ib1.y - gl.y); iz1 = (ia1.z - gh.z) + (ib1.z - gl.z);
     }
     Acc32 p0 = {0.f, 0.f, 0.f, 0.f}, p1 = {0.f, 0.f, 0.f, 0.f};
-    TileCursor cur; cur.init(arena, head, n);
+    TileCursor cur; cur.init(arena, head, n, head2, n2);
     int tn0 = 0, tn1 = 0, tn2 = 0;
     int id2[SP_REC];
     float4 q0[SP_REC], q1[SP_REC], q2[SP_REC];
@@ -218,7 +234,7 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
     while (tn0 > 0) {
         if (active) {
             const SpBuf& bf = sm.sp[cb];
-#pragma unroll 2
+            UNROLL_J
             for (int j = slice; j < tn0; j += S) {
                 const float4 a = bf.q0[j];
                 if (PRECISE) {
@@ -247,7 +263,7 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
 template <bool QUAD>
 __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
                                                  const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
-                                                 const unsigned* __restrict__ perm,
+                                                 const unsigned* __restrict__ perm, const SuperRec* __restrict__ srec,
                                                  double* __restrict__ oax, double* __restrict__ oay, double* __restrict__ oaz, double* __restrict__ opot,
                                                  ForceConst fc, double G) {
     __shared__ ForceSmem sm;
@@ -280,8 +296,10 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
         }
         Acc64 acc0 = {0, 0, 0, 0}, acc1 = {0, 0, 0, 0};
 
-        sp_phase<QUAD, false>(sm, arena, nsp, gr->head_sp, gr->n_sp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
-        sp_phase<QUAD, true>(sm, arena, nsp, gr->head_spp, gr->n_spp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
+        // cells common to the whole super-group (decided once by k_walk_super), then the group's own cells
+        const SuperRec* sr = &srec[gr->sid];
+        sp_phase<QUAD, false>(sm, arena, nsp, sr->head_sp, sr->n_sp, gr->head_sp, gr->n_sp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
+        sp_phase<QUAD, true>(sm, arena, nsp, sr->head_spp, sr->n_spp, gr->head_spp, gr->n_spp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
 
         // ---- particles: near ranges (changeover) then far ranges (plain Newtonian), float-float ----------
         {
@@ -392,9 +410,9 @@ cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, doub
     if (per_sm < 1) per_sm = 1;
     const int grid = t->sm_count * per_sm;
     if (t->p.multipole >= 2)
-        k_force<true><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, ax, ay, az, pot, fc, t->p.G);
+        k_force<true><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.srec, ax, ay, az, pot, fc, t->p.G);
     else
-        k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, ax, ay, az, pot, fc, t->p.G);
+        k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.srec, ax, ay, az, pot, fc, t->p.G);
     KCHECK(s, "k_force");
     petar_count_launch(2);
     stage_end(t, PETAR_STAGE_FORCE, s);

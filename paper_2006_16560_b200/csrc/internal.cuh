@@ -27,6 +27,8 @@ struct DevHeader {
     int group_ticket;   // dynamic scheduling counters (reset before each consumer kernel)
     int group_ticket2;
     int group_ticket3;
+    int n_super;
+    int super_ticket;
     int pad_;
     unsigned long long n_epep, n_epsp, n_epep_near, n_ep_list, n_sp_list;
     unsigned long long nb_total;
@@ -54,7 +56,22 @@ struct __align__(16) GroupRec {
     int n_ep_part, n_epn_part;         // particles in all EP ranges / in near ranges
     int head_spp, n_spp;               // cells closer than the group's own size: float-float ("precise") path
     double lo[3], hi[3], rmax;
-    double pad2;
+    int sid;                           // super-group (see SuperRec) this group lies in
+    int pad2;
+};
+
+// super-group: tree cell with <= PETAR_N_SUPER members (parent has more).  Its walk decides, once for all
+// the i-groups inside it, the cells that every one of them accepts ("common" lists) and leaves the rest
+// ("deferred" cells) to the per-group walks, which start from them instead of from the root.
+#ifndef PETAR_N_SUPER
+#define PETAR_N_SUPER 512
+#endif
+struct __align__(16) SuperRec {
+    int node, begin, end;
+    int head_sp, n_sp;                 // common cells, group-relative path
+    int head_spp, n_spp;               // common cells, float-float path
+    int head_def, n_def;               // deferred cells (node ids)
+    int pad[3];
 };
 
 struct Workspace {
@@ -78,6 +95,8 @@ struct Workspace {
     int node_cap;
     // groups
     GroupRec* grp; int group_cap;
+    SuperRec* srec;                // [group_cap] super-groups
+    int* smap;                     // [N] sorted position -> super-group id
     // list arena
     int* arena; int arena_chunks;
     // neighbour temporaries

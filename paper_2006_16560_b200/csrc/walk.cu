@@ -51,11 +51,55 @@ __device__ __forceinline__ void list_append(ListCursor& c, bool take, int per, i
     c.pos = n * per - space;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Super-groups.  A node is a super-group iff (count <= PETAR_N_SUPER or it is a leaf) and its parent
+// holds more than PETAR_N_SUPER particles (or it is the root).  Every i-group lies inside exactly one.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_super_collect(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
+                                                       const unsigned long long* __restrict__ key, long long n,
+                                                       SuperRec* __restrict__ srec, int node_cap) {
+    const int nn = h->n_nodes;
+    if (nn > node_cap) return;
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= nn) return;
+    const int4 d = nw[id].d;
+    const int level = d.w & 255;
+    const bool leaf = (d.w >> 16) & 1;
+    if (!(d.y - d.x <= PETAR_N_SUPER || leaf)) return;
+    if (level > 0) {
+        // parent's particle count: the range of keys that share the level-1 prefix of this cell
+        const int shift = 3 * (PETAR_MAXLEVEL - (level - 1));
+        const unsigned long long pref = (level - 1 > 0) ? (key[d.x] >> shift) : 0ull;
+        long long lo = 0, hi = d.x;                 // first index whose prefix equals pref
+        while (lo < hi) { long long mid = (lo + hi) >> 1; if (((level - 1 > 0) ? (key[mid] >> shift) : 0ull) < pref) lo = mid + 1; else hi = mid; }
+        const long long pb = lo;
+        lo = d.y; hi = n;                           // first index whose prefix exceeds pref
+        while (lo < hi) { long long mid = (lo + hi) >> 1; if (((level - 1 > 0) ? (key[mid] >> shift) : 0ull) <= pref) lo = mid + 1; else hi = mid; }
+        if (lo - pb <= PETAR_N_SUPER) return;       // an ancestor is the super-group
+    }
+    const int sid = atomicAdd(&h->n_super, 1);
+    SuperRec r;
+    r.node = id; r.begin = d.x; r.end = d.y;
+    r.head_sp = r.head_spp = r.head_def = -1; r.n_sp = r.n_spp = r.n_def = 0;
+    r.pad[0] = r.pad[1] = r.pad[2] = 0;
+    srec[sid] = r;
+}
+
+__global__ void __launch_bounds__(256) k_super_map(const DevHeader* __restrict__ h, const SuperRec* __restrict__ srec, int* __restrict__ smap) {
+    const int lane = threadIdx.x & 31;
+    const int ns = h->n_super;
+    for (int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; s < ns; s += (gridDim.x * blockDim.x) >> 5)
+        for (int p = srec[s].begin + lane; p < srec[s].end; p += 32) smap[p] = s;
+}
+
 // fp64 MAC of rule O7 (exactly this operation order); returns act: 0 SP, 1 EP near, 2 EP far, 3 open
-__device__ __forceinline__ int mac_exact(const NodeMac& c, const int level, const bool leaf,
-                                         const double glo0, const double glo1, const double glo2,
-                                         const double ghi0, const double ghi1, const double ghi2,
-                                         const double grmax, const double theta2, const double twoh) {
+__device__ __noinline__ int mac_exact(const NodeMac* __restrict__ cp, const int level, const bool leaf,
+                                      const GroupRec* __restrict__ gr, const double theta, const double twoh) {
+    const NodeMac c = *cp;
+    const double glo0 = gr->lo[0], glo1 = gr->lo[1], glo2 = gr->lo[2];
+    const double ghi0 = gr->hi[0], ghi1 = gr->hi[1], ghi2 = gr->hi[2];
+    const double grmax = gr->rmax;
+    const double theta2 = theta * theta;
     double gx = fmax(0.0, fmax(c.lo[0] - ghi0, glo0 - c.hi[0]));
     double gy = fmax(0.0, fmax(c.lo[1] - ghi1, glo1 - c.hi[1]));
     double gz = fmax(0.0, fmax(c.lo[2] - ghi2, glo2 - c.hi[2]));
@@ -80,9 +124,117 @@ __device__ __forceinline__ int mac_exact(const NodeMac& c, const int level, cons
 // 8 * 2^-24 (A_c + A_g) = eps_c + eps_g (component differences: 2(u_c+u_g) each; norm: 2 sqrt(3)(u_c+u_g);
 // rounding of the sum of squares: < 2.6 (u_c+u_g)); thresholds get a further relative 2^-22 for their own
 // rounding and the fp32 conversion of rmax and of the per-level edge/theta.
-#define WALK_RESERVE 160         // > 7 * 21: room for a pure depth-first descent from any state
-__global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
+#define WALK_RESERVE 160
+// Walk of one super-group S (one warp each).  All tests are fp32 with the error band described below
+// and only DEFINITE outcomes are used, so the result is sound for every i-group g inside S:
+//   accepted for S  (box(S) not within R of the cell, edge < theta * dist(box(S), com))  =>  accepted by every g,
+//        because box(g) is inside box(S): both distances can only grow and rmax_g <= rmax_S;
+//   edge >= theta * (largest distance from com to a corner of box(S))  =>  not "far" for any g  =>  opened by every g;
+//   anything else (and every leaf) is DEFERRED to the per-group walks.
+// Hence the cells a group accepts are exactly S's common cells plus what its own walk finds below the
+// deferred cells - the same set rule O7 gives when walked from the root.
+__global__ void __launch_bounds__(WALK_WARPS * 32) k_walk_super(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
+                                                                SuperRec* __restrict__ srec, int* __restrict__ arena, int arena_chunks,
+                                                                double theta, int node_cap) {
+    __shared__ int s_stack[WALK_WARPS][WALK_STACK];
+    __shared__ float s_lt[PETAR_NLEVELS];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int* stack = s_stack[w];
+    const int ns = h->n_super;
+    if (h->n_nodes > node_cap || h->n_nodes <= 0) return;
+    const double twoh = 2.0 * h->h;
+    if (threadIdx.x < PETAR_NLEVELS) s_lt[threadIdx.x] = (theta > 0.0) ? (float)(ldexp(twoh, -(int)threadIdx.x) / theta) : INFINITY;
+    __syncthreads();
+    for (;;) {
+        int s = 0;
+        if (lane == 0) s = atomicAdd(&h->super_ticket, 1);
+        s = __shfl_sync(0xffffffffu, s, 0);
+        if (s >= ns) break;
+        const NodeW sb = nw[srec[s].node];           // the super-group's own cell: tight box, rmax, eps
+        const float fl0 = sb.a.x, fl1 = sb.a.y, fl2 = sb.a.z, fh0 = sb.a.w, fh1 = sb.b.x, fh2 = sb.b.y;
+        const float frm = sb.c.y, geps = sb.c.z;
+        const float gedge = fmaxf(fh0 - fl0, fmaxf(fh1 - fl1, fh2 - fl2));
+        const float gedge2 = gedge * gedge;
+        ListCursor lsp = {-1, -1, 0, 0}, lspp = {-1, -1, 0, 0}, ldef = {-1, -1, 0, 0};
+        int n_sp = 0, n_spp = 0, n_def = 0;
+        int top = 1;
+        if (lane == 0) stack[0] = 0;
+        __syncwarp();
+        while (top > 0) {
+            int p = min(32, top);
+            if (top + 7 * p > WALK_STACK - WALK_RESERVE) p = max(1, min(p, (WALK_STACK - WALK_RESERVE - top) / 7));
+            const int node = (lane < p) ? stack[top - p + lane] : -1;
+            top -= p;
+            __syncwarp();
+            int act = -1;                      // 0 common (plain), 4 common (precise), 3 open, 5 deferred
+            int fc = 0, nch = 0;
+            if (node >= 0) {
+                const NodeW c = nw[node];
+                const int meta = c.d.w;
+                const int level = meta & 255;
+                const bool leaf = (meta >> 16) & 1;
+                fc = c.d.z; nch = (meta >> 8) & 15;
+                const float gx = fmaxf(0.f, fmaxf(c.a.x - fh0, fl0 - c.a.w));
+                const float gy = fmaxf(0.f, fmaxf(c.a.y - fh1, fl1 - c.b.x));
+                const float gz = fmaxf(0.f, fmaxf(c.a.z - fh2, fl2 - c.b.y));
+                const float d2b = fmaf(gz, gz, fmaf(gy, gy, gx * gx));
+                const float px = fmaxf(0.f, fmaxf(fl0 - c.b.z, c.b.z - fh0));
+                const float py = fmaxf(0.f, fmaxf(fl1 - c.b.w, c.b.w - fh1));
+                const float pz = fmaxf(0.f, fmaxf(fl2 - c.c.x, c.c.x - fh2));
+                const float d2c = fmaf(pz, pz, fmaf(py, py, px * px));
+                const float mx = fmaxf(fabsf(c.b.z - fl0), fabsf(fh0 - c.b.z));
+                const float my = fmaxf(fabsf(c.b.w - fl1), fabsf(fh1 - c.b.w));
+                const float mz = fmaxf(fabsf(c.c.x - fl2), fabsf(fh2 - c.c.x));
+                const float dmax2 = fmaf(mz, mz, fmaf(my, my, mx * mx));
+                const float D = geps + c.c.z;
+                const float R = fmaxf(frm, c.c.y);
+                const float Dr = fmaf(R, 2.4e-7f, D);
+                const float Rp = R + Dr;
+                const bool near_no = d2b > Rp * Rp;
+                const float L = s_lt[level];
+                const float Dl = fmaf(L, 2.4e-7f, D);
+                const float Lm = fmaxf(L - Dl, 0.f), Lp = L + Dl;
+                const bool far_yes = d2c > Lp * Lp;
+                const bool open_all = !leaf && (dmax2 < Lm * Lm);
+                if (near_no && far_yes) act = (d2b < gedge2) ? 4 : 0;
+                else if (open_all) act = 3;
+                else act = 5;
+            }
+            list_append(lsp, act == 0, 1, node, 0, arena, arena_chunks, h, lane);
+            list_append(lspp, act == 4, 1, node, 0, arena, arena_chunks, h, lane);
+            list_append(ldef, act == 5, 1, node, 0, arena, arena_chunks, h, lane);
+            n_sp += __popc(__ballot_sync(0xffffffffu, act == 0));
+            n_spp += __popc(__ballot_sync(0xffffffffu, act == 4));
+            n_def += __popc(__ballot_sync(0xffffffffu, act == 5));
+            const int push = (act == 3) ? nch : 0;
+            int pref = push;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int a = __shfl_up_sync(0xffffffffu, pref, o);
+                if (lane >= o) pref += a;
+            }
+            const int total_push = __shfl_sync(0xffffffffu, pref, 31);
+            if (top + total_push > WALK_STACK) { if (lane == 0) atomicOr(&h->status, PETAR_ST_STACK); top = 0; break; }
+            const int at = top + pref - push;
+            for (int k = 0; k < push; ++k) stack[at + k] = fc + k;
+            top += total_push;
+            __syncwarp();
+        }
+        if (lane == 0) {
+            SuperRec* so = &srec[s];
+            so->head_sp = lsp.head; so->n_sp = n_sp; so->head_spp = lspp.head; so->n_spp = n_spp;
+            so->head_def = ldef.head; so->n_def = n_def;
+        }
+    }
+}
+
+         // > 7 * 21: room for a pure depth-first descent from any state
+#ifndef WALK_MIN_CTAS
+#define WALK_MIN_CTAS 3
+#endif
+__global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
                                                           const NodeMac* __restrict__ nmac, GroupRec* __restrict__ grp,
+                                                          const SuperRec* __restrict__ srec, const int* __restrict__ smap,
                                                           int* __restrict__ arena, int arena_chunks, double theta, int node_cap) {
     __shared__ int s_stack[WALK_WARPS][WALK_STACK];
     __shared__ float s_lt[PETAR_NLEVELS];          // edge(level) / theta  (inf when theta == 0: nothing is ever "far")
@@ -90,7 +242,6 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
     int* stack = s_stack[w];
     const int ng = h->n_groups;
     if (h->n_nodes > node_cap || h->n_nodes <= 0) return;
-    const double theta2 = theta * theta;
     const double twoh = 2.0 * h->h;
     const double rcx = h->c[0], rcy = h->c[1], rcz = h->c[2];
     if (threadIdx.x < PETAR_NLEVELS) s_lt[threadIdx.x] = (theta > 0.0) ? (float)(ldexp(twoh, -(int)threadIdx.x) / theta) : INFINITY;
@@ -102,14 +253,11 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g >= ng) break;
         const GroupRec* gr = &grp[g];
-        const double glo0 = gr->lo[0], glo1 = gr->lo[1], glo2 = gr->lo[2];
-        const double ghi0 = gr->hi[0], ghi1 = gr->hi[1], ghi2 = gr->hi[2];
-        const double grmax = gr->rmax;
         const int n_i = gr->end - gr->begin;
         // fp32 copy of the group's box (relative to the root centre) and its error bound
-        const float fl0 = (float)(glo0 - rcx), fl1 = (float)(glo1 - rcy), fl2 = (float)(glo2 - rcz);
-        const float fh0 = (float)(ghi0 - rcx), fh1 = (float)(ghi1 - rcy), fh2 = (float)(ghi2 - rcz);
-        const float frm = (float)grmax;
+        const float fl0 = (float)(gr->lo[0] - rcx), fl1 = (float)(gr->lo[1] - rcy), fl2 = (float)(gr->lo[2] - rcz);
+        const float fh0 = (float)(gr->hi[0] - rcx), fh1 = (float)(gr->hi[1] - rcy), fh2 = (float)(gr->hi[2] - rcz);
+        const float frm = (float)gr->rmax;
         const float geps = 4.8e-7f * fmaxf(fmaxf(fmaxf(fabsf(fl0), fabsf(fh0)), fmaxf(fabsf(fl1), fabsf(fh1))), fmaxf(fabsf(fl2), fabsf(fh2)));
         ListCursor lsp = {-1, -1, 0, 0}, lspp = {-1, -1, 0, 0}, lepn = {-1, -1, 0, 0}, lepf = {-1, -1, 0, 0};
         int n_sp = 0, n_spp = 0, n_epn = 0, n_epf = 0, n_ep_part = 0, n_epn_part = 0;
@@ -117,10 +265,20 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
         // kernel evaluates them with float-float coordinates, all others with group-relative floats
         const float gedge = fmaxf(fh0 - fl0, fmaxf(fh1 - fl1, fh2 - fl2));
         const float gedge2 = gedge * gedge;
-        int top = 1;
-        if (lane == 0) stack[0] = 0;
-        __syncwarp();
-        while (top > 0) {
+        // the walk starts from the cells the super-group's walk deferred (k_walk_super), fed in batches
+        const int sid = smap[gr->begin];
+        const SuperRec* sr = &srec[sid];
+        int dchunk = sr->head_def, dremaining = sr->n_def, doff = 0;
+        int top = 0;
+        while (top > 0 || dremaining > 0) {
+            if (top == 0) {                    // frontier empty: take the next (up to 256) deferred cells
+                const int* cp = arena + (size_t)dchunk * PETAR_CHUNK;
+                const int k = min(256, min(dremaining, PETAR_CHUNK_PAYLOAD - doff));
+                for (int e = lane; e < k; e += 32) stack[e] = cp[PETAR_CHUNK_HDR + doff + e];
+                top = k; dremaining -= k; doff += k;
+                if (dremaining > 0 && doff >= PETAR_CHUNK_PAYLOAD) { dchunk = cp[0]; doff = 0; }
+                __syncwarp();
+            }
             // pop up to 32 nodes; throttle towards depth-first order when the frontier nears its capacity
             // (a pure depth-first descent adds at most 7 entries per level, < WALK_RESERVE in total)
             int p = min(32, top);
@@ -158,7 +316,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
                 else if (!leaf && (near_yes || far_no)) act = 3;
                 else if (leaf && near_yes) act = 1;
                 else if (leaf && near_no && far_no) act = 2;
-                else act = mac_exact(nmac[node], level, leaf, glo0, glo1, glo2, ghi0, ghi1, ghi2, grmax, theta2, twoh);
+                else act = mac_exact(&nmac[node], level, leaf, gr, theta, twoh);
                 if (act == 0 && d2b < gedge2) act = 4;
             }
             // outputs
@@ -197,12 +355,14 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
             go->n_sp = n_sp; go->n_epn = n_epn; go->n_epf = n_epf;
             go->head_spp = lspp.head; go->n_spp = n_spp;
             go->n_ep_part = n_ep_part; go->n_epn_part = n_epn_part;
+            go->sid = sid;
         }
+        const int n_common = sr->n_sp + sr->n_spp;
         t_epep += (unsigned long long)n_i * (unsigned long long)n_ep_part;
         t_near += (unsigned long long)n_i * (unsigned long long)n_epn_part;
-        t_epsp += (unsigned long long)n_i * (unsigned long long)(n_sp + n_spp);
+        t_epsp += (unsigned long long)n_i * (unsigned long long)(n_sp + n_spp + n_common);
         t_eplist += (unsigned long long)(n_epn + n_epf);
-        t_splist += (unsigned long long)(n_sp + n_spp);
+        t_splist += (unsigned long long)(n_sp + n_spp + n_common);
     }
     if (lane == 0) {
         atomicAdd(&h->n_epep, t_epep); atomicAdd(&h->n_epsp, t_epsp); atomicAdd(&h->n_epep_near, t_near);
@@ -211,7 +371,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk(DevHeader* __restrict_
 }
 
 __global__ void k_reset_ticket(DevHeader* h, int which) {
-    if (threadIdx.x == 0) { if (which == 0) { h->group_ticket = 0; h->arena_top = 0; h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = 0ull; } else h->group_ticket3 = 0; }
+    if (threadIdx.x == 0) { if (which == 0) { h->group_ticket = 0; h->arena_top = 0; h->n_super = 0; h->super_ticket = 0; h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = 0ull; } else h->group_ticket3 = 0; }
 }
 
 cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
@@ -223,9 +383,15 @@ cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_walk, WALK_WARPS * 32, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
-    k_walk<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, w.nmac, w.grp, w.arena, w.arena_chunks, t->p.theta, w.node_cap);
+    k_super_collect<<<cdiv(w.node_cap, 256), 256, 0, s>>>(w.hdr, w.nw, w.key, t->N, w.srec, w.node_cap);
+    KCHECK(s, "k_super_collect");
+    k_super_map<<<t->sm_count * 8, 256, 0, s>>>(w.hdr, w.srec, w.smap);
+    KCHECK(s, "k_super_map");
+    k_walk_super<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, w.srec, w.arena, w.arena_chunks, t->p.theta, w.node_cap);
+    KCHECK(s, "k_walk_super");
+    k_walk<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, w.nmac, w.grp, w.srec, w.smap, w.arena, w.arena_chunks, t->p.theta, w.node_cap);
     KCHECK(s, "k_walk");
-    petar_count_launch(2);
+    petar_count_launch(5);
     stage_end(t, PETAR_STAGE_WALK, s);
     return cudaGetLastError();
 }
@@ -324,12 +490,12 @@ cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, 
 // ------------------------------------------------------------------------------------------------
 // list export (tests): flatten the chunk chains.
 // ------------------------------------------------------------------------------------------------
-__global__ void k_list_sizes(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, int* __restrict__ sizes) {
+__global__ void k_list_sizes(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const SuperRec* __restrict__ srec, int* __restrict__ sizes) {
     int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= h->n_groups) return;
-    sizes[3 * g] = grp[g].n_sp + grp[g].n_spp; sizes[3 * g + 1] = 2 * grp[g].n_epn; sizes[3 * g + 2] = 2 * grp[g].n_epf;
+    sizes[3 * g] = grp[g].n_sp + grp[g].n_spp + srec[grp[g].sid].n_sp + srec[grp[g].sid].n_spp; sizes[3 * g + 1] = 2 * grp[g].n_epn; sizes[3 * g + 2] = 2 * grp[g].n_epf;
 }
-__global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
+__global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const SuperRec* __restrict__ srec, const int* __restrict__ arena,
                                const long long* __restrict__ offs, int* __restrict__ out, long long out_entries) {
     const int lane = threadIdx.x & 31;
     long long wid = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -338,7 +504,7 @@ __global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* 
     int chunk = which == 0 ? grp[g].head_sp : which == 1 ? grp[g].head_epn : grp[g].head_epf;
     int remaining = which == 0 ? grp[g].n_sp : which == 1 ? 2 * grp[g].n_epn : 2 * grp[g].n_epf;
     long long o = offs[wid];
-    for (int part = 0; part < 2; ++part) {
+    for (int part = 0; part < 4; ++part) {
         while (chunk >= 0 && remaining > 0) {
             const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
             int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
@@ -346,13 +512,17 @@ __global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* 
             o += ne; remaining -= ne; chunk = cp[0];
         }
         if (which != 0) break;
-        chunk = grp[g].head_spp; remaining = grp[g].n_spp;       // "SP" = plain cells, then precise cells
+        // "SP" = own plain cells, own precise cells, then the super-group's common cells (plain, precise)
+        const SuperRec* sr = &srec[grp[g].sid];
+        if (part == 0) { chunk = grp[g].head_spp; remaining = grp[g].n_spp; }
+        else if (part == 1) { chunk = sr->head_sp; remaining = sr->n_sp; }
+        else if (part == 2) { chunk = sr->head_spp; remaining = sr->n_spp; }
     }
 }
-__global__ void k_group_cnt(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, int* __restrict__ out, int what) {
+__global__ void k_group_cnt(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const SuperRec* __restrict__ srec, int* __restrict__ out, int what, int walked) {
     int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= h->n_groups) return;
-    if (what == PETAR_DBG_GROUP_CNT) { out[4 * g] = grp[g].n_sp + grp[g].n_spp; out[4 * g + 1] = grp[g].n_epn; out[4 * g + 2] = grp[g].n_epf; out[4 * g + 3] = grp[g].n_ep_part; }
+    if (what == PETAR_DBG_GROUP_CNT) { out[4 * g] = grp[g].n_sp + grp[g].n_spp + (walked ? srec[grp[g].sid].n_sp + srec[grp[g].sid].n_spp : 0); out[4 * g + 1] = grp[g].n_epn; out[4 * g + 2] = grp[g].n_epf; out[4 * g + 3] = grp[g].n_ep_part; }
     else { out[2 * g] = grp[g].begin; out[2 * g + 1] = grp[g].end; }
 }
 __global__ void k_group_dbl(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, double* __restrict__ out) {
@@ -378,7 +548,7 @@ cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_b
     if (what == PETAR_DBG_GROUP_CNT || what == PETAR_DBG_GROUP_INT) {
         size_t need = (size_t)ng * (what == PETAR_DBG_GROUP_CNT ? 16 : 8);
         if (dst_bytes < need) return cudaErrorInvalidValue;
-        if (ng) k_group_cnt<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, (int*)dst, what);
+        if (ng) k_group_cnt<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, (int*)dst, what, t->walked ? 1 : 0);
         KCHECK(s, "k_group_cnt");
     } else if (what == PETAR_DBG_GROUP_DBL) {
         if (dst_bytes < (size_t)ng * 56) return cudaErrorInvalidValue;
@@ -393,7 +563,7 @@ cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_b
         if (!ng) return cudaSuccess;
         int* sizes = w.exp_scratch;                                       // 3 ng ints
         long long* offs = (long long*)(w.exp_scratch + 4ll * (ng + 1));   // 3 ng + 1 int64 (16-byte aligned)
-        k_list_sizes<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, sizes);
+        k_list_sizes<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, sizes);
         KCHECK(s, "k_list_sizes");
         cudaError_t e = launch_scan_i32_to_i64(sizes, offs, 3ll * ng, (long long*)w.scan_tmp, s);
         if (e != cudaSuccess) return e;
@@ -401,7 +571,7 @@ cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_b
             if (dst_bytes < (size_t)(3ll * ng + 1) * 8) return cudaErrorInvalidValue;
             return cudaMemcpyAsync(dst, offs, (size_t)(3ll * ng + 1) * 8, cudaMemcpyDeviceToDevice, s);
         }
-        k_list_flatten<<<cdiv(3ll * ng * 32, 256), 256, 0, s>>>(w.hdr, w.grp, w.arena, offs, (int*)dst, (long long)(dst_bytes / 4));
+        k_list_flatten<<<cdiv(3ll * ng * 32, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, w.arena, offs, (int*)dst, (long long)(dst_bytes / 4));
         KCHECK(s, "k_list_flatten");
     }
     return cudaGetLastError();

@@ -328,6 +328,48 @@ def test_full_size(cfg):
     t.close()
 
 
+def test_config5_capacity():
+    """Config 5 (N = 10,485,760, everything resident in HBM): structures bit-exact over the whole system;
+    lists, counts, forces and neighbour rows on sampled i-groups the oracle can compute one by one."""
+    w = make_workload(5)
+    t, T = _gpu_tree(w), _ora_tree(w)
+    check_structures(t, T, w)
+    counts = t.force(want_counts=True)
+    assert _P().petar_tree_status(t.handle) == 0
+    rng = np.random.default_rng(5)
+    sel = np.sort(rng.choice(T.n_groups, size=60, replace=False))
+    gc = _np(t.export("GROUP_CNT")).reshape(-1, 4)
+    offs, lists = t.export("LISTS")
+    offs, lists = _np(offs), _np(lists)
+    for g in sel[:20]:
+        sp, ep = T.walk_lists(int(g))
+        assert gc[g, 0] == len(sp) and gc[g, 1] + gc[g, 2] == len(ep) and gc[g, 3] == int((ep[:, 1] - ep[:, 0]).sum())
+        assert np.array_equal(np.sort(lists[offs[3 * g]:offs[3 * g + 1]]), np.sort(sp))
+        gn = lists[offs[3 * g + 1]:offs[3 * g + 2]].reshape(-1, 2)
+        near = ep[ep[:, 2] == 1][:, :2]
+        assert np.array_equal(gn[np.argsort(gn[:, 0])], near[np.argsort(near[:, 0])])
+    a = T.force(sel)
+    g4 = [_np(v) for v in (t.acc_x, t.acc_y, t.acc_z, t.pot)]
+    ea, ep_ = _rel_err(g4, a)
+    assert ea.size > 500 and ea.max() < TOL and ep_.max() < TOL, (ea.max(), ep_.max())
+    off, idx = t.neighbors()
+    off, idx = _np(off), _np(idx)
+    ooff, oidx = T.neighbors(sel)
+    key, perm = T.keys()
+    gb, ge, *_ = T.groups()
+    n_checked = 0
+    for g in sel:
+        for o in perm[gb[g]:ge[g]]:
+            row = np.sort(idx[off[o]:off[o + 1]])
+            assert np.array_equal(row, oidx[ooff[o]:ooff[o + 1]])
+            n_checked += len(row)
+    assert n_checked > 50
+    # properties that hold at any size
+    assert all(np.all(np.isfinite(v)) for v in g4) and np.all(g4[3] < 0)
+    assert counts.n_epep + counts.n_epsp > 5e10
+    t.close()
+
+
 def test_rms_error_vs_direct_sum_config4():
     """Reported separately (north_star): RMS relative force error against the DEFINITION (direct long-range sum
     over all N sources) on a 4096-target subsample, theta sweep of config 4.  PARITY UNPINNED: the paper prints
