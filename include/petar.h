@@ -139,6 +139,8 @@ const char* petar_strerror(int code);
  *   PETAR_DBG_GROUP_INT int32[ng*2]: begin, end
  *   PETAR_DBG_GROUP_DBL double[ng*7]: lo[3], hi[3], rmax
  *   PETAR_DBG_GROUP_CNT int32[ng*4]: n_sp, n_ep ranges (near), n_ep ranges (far), n_ep particles
+ *   PETAR_DBG_GROUP_SUPER int32[ng*4]: super-group id, its particle count, cells its walk accepted
+ *                        for all of its groups ("common" cells, part of n_sp above), cells it deferred
  *   PETAR_DBG_LIST_OFFS int64[ng*3+1]: start of each group's SP / near-EP / far-EP block in the
  *                        flattened list below, in 4-byte entries; last = total
  *   PETAR_DBG_LISTS    int32[total]: SP node ids; EP ranges as (begin, end) pairs
@@ -154,6 +156,7 @@ const char* petar_strerror(int code);
 #define PETAR_DBG_GROUP_CNT 8
 #define PETAR_DBG_LIST_OFFS 9
 #define PETAR_DBG_LISTS 10
+#define PETAR_DBG_GROUP_SUPER 11
 int petar_debug_export(petar_tree* t, int what, void* dst, size_t dst_bytes, void* cuda_stream);
 
 /* Per-stage device times of the last build / force / neighbour call on this tree, in ms, measured

@@ -15,7 +15,7 @@ EXPORTS = [
 ]
 STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor"]
 DBG = dict(HEADER=0, ROOT=1, KEYS=2, PERM=3, NODE_INT=4, NODE_DBL=5, GROUP_INT=6, GROUP_DBL=7, GROUP_CNT=8,
-           LIST_OFFS=9, LISTS=10)
+           LIST_OFFS=9, LISTS=10, GROUP_SUPER=11)
 
 
 class PetarError(RuntimeError):
@@ -242,7 +242,7 @@ class Tree:
         n = self.N
         spec = dict(ROOT=(4, t.float64), KEYS=(n, t.int64), PERM=(n, t.int32), NODE_INT=(nn * 4, t.int32),
                     NODE_DBL=(nn * 17, t.float64), GROUP_INT=(ng * 2, t.int32), GROUP_DBL=(ng * 7, t.float64),
-                    GROUP_CNT=(ng * 4, t.int32), LIST_OFFS=(ng * 3 + 1, t.int64))
+                    GROUP_CNT=(ng * 4, t.int32), GROUP_SUPER=(ng * 4, t.int32), LIST_OFFS=(ng * 3 + 1, t.int64))
         if name == "LISTS":
             offs = self.export("LIST_OFFS")
             total = int(offs[-1])

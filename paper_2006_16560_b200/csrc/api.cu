@@ -259,9 +259,9 @@ extern "C" int petar_debug_export(petar_tree* t, int what, void* dst, size_t dst
         case PETAR_DBG_KEYS: rc = copy(w.key, n * 8); break;
         case PETAR_DBG_PERM: rc = copy(w.idx, n * 4); break;
         case PETAR_DBG_NODE_INT: rc = copy(w.nint, (size_t)hh.n_nodes * sizeof(NodeInt)); break;
-        case PETAR_DBG_NODE_DBL: case PETAR_DBG_GROUP_INT: case PETAR_DBG_GROUP_DBL: case PETAR_DBG_GROUP_CNT:
+        case PETAR_DBG_NODE_DBL: case PETAR_DBG_GROUP_INT: case PETAR_DBG_GROUP_DBL: case PETAR_DBG_GROUP_CNT: case PETAR_DBG_GROUP_SUPER:
         case PETAR_DBG_LIST_OFFS: case PETAR_DBG_LISTS: {
-            if ((what == PETAR_DBG_GROUP_CNT || what == PETAR_DBG_LIST_OFFS || what == PETAR_DBG_LISTS) && !t->walked) return PETAR_ENOTBUILT;
+            if ((what == PETAR_DBG_GROUP_CNT || what == PETAR_DBG_GROUP_SUPER || what == PETAR_DBG_LIST_OFFS || what == PETAR_DBG_LISTS) && !t->walked) return PETAR_ENOTBUILT;
             cudaError_t e = launch_export_lists(t, what, dst, dst_bytes, s);
             if (e == cudaErrorInvalidValue) return PETAR_EINVAL;
             CK(e);

@@ -523,6 +523,7 @@ __global__ void k_group_cnt(const DevHeader* __restrict__ h, const GroupRec* __r
     int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= h->n_groups) return;
     if (what == PETAR_DBG_GROUP_CNT) { out[4 * g] = grp[g].n_sp + grp[g].n_spp + (walked ? srec[grp[g].sid].n_sp + srec[grp[g].sid].n_spp : 0); out[4 * g + 1] = grp[g].n_epn; out[4 * g + 2] = grp[g].n_epf; out[4 * g + 3] = grp[g].n_ep_part; }
+    else if (what == PETAR_DBG_GROUP_SUPER) { const SuperRec* sr = &srec[grp[g].sid]; out[4 * g] = grp[g].sid; out[4 * g + 1] = sr->end - sr->begin; out[4 * g + 2] = sr->n_sp + sr->n_spp; out[4 * g + 3] = sr->n_def; }
     else { out[2 * g] = grp[g].begin; out[2 * g + 1] = grp[g].end; }
 }
 __global__ void k_group_dbl(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, double* __restrict__ out) {
@@ -545,8 +546,8 @@ __global__ void k_node_dbl(const DevHeader* __restrict__ h, const NodeMac* __res
 cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_bytes, cudaStream_t s) {
     Workspace& w = t->w;
     int ng = t->pinned[1], nn = t->pinned[0];
-    if (what == PETAR_DBG_GROUP_CNT || what == PETAR_DBG_GROUP_INT) {
-        size_t need = (size_t)ng * (what == PETAR_DBG_GROUP_CNT ? 16 : 8);
+    if (what == PETAR_DBG_GROUP_CNT || what == PETAR_DBG_GROUP_INT || what == PETAR_DBG_GROUP_SUPER) {
+        size_t need = (size_t)ng * (what == PETAR_DBG_GROUP_INT ? 8 : 16);
         if (dst_bytes < need) return cudaErrorInvalidValue;
         if (ng) k_group_cnt<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, (int*)dst, what, t->walked ? 1 : 0);
         KCHECK(s, "k_group_cnt");
