@@ -139,8 +139,9 @@ const char* petar_strerror(int code);
  *   PETAR_DBG_GROUP_INT int32[ng*2]: begin, end
  *   PETAR_DBG_GROUP_DBL double[ng*7]: lo[3], hi[3], rmax
  *   PETAR_DBG_GROUP_CNT int32[ng*4]: n_sp, n_ep ranges (near), n_ep ranges (far), n_ep particles
- *   PETAR_DBG_GROUP_SUPER int32[ng*4]: super-group id, its particle count, cells its walk accepted
- *                        for all of its groups ("common" cells, part of n_sp above), cells it deferred
+ *   PETAR_DBG_GROUP_SUPER int32[ng*8]: for each of the two super-group levels: super-group id, its
+ *                        particle count, cells its walk accepted for all of its groups ("common"
+ *                        cells, part of n_sp above), cells it deferred
  *   PETAR_DBG_LIST_OFFS int64[ng*3+1]: start of each group's SP / near-EP / far-EP block in the
  *                        flattened list below, in 4-byte entries; last = total
  *   PETAR_DBG_LISTS    int32[total]: SP node ids; EP ranges as (begin, end) pairs

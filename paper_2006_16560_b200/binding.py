@@ -242,7 +242,7 @@ class Tree:
         n = self.N
         spec = dict(ROOT=(4, t.float64), KEYS=(n, t.int64), PERM=(n, t.int32), NODE_INT=(nn * 4, t.int32),
                     NODE_DBL=(nn * 17, t.float64), GROUP_INT=(ng * 2, t.int32), GROUP_DBL=(ng * 7, t.float64),
-                    GROUP_CNT=(ng * 4, t.int32), GROUP_SUPER=(ng * 4, t.int32), LIST_OFFS=(ng * 3 + 1, t.int64))
+                    GROUP_CNT=(ng * 4, t.int32), GROUP_SUPER=(ng * 8, t.int32), LIST_OFFS=(ng * 3 + 1, t.int64))
         if name == "LISTS":
             offs = self.export("LIST_OFFS")
             total = int(offs[-1])

@@ -44,7 +44,7 @@ __global__ void k_reset_header(DevHeader* h) {
     if (threadIdx.x == 0) {
         for (int k = 0; k < 3; ++k) { h->bbox[k] = ~0ull; h->bbox[3 + k] = 0ull; }
         h->n_nodes = 0; h->n_groups = 0; h->status = 0; h->arena_top = 0;
-        h->group_ticket = 0; h->group_ticket2 = 0; h->group_ticket3 = 0; h->n_super = 0; h->super_ticket = 0;
+        h->group_ticket = 0; h->group_ticket2 = 0; h->group_ticket3 = 0; for (int l = 0; l < PETAR_NSUP; ++l) { h->n_super[l] = 0; h->super_ticket[l] = 0; }
         h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = 0ull; h->nb_total = 0ull;
         for (int l = 0; l < PETAR_NLEVELS + 2; ++l) h->level_off[l] = 0;
     }
@@ -573,7 +573,7 @@ __global__ void __launch_bounds__(256) k_groups_finish(GroupRec* __restrict__ gr
             r->end = e; r->head_sp = r->head_epn = r->head_epf = -1;
             r->n_sp = r->n_epn = r->n_epf = 0; r->n_ep_part = r->n_epn_part = 0; r->head_spp = -1; r->n_spp = 0;
             for (int k = 0; k < 3; ++k) { r->lo[k] = lo[k]; r->hi[k] = hi[k]; }
-            r->rmax = rmax; r->sid = 0; r->pad2 = 0;
+            r->rmax = rmax; r->sid[0] = 0; r->sid[1] = 0;
         }
     }
 }

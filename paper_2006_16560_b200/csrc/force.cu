@@ -142,7 +142,8 @@ union __align__(16) ForceSmem {
 
 // uniform cursor over the tiles (<= SP_TILE entries, never straddling a chunk) of TWO chunked lists in a
 // row (the super-group's common cells, then the group's own cells)
-struct TileCursor {
+template <int TILE>
+struct TileCursorT {
     const int* cp; int chunk, nxt, off, remaining;
     int head_b, n_b;
     __device__ __forceinline__ void start(const int* arena, int head, int n) {
@@ -154,7 +155,7 @@ struct TileCursor {
         if (n1 > 0) { head_b = head2; n_b = n2; start(arena, head1, n1); }
         else { head_b = -1; n_b = 0; start(arena, head2, n2); }
     }
-    __device__ __forceinline__ int count() const { return (chunk >= 0 && remaining > 0) ? min(SP_TILE, min(remaining, PETAR_CHUNK_PAYLOAD - off)) : 0; }
+    __device__ __forceinline__ int count() const { return (chunk >= 0 && remaining > 0) ? min(TILE, min(remaining, PETAR_CHUNK_PAYLOAD - off)) : 0; }
     __device__ __forceinline__ void advance(const int* arena, int n) {
         remaining -= n; off += n;
         if (remaining > 0 && off >= PETAR_CHUNK_PAYLOAD) {
@@ -167,6 +168,8 @@ struct TileCursor {
         }
     }
 };
+
+typedef TileCursorT<SP_TILE> TileCursor;
 
 // One super-particle list of the group (3-stage pipeline).  gh/gl: group centre (float-float, root-relative).
 template <bool QUAD, bool PRECISE>
@@ -263,7 +266,7 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
 template <bool QUAD>
 __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
                                                  const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
-                                                 const unsigned* __restrict__ perm, const SuperRec* __restrict__ srec,
+                                                 const unsigned* __restrict__ perm, const double* __restrict__ part, const long long n_part,
                                                  double* __restrict__ oax, double* __restrict__ oay, double* __restrict__ oaz, double* __restrict__ opot,
                                                  ForceConst fc, double G) {
     __shared__ ForceSmem sm;
@@ -296,10 +299,9 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
         }
         Acc64 acc0 = {0, 0, 0, 0}, acc1 = {0, 0, 0, 0};
 
-        // cells common to the whole super-group (decided once by k_walk_super), then the group's own cells
-        const SuperRec* sr = &srec[gr->sid];
-        sp_phase<QUAD, false>(sm, arena, nsp, sr->head_sp, sr->n_sp, gr->head_sp, gr->n_sp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
-        sp_phase<QUAD, true>(sm, arena, nsp, sr->head_spp, sr->n_spp, gr->head_spp, gr->n_spp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
+        // the group's own cells (the cells common to its super-groups were summed by k_force_units into `part`)
+        sp_phase<QUAD, false>(sm, arena, nsp, -1, 0, gr->head_sp, gr->n_sp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
+        sp_phase<QUAD, true>(sm, arena, nsp, -1, 0, gr->head_spp, gr->n_spp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
 
         // ---- particles: near ranges (changeover) then far ranges (plain Newtonian), float-float ----------
         {
@@ -373,6 +375,8 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
         for (int k = t; k < n_i * 4; k += FT) {
             const int i = k >> 2, comp = k & 3;
             double s = 0.0;
+#pragma unroll
+            for (int l = 0; l < PETAR_NSUP; ++l) s += part[((size_t)l * n_part + gb + i) * 4 + comp];
             for (int sl = 0; sl < S; ++sl) s += sm.red[(size_t)(sl * (2 * P) + i) * 4 + comp];
             const unsigned o = perm[gb + i];
             if (comp == 3) { if (opot) opot[o] = -G * s; }
@@ -384,7 +388,254 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
     }
 }
 
-__global__ void k_reset_ticket2(DevHeader* h) { if (threadIdx.x == 0) h->group_ticket2 = 0; }
+
+// ------------------------------------------------------------------------------------------------
+// Phase A: the cells COMMON to a super-group (accepted once for all of its i-groups by k_walk_super)
+// against all of its particles.  The super-group's particles are cut into units of 128, 64, 32 and
+// < 32 particles; one CTA of four warps per unit.  Every warp holds ALL of the unit's particles, four per
+// lane (slot = lane % P, P = ceil(cnt/4)); the remaining factor S = 32 / P splits a staged tile into
+// interleaved slices, so units of 128 / 64 / 32 particles keep all 32 lanes busy.  The warps share out
+// the list tile by tile (warp w takes tiles w, w + 4, ...) and run without CTA barriers: each stages its
+// own tiles (ids two tiles ahead, records one tile ahead in registers, double-buffered shared memory);
+// the four partial sums meet once per unit.
+// Each (level, particle) is written exactly once into part[level][sorted position][ax, ay, az, pot]
+// (unscaled by G), in a fixed summation order; k_force adds these to the group's own sums.
+// ------------------------------------------------------------------------------------------------
+#define UW 4                   // warps per CTA
+#ifndef UNITS_MIN_CTAS
+#define UNITS_MIN_CTAS 3
+#endif
+#ifndef NI
+#define NI 4                   // i-particles per lane
+#endif
+#define UNIT_MAX (32 * NI)     // particles per unit
+#ifndef UT
+#define UT 32                  // cells per staged warp tile
+#endif
+#define UREC (UT / 32)
+struct UBuf { float4 q0[UT], q1[UT], q2[UT]; float q3[UT]; };          // 3328 B
+
+// Cursor of ONE warp over its share of a chunked list: the list is cut into tiles of UT entries (never
+// straddling a chunk) and warp w of the CTA takes every UW-th tile.
+struct WarpTileCursor {
+    const int* arena; const int* cp; int chunk, ne, t, remaining;
+    __device__ __forceinline__ void start(const int* arena_, int head, int n, int w) {
+        arena = arena_; chunk = (n > 0) ? head : -1; remaining = n; ne = min(n, PETAR_CHUNK_PAYLOAD); t = w;
+        cp = arena + (size_t)(chunk >= 0 ? chunk : 0) * PETAR_CHUNK;
+    }
+    // entries of this warp's next tile (0 = list exhausted); ids receives their address
+    __device__ __forceinline__ int next(const int*& ids) {
+        while (chunk >= 0 && remaining > 0) {
+            if (t * UT < ne) { ids = cp + PETAR_CHUNK_HDR + t * UT; const int c = min(UT, ne - t * UT); t += UW; return c; }
+            t -= (ne + UT - 1) / UT;
+            remaining -= ne;
+            chunk = (remaining > 0) ? cp[0] : -1;
+            if (chunk >= 0) { cp = arena + (size_t)chunk * PETAR_CHUNK; ne = min(remaining, PETAR_CHUNK_PAYLOAD); }
+        }
+        return 0;
+    }
+};
+
+// fp64 accumulators of phase A live in shared memory (s_acc[component][thread], conflict-free): 16 per lane
+__device__ __forceinline__ void flush_smem(Acc32& p, double* __restrict__ a) {
+    a[0] += (double)p.ax; a[UW * 32] += (double)p.ay; a[2 * UW * 32] += (double)p.az; a[3 * UW * 32] += (double)p.pot;
+    p.ax = p.ay = p.az = p.pot = 0.0f;
+}
+
+template <bool QUAD, bool PRECISE>
+__device__ __forceinline__ void unit_phase(UBuf* __restrict__ bufs, const int* __restrict__ arena, const NodeSp* __restrict__ nsp,
+                                           const int head, const int n, const int w, const int lane, const int slice, const int S, const bool active,
+                                           const float4* __restrict__ pa, const float4* __restrict__ pb, const int i0, const int ilast,
+                                           const float3 gh, double* __restrict__ sacc) {
+    if (n <= 0) return;             // warp-uniform
+    float ix[NI], iy[NI], iz[NI], lx[NI], ly[NI], lz[NI];
+    float4 ia[NI], ib[NI];
+#pragma unroll
+    for (int k = 0; k < NI; ++k) { const int i = min(i0 + k, ilast); ia[k] = pa[i]; ib[k] = pb[i]; }
+#pragma unroll
+    for (int k = 0; k < NI; ++k) {
+        if (PRECISE) { ix[k] = -ia[k].x; iy[k] = -ia[k].y; iz[k] = -ia[k].z; lx[k] = -ib[k].x; ly[k] = -ib[k].y; lz[k] = -ib[k].z; }
+        else { ix[k] = (ia[k].x - gh.x) + ib[k].x; iy[k] = (ia[k].y - gh.y) + ib[k].y; iz[k] = (ia[k].z - gh.z) + ib[k].z; lx[k] = ly[k] = lz[k] = 0.f; }
+    }
+    Acc32 p[NI];
+#pragma unroll
+    for (int k = 0; k < NI; ++k) p[k].ax = p[k].ay = p[k].az = p[k].pot = 0.f;
+    WarpTileCursor cur; cur.start(arena, head, n, w);
+    int tn0 = 0, tn1 = 0, tn2 = 0;
+    int id2[UREC];
+    float4 q0[UREC], q1[UREC], q2[UREC];
+#pragma unroll
+    for (int r = 0; r < UREC; ++r) id2[r] = 0;
+    auto load_ids = [&]() {
+        const int* ids = nullptr;
+        tn2 = cur.next(ids);
+#pragma unroll
+        for (int r = 0; r < UREC; ++r) if (lane + r * 32 < tn2) id2[r] = ids[lane + r * 32];
+    };
+    auto load_recs = [&]() {
+        tn1 = tn2;
+#pragma unroll
+        for (int r = 0; r < UREC; ++r) if (lane + r * 32 < tn1) { const NodeSp* sp = &nsp[id2[r]]; q0[r] = sp->q0; q1[r] = sp->q1; if (QUAD) q2[r] = sp->q2; }
+    };
+    auto store_recs = [&](UBuf& bf) {
+#pragma unroll
+        for (int r = 0; r < UREC; ++r) {
+            const int k = lane + r * 32;
+            if (k < tn1) {
+                const float bzz = -(q1[r].w + q2[r].x);
+                if (PRECISE) {
+                    bf.q0[k] = q0[r];
+                    bf.q1[k] = q1[r];
+                    if (QUAD) { bf.q2[k] = make_float4(q2[r].x, bzz, q2[r].y, q2[r].z); bf.q3[k] = q2[r].w; }
+                } else {
+                    bf.q0[k] = make_float4((q0[r].x - gh.x) + q1[r].x, (q0[r].y - gh.y) + q1[r].y, (q0[r].z - gh.z) + q1[r].z, q0[r].w);
+                    if (QUAD) { bf.q1[k] = make_float4(q1[r].w, q2[r].x, bzz, q2[r].y); bf.q2[k] = make_float4(q2[r].z, q2[r].w, 0.f, 0.f); }
+                }
+            }
+        }
+    };
+    const int fl_every = max(1, S >> 1);     // flush the fp32 partial sums after ~32-64 terms
+    int fl = 0;
+    __syncwarp();               // this warp's buffers are free (previous phase consumed)
+    load_ids();
+    load_recs();
+    load_ids();
+    store_recs(bufs[0]); tn0 = tn1;
+    load_recs();
+    load_ids();
+    __syncwarp();
+    int cb = 0;
+    while (tn0 > 0) {
+        if (active) {
+            const UBuf& bf = bufs[cb];
+#pragma unroll 1
+            for (int j = slice; j < tn0; j += S) {
+                const float4 a = bf.q0[j];
+                if (PRECISE) {
+                    const float4 b = bf.q1[j];
+                    float4 c = make_float4(0.f, 0.f, 0.f, 0.f); float byz = 0.f;
+                    if (QUAD) { c = bf.q2[j]; byz = bf.q3[j]; }
+#pragma unroll
+                    for (int k = 0; k < NI; ++k)
+                        cell_term<QUAD>(p[k], (a.x + ix[k]) + (b.x + lx[k]), (a.y + iy[k]) + (b.y + ly[k]), (a.z + iz[k]) + (b.z + lz[k]), a.w, b.w, c.x, c.y, c.z, c.w, byz);
+                } else {
+                    float4 b = make_float4(0.f, 0.f, 0.f, 0.f); float2 c = make_float2(0.f, 0.f);
+                    if (QUAD) { b = bf.q1[j]; c = *reinterpret_cast<const float2*>(&bf.q2[j]); }
+#pragma unroll
+                    for (int k = 0; k < NI; ++k)
+                        cell_term<QUAD>(p[k], a.x - ix[k], a.y - iy[k], a.z - iz[k], a.w, b.x, b.y, b.z, b.w, c.x, c.y);
+                }
+            }
+            if (++fl >= fl_every) {
+                fl = 0;
+#pragma unroll
+                for (int k = 0; k < NI; ++k) flush_smem(p[k], sacc + 4 * k * (UW * 32));
+            }
+        }
+        store_recs(bufs[cb ^ 1]); tn0 = tn1;
+        load_recs();
+        load_ids();
+        cb ^= 1;
+        __syncwarp();
+    }
+    if (active) {
+#pragma unroll
+        for (int k = 0; k < NI; ++k) flush_smem(p[k], sacc + 4 * k * (UW * 32));
+    }
+}
+
+template <bool QUAD>
+__global__ void __launch_bounds__(UW * 32, UNITS_MIN_CTAS) k_force_units(DevHeader* __restrict__ h, const ForceUnit* __restrict__ units, const SuperRec* __restrict__ srec,
+                                                            const int group_cap, const NodeW* __restrict__ nw, const int* __restrict__ arena,
+                                                            const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
+                                                            double* __restrict__ part, const long long n_part) {
+    __shared__ __align__(16) UBuf s_buf[UW][2];
+    __shared__ double s_acc[4 * NI][UW * 32];
+    __shared__ int s_u;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double* sacc = &s_acc[0][threadIdx.x];
+    const int nu = h->unit_off[PETAR_UNIT_CLASSES];
+    for (;;) {
+        __syncthreads();                    // s_u and s_acc of the previous unit consumed
+        if (threadIdx.x == 0) s_u = atomicAdd(&h->unit_ticket, 1);
+        __syncthreads();
+        const int u = s_u;
+        if (u >= nu) break;
+        const ForceUnit fu = units[u];
+        const SuperRec* sr = &srec[(size_t)fu.level * group_cap + fu.rec];
+        const int cnt = fu.cnt;
+        const int P = (cnt + NI - 1) / NI, S = 32 / P;
+        const int slot = lane % P, slice = lane / P;
+        const bool active = slice < S;
+        const int i0 = fu.ibeg + NI * slot, ilast = fu.ibeg + cnt - 1;
+        // any fp32 point inside the super-group's box serves as the origin of the group-relative floats
+        const float4 ba = nw[sr->node].a, bb = nw[sr->node].b;
+        const float3 gh = make_float3(0.5f * (ba.x + ba.w), 0.5f * (ba.y + bb.x), 0.5f * (ba.z + bb.y));
+#pragma unroll
+        for (int c = 0; c < 4 * NI; ++c) sacc[c * (UW * 32)] = 0.0;
+        unit_phase<QUAD, false>(s_buf[w], arena, nsp, sr->head_sp, sr->n_sp, w, lane, slice, S, active, pa, pb, i0, ilast, gh, sacc);
+        unit_phase<QUAD, true>(s_buf[w], arena, nsp, sr->head_spp, sr->n_spp, w, lane, slice, S, active, pa, pb, i0, ilast, gh, sacc);
+        // ordered reduction over the warps and their slices
+        __syncthreads();
+        double* out = part + ((size_t)fu.level * n_part + fu.ibeg) * 4;
+        for (int e = threadIdx.x; e < cnt * 4; e += UW * 32) {
+            const int i = e >> 2, comp = e & 3;
+            double sum = 0.0;
+            for (int ww = 0; ww < UW; ++ww)
+                for (int sl = 0; sl < S; ++sl) sum += s_acc[(i % NI) * 4 + comp][ww * 32 + sl * P + (i / NI)];
+            out[e] = sum;
+        }
+    }
+}
+
+// unit table: every super-group is cut into units of 128 particles, then at most one of 64, one of 32 and
+// one of < 32; units are stored by size class (largest first) so the ticket order ends with the small ones
+template <class F>
+__device__ __forceinline__ void for_units(const int begin, const int n, F f) {
+    int b = begin, r = n;
+    while (r >= UNIT_MAX) { f(0, b, UNIT_MAX); b += UNIT_MAX; r -= UNIT_MAX; }
+    if (r >= UNIT_MAX / 2) { f(1, b, UNIT_MAX / 2); b += UNIT_MAX / 2; r -= UNIT_MAX / 2; }
+    if (r >= UNIT_MAX / 4) { f(2, b, UNIT_MAX / 4); b += UNIT_MAX / 4; r -= UNIT_MAX / 4; }
+    if (r > 0) f(3, b, r);
+}
+__global__ void __launch_bounds__(256) k_units_count(DevHeader* __restrict__ h, const SuperRec* __restrict__ srec, const int group_cap) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+#pragma unroll
+    for (int l = 0; l < PETAR_NSUP; ++l) {
+        if (id >= h->n_super[l]) continue;
+        const SuperRec* sr = &srec[(size_t)l * group_cap + id];
+        int c[PETAR_UNIT_CLASSES] = {0, 0, 0, 0};
+        for_units(sr->begin, sr->end - sr->begin, [&](int cls, int, int) { ++c[cls]; });
+#pragma unroll
+        for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) if (c[k]) atomicAdd(&h->unit_cnt[k], c[k]);
+    }
+}
+__global__ void k_units_offsets(DevHeader* h, const int unit_cap) {
+    if (threadIdx.x == 0) {
+        int o = 0;
+        for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) { h->unit_off[k] = o; o += h->unit_cnt[k]; h->unit_fill[k] = 0; }
+        if (o > unit_cap) { atomicOr(&h->status, PETAR_ST_LIST_CAP); o = 0; }      // cannot happen: <= one unit per particle and level
+        h->unit_off[PETAR_UNIT_CLASSES] = o;
+    }
+}
+__global__ void __launch_bounds__(256) k_units_fill(DevHeader* __restrict__ h, const SuperRec* __restrict__ srec, const int group_cap, ForceUnit* __restrict__ units) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h->unit_off[PETAR_UNIT_CLASSES] == 0) return;
+#pragma unroll
+    for (int l = 0; l < PETAR_NSUP; ++l) {
+        if (id >= h->n_super[l]) continue;
+        const SuperRec* sr = &srec[(size_t)l * group_cap + id];
+        for_units(sr->begin, sr->end - sr->begin, [&](int cls, int b, int cnt) {
+            const int at = h->unit_off[cls] + atomicAdd(&h->unit_fill[cls], 1);
+            ForceUnit fu; fu.rec = id; fu.ibeg = b; fu.cnt = cnt; fu.level = l;
+            units[at] = fu;
+        });
+    }
+}
+
+__global__ void k_reset_ticket2(DevHeader* h) {
+    if (threadIdx.x == 0) { h->group_ticket2 = 0; h->unit_ticket = 0; for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) h->unit_cnt[k] = 0; }
+}
 
 cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s) {
     Workspace& w = t->w;
@@ -402,19 +653,36 @@ cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, doub
     stage_begin(t, s);
     k_reset_ticket2<<<1, 32, 0, s>>>(w.hdr);
     KCHECK(s, "k_reset_ticket2");
+    const bool quad = t->p.multipole >= 2;
+    // phase A: unit table, then the super-groups' common cells
+    const int nrec_blocks = cdiv(w.group_cap, 256);
+    k_units_count<<<nrec_blocks, 256, 0, s>>>(w.hdr, w.srec, w.group_cap);
+    KCHECK(s, "k_units_count");
+    k_units_offsets<<<1, 32, 0, s>>>(w.hdr, w.unit_cap);
+    KCHECK(s, "k_units_offsets");
+    k_units_fill<<<nrec_blocks, 256, 0, s>>>(w.hdr, w.srec, w.group_cap, w.units);
+    KCHECK(s, "k_units_fill");
     int per_sm = 0;
     cudaError_t e;
-    if (t->p.multipole >= 2) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<true>, FT, 0);
+    if (quad) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force_units<true>, UW * 32, 0);
+    else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force_units<false>, UW * 32, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    if (quad) k_force_units<true><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, (long long)t->N);
+    else k_force_units<false><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, (long long)t->N);
+    KCHECK(s, "k_force_units");
+    // phase B: the groups' own lists
+    if (quad) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<true>, FT, 0);
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<false>, FT, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     const int grid = t->sm_count * per_sm;
-    if (t->p.multipole >= 2)
-        k_force<true><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.srec, ax, ay, az, pot, fc, t->p.G);
+    if (quad)
+        k_force<true><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.part, (long long)t->N, ax, ay, az, pot, fc, t->p.G);
     else
-        k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.srec, ax, ay, az, pot, fc, t->p.G);
+        k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.part, (long long)t->N, ax, ay, az, pot, fc, t->p.G);
     KCHECK(s, "k_force");
-    petar_count_launch(2);
+    petar_count_launch(6);
     stage_end(t, PETAR_STAGE_FORCE, s);
     return cudaGetLastError();
 }

@@ -10,6 +10,18 @@
 #define PETAR_CHUNK 1024           // list arena chunk, in 4-byte entries; [0] = next chunk (or -1), [1] unused
 #define PETAR_CHUNK_HDR 2
 #define PETAR_CHUNK_PAYLOAD (PETAR_CHUNK - PETAR_CHUNK_HDR)   // 1022 entries (even: EP ranges are pairs)
+// super-group levels (see SuperRec): level l holds the tree cells with <= PETAR_SUP_LIMIT(l) members
+#ifndef PETAR_NSUP
+#define PETAR_NSUP 2
+#endif
+#ifndef PETAR_SUP_T0
+#define PETAR_SUP_T0 4096
+#endif
+#ifndef PETAR_SUP_T1
+#define PETAR_SUP_T1 512
+#endif
+#define PETAR_SUP_LIMIT(l) ((l) == 0 ? PETAR_SUP_T0 : PETAR_SUP_T1)
+#define PETAR_UNIT_CLASSES 4       // phase-A force units of 128, 64, 32 and < 32 particles
 
 // ---- device-resident header (one per tree, lives at the start of the workspace) -----------------
 struct DevHeader {
@@ -27,9 +39,13 @@ struct DevHeader {
     int group_ticket;   // dynamic scheduling counters (reset before each consumer kernel)
     int group_ticket2;
     int group_ticket3;
-    int n_super;
-    int super_ticket;
-    int pad_;
+    int n_super[PETAR_NSUP];       // super-groups per level
+    int super_ticket[PETAR_NSUP];
+    int unit_cnt[PETAR_UNIT_CLASSES];      // force units (phase A) per size class
+    int unit_off[PETAR_UNIT_CLASSES + 1];
+    int unit_fill[PETAR_UNIT_CLASSES];
+    int unit_ticket;
+    int pad_[2];
     unsigned long long n_epep, n_epsp, n_epep_near, n_ep_list, n_sp_list;
     unsigned long long nb_total;
 };
@@ -56,16 +72,14 @@ struct __align__(16) GroupRec {
     int n_ep_part, n_epn_part;         // particles in all EP ranges / in near ranges
     int head_spp, n_spp;               // cells closer than the group's own size: float-float ("precise") path
     double lo[3], hi[3], rmax;
-    int sid;                           // super-group (see SuperRec) this group lies in
-    int pad2;
+    int sid[2];                        // super-group (see SuperRec) of each level this group lies in
 };
 
-// super-group: tree cell with <= PETAR_N_SUPER members (parent has more).  Its walk decides, once for all
-// the i-groups inside it, the cells that every one of them accepts ("common" lists) and leaves the rest
-// ("deferred" cells) to the per-group walks, which start from them instead of from the root.
-#ifndef PETAR_N_SUPER
-#define PETAR_N_SUPER 512
-#endif
+// super-group of level l: tree cell with <= PETAR_SUP_LIMIT(l) members (parent has more).  Its walk decides,
+// once for all the i-groups inside it, the cells that every one of them accepts ("common" lists) and
+// leaves the rest ("deferred" cells) to the next level's walks (level l+1 super-groups, finally the
+// i-groups), which start from them instead of from the root.  Records of level l live at
+// srec[l * group_cap + id], the map sorted position -> id at smap[l * N + position].
 struct __align__(16) SuperRec {
     int node, begin, end;
     int head_sp, n_sp;                 // common cells, group-relative path
@@ -73,6 +87,9 @@ struct __align__(16) SuperRec {
     int head_def, n_def;               // deferred cells (node ids)
     int pad[3];
 };
+
+// phase-A force unit: <= 128 consecutive particles of one super-group against its common cell lists
+struct __align__(16) ForceUnit { int rec; int ibeg; int cnt; int level; };
 
 struct Workspace {
     DevHeader* hdr;
@@ -95,8 +112,10 @@ struct Workspace {
     int node_cap;
     // groups
     GroupRec* grp; int group_cap;
-    SuperRec* srec;                // [group_cap] super-groups
-    int* smap;                     // [N] sorted position -> super-group id
+    SuperRec* srec;                // [PETAR_NSUP][group_cap] super-groups
+    int* smap;                     // [PETAR_NSUP][N] sorted position -> super-group id
+    struct ForceUnit* units; int unit_cap;   // phase-A force units (force.cu)
+    double* part;                  // [PETAR_NSUP][N][4] phase-A partial sums (sorted order): ax, ay, az, pot
     // list arena
     int* arena; int arena_chunks;
     // neighbour temporaries

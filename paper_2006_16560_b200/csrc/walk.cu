@@ -52,12 +52,13 @@ __device__ __forceinline__ void list_append(ListCursor& c, bool take, int per, i
 }
 
 // ------------------------------------------------------------------------------------------------
-// Super-groups.  A node is a super-group iff (count <= PETAR_N_SUPER or it is a leaf) and its parent
-// holds more than PETAR_N_SUPER particles (or it is the root).  Every i-group lies inside exactly one.
+// Super-groups.  A node is a level-l super-group iff (count <= T_l or it is a leaf) and its parent
+// holds more than T_l particles (or it is the root).  T_l >= n_group_limit, so every i-group lies inside
+// exactly one super-group of every level, and a level-(l+1) super-group inside exactly one of level l.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_super_collect(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
                                                        const unsigned long long* __restrict__ key, long long n,
-                                                       SuperRec* __restrict__ srec, int node_cap) {
+                                                       SuperRec* __restrict__ srec, int node_cap, int lvl, int limit) {
     const int nn = h->n_nodes;
     if (nn > node_cap) return;
     const int id = blockIdx.x * blockDim.x + threadIdx.x;
@@ -65,7 +66,7 @@ __global__ void __launch_bounds__(256) k_super_collect(DevHeader* __restrict__ h
     const int4 d = nw[id].d;
     const int level = d.w & 255;
     const bool leaf = (d.w >> 16) & 1;
-    if (!(d.y - d.x <= PETAR_N_SUPER || leaf)) return;
+    if (!(d.y - d.x <= limit || leaf)) return;
     if (level > 0) {
         // parent's particle count: the range of keys that share the level-1 prefix of this cell
         const int shift = 3 * (PETAR_MAXLEVEL - (level - 1));
@@ -75,9 +76,9 @@ __global__ void __launch_bounds__(256) k_super_collect(DevHeader* __restrict__ h
         const long long pb = lo;
         lo = d.y; hi = n;                           // first index whose prefix exceeds pref
         while (lo < hi) { long long mid = (lo + hi) >> 1; if (((level - 1 > 0) ? (key[mid] >> shift) : 0ull) <= pref) lo = mid + 1; else hi = mid; }
-        if (lo - pb <= PETAR_N_SUPER) return;       // an ancestor is the super-group
+        if (lo - pb <= limit) return;               // an ancestor is the super-group
     }
-    const int sid = atomicAdd(&h->n_super, 1);
+    const int sid = atomicAdd(&h->n_super[lvl], 1);
     SuperRec r;
     r.node = id; r.begin = d.x; r.end = d.y;
     r.head_sp = r.head_spp = r.head_def = -1; r.n_sp = r.n_spp = r.n_def = 0;
@@ -85,9 +86,9 @@ __global__ void __launch_bounds__(256) k_super_collect(DevHeader* __restrict__ h
     srec[sid] = r;
 }
 
-__global__ void __launch_bounds__(256) k_super_map(const DevHeader* __restrict__ h, const SuperRec* __restrict__ srec, int* __restrict__ smap) {
+__global__ void __launch_bounds__(256) k_super_map(const DevHeader* __restrict__ h, const SuperRec* __restrict__ srec, int* __restrict__ smap, int lvl) {
     const int lane = threadIdx.x & 31;
-    const int ns = h->n_super;
+    const int ns = h->n_super[lvl];
     for (int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; s < ns; s += (gridDim.x * blockDim.x) >> 5)
         for (int p = srec[s].begin + lane; p < srec[s].end; p += 32) smap[p] = s;
 }
@@ -133,21 +134,24 @@ __device__ __noinline__ int mac_exact(const NodeMac* __restrict__ cp, const int 
 //   anything else (and every leaf) is DEFERRED to the per-group walks.
 // Hence the cells a group accepts are exactly S's common cells plus what its own walk finds below the
 // deferred cells - the same set rule O7 gives when walked from the root.
+// A super-group of level l > 0 starts from the cells its level-(l-1) super-group deferred (psrec / psmap);
+// level 0 starts from the root.
 __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk_super(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
-                                                                SuperRec* __restrict__ srec, int* __restrict__ arena, int arena_chunks,
-                                                                double theta, int node_cap) {
+                                                                SuperRec* __restrict__ srec, const SuperRec* __restrict__ psrec,
+                                                                const int* __restrict__ psmap, int* __restrict__ arena, int arena_chunks,
+                                                                double theta, int node_cap, int lvl) {
     __shared__ int s_stack[WALK_WARPS][WALK_STACK];
     __shared__ float s_lt[PETAR_NLEVELS];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     int* stack = s_stack[w];
-    const int ns = h->n_super;
+    const int ns = h->n_super[lvl];
     if (h->n_nodes > node_cap || h->n_nodes <= 0) return;
     const double twoh = 2.0 * h->h;
     if (threadIdx.x < PETAR_NLEVELS) s_lt[threadIdx.x] = (theta > 0.0) ? (float)(ldexp(twoh, -(int)threadIdx.x) / theta) : INFINITY;
     __syncthreads();
     for (;;) {
         int s = 0;
-        if (lane == 0) s = atomicAdd(&h->super_ticket, 1);
+        if (lane == 0) s = atomicAdd(&h->super_ticket[lvl], 1);
         s = __shfl_sync(0xffffffffu, s, 0);
         if (s >= ns) break;
         const NodeW sb = nw[srec[s].node];           // the super-group's own cell: tight box, rmax, eps
@@ -157,10 +161,20 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk_super(DevHeader* __res
         const float gedge2 = gedge * gedge;
         ListCursor lsp = {-1, -1, 0, 0}, lspp = {-1, -1, 0, 0}, ldef = {-1, -1, 0, 0};
         int n_sp = 0, n_spp = 0, n_def = 0;
-        int top = 1;
-        if (lane == 0) stack[0] = 0;
+        int top = 0, dchunk = -1, dremaining = 0, doff = 0;
+        if (psrec) { const SuperRec* pr = &psrec[psmap[srec[s].begin]]; dchunk = pr->head_def; dremaining = pr->n_def; }
+        else { top = 1; if (lane == 0) stack[0] = 0; }
         __syncwarp();
-        while (top > 0) {
+        while (top > 0 || dremaining > 0) {
+            if (top == 0) {                    // frontier empty: take the next (up to 256) cells the parent deferred
+                if (dchunk < 0) break;         // truncated list (arena exhausted, PETAR_ST_LIST_CAP is set)
+                const int* cp = arena + (size_t)dchunk * PETAR_CHUNK;
+                const int k = min(256, min(dremaining, PETAR_CHUNK_PAYLOAD - doff));
+                for (int e = lane; e < k; e += 32) stack[e] = cp[PETAR_CHUNK_HDR + doff + e];
+                top = k; dremaining -= k; doff += k;
+                if (dremaining > 0 && doff >= PETAR_CHUNK_PAYLOAD) { dchunk = cp[0]; doff = 0; }
+                __syncwarp();
+            }
             int p = min(32, top);
             if (top + 7 * p > WALK_STACK - WALK_RESERVE) p = max(1, min(p, (WALK_STACK - WALK_RESERVE - top) / 7));
             const int node = (lane < p) ? stack[top - p + lane] : -1;
@@ -214,7 +228,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk_super(DevHeader* __res
                 if (lane >= o) pref += a;
             }
             const int total_push = __shfl_sync(0xffffffffu, pref, 31);
-            if (top + total_push > WALK_STACK) { if (lane == 0) atomicOr(&h->status, PETAR_ST_STACK); top = 0; break; }
+            if (top + total_push > WALK_STACK) { if (lane == 0) atomicOr(&h->status, PETAR_ST_STACK); top = 0; break; }   // cannot happen (throttle above)
             const int at = top + pref - push;
             for (int k = 0; k < push; ++k) stack[at + k] = fc + k;
             top += total_push;
@@ -235,7 +249,8 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk_super(DevHeader* __res
 __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
                                                           const NodeMac* __restrict__ nmac, GroupRec* __restrict__ grp,
                                                           const SuperRec* __restrict__ srec, const int* __restrict__ smap,
-                                                          int* __restrict__ arena, int arena_chunks, double theta, int node_cap) {
+                                                          int* __restrict__ arena, int arena_chunks, double theta, int node_cap,
+                                                          long long n_part, int group_cap) {
     __shared__ int s_stack[WALK_WARPS][WALK_STACK];
     __shared__ float s_lt[PETAR_NLEVELS];          // edge(level) / theta  (inf when theta == 0: nothing is ever "far")
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -266,12 +281,15 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
         const float gedge = fmaxf(fh0 - fl0, fmaxf(fh1 - fl1, fh2 - fl2));
         const float gedge2 = gedge * gedge;
         // the walk starts from the cells the super-group's walk deferred (k_walk_super), fed in batches
-        const int sid = smap[gr->begin];
-        const SuperRec* sr = &srec[sid];
+        int sid[PETAR_NSUP];
+#pragma unroll
+        for (int l = 0; l < PETAR_NSUP; ++l) sid[l] = smap[(size_t)l * n_part + gr->begin];
+        const SuperRec* sr = &srec[(size_t)(PETAR_NSUP - 1) * group_cap + sid[PETAR_NSUP - 1]];
         int dchunk = sr->head_def, dremaining = sr->n_def, doff = 0;
         int top = 0;
         while (top > 0 || dremaining > 0) {
             if (top == 0) {                    // frontier empty: take the next (up to 256) deferred cells
+                if (dchunk < 0) break;         // truncated list (arena exhausted, PETAR_ST_LIST_CAP is set)
                 const int* cp = arena + (size_t)dchunk * PETAR_CHUNK;
                 const int k = min(256, min(dremaining, PETAR_CHUNK_PAYLOAD - doff));
                 for (int e = lane; e < k; e += 32) stack[e] = cp[PETAR_CHUNK_HDR + doff + e];
@@ -355,9 +373,12 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
             go->n_sp = n_sp; go->n_epn = n_epn; go->n_epf = n_epf;
             go->head_spp = lspp.head; go->n_spp = n_spp;
             go->n_ep_part = n_ep_part; go->n_epn_part = n_epn_part;
-            go->sid = sid;
+#pragma unroll
+            for (int l = 0; l < PETAR_NSUP; ++l) go->sid[l] = sid[l];
         }
-        const int n_common = sr->n_sp + sr->n_spp;
+        int n_common = 0;
+#pragma unroll
+        for (int l = 0; l < PETAR_NSUP; ++l) { const SuperRec* q = &srec[(size_t)l * group_cap + sid[l]]; n_common += q->n_sp + q->n_spp; }
         t_epep += (unsigned long long)n_i * (unsigned long long)n_ep_part;
         t_near += (unsigned long long)n_i * (unsigned long long)n_epn_part;
         t_epsp += (unsigned long long)n_i * (unsigned long long)(n_sp + n_spp + n_common);
@@ -371,7 +392,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
 }
 
 __global__ void k_reset_ticket(DevHeader* h, int which) {
-    if (threadIdx.x == 0) { if (which == 0) { h->group_ticket = 0; h->arena_top = 0; h->n_super = 0; h->super_ticket = 0; h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = 0ull; } else h->group_ticket3 = 0; }
+    if (threadIdx.x == 0) { if (which == 0) { h->group_ticket = 0; h->arena_top = 0; for (int l = 0; l < PETAR_NSUP; ++l) { h->n_super[l] = 0; h->super_ticket[l] = 0; } h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = 0ull; } else h->group_ticket3 = 0; }
 }
 
 cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
@@ -383,15 +404,21 @@ cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_walk, WALK_WARPS * 32, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
-    k_super_collect<<<cdiv(w.node_cap, 256), 256, 0, s>>>(w.hdr, w.nw, w.key, t->N, w.srec, w.node_cap);
-    KCHECK(s, "k_super_collect");
-    k_super_map<<<t->sm_count * 8, 256, 0, s>>>(w.hdr, w.srec, w.smap);
-    KCHECK(s, "k_super_map");
-    k_walk_super<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, w.srec, w.arena, w.arena_chunks, t->p.theta, w.node_cap);
-    KCHECK(s, "k_walk_super");
-    k_walk<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, w.nmac, w.grp, w.srec, w.smap, w.arena, w.arena_chunks, t->p.theta, w.node_cap);
+    for (int l = 0; l < PETAR_NSUP; ++l) {
+        SuperRec* sl = w.srec + (size_t)l * w.group_cap;
+        int* ml = w.smap + (size_t)l * t->N;
+        k_super_collect<<<cdiv(w.node_cap, 256), 256, 0, s>>>(w.hdr, w.nw, w.key, t->N, sl, w.node_cap, l, PETAR_SUP_LIMIT(l));
+        KCHECK(s, "k_super_collect");
+        k_super_map<<<t->sm_count * 8, 256, 0, s>>>(w.hdr, sl, ml, l);
+        KCHECK(s, "k_super_map");
+        k_walk_super<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, sl, l ? sl - w.group_cap : nullptr, l ? ml - t->N : nullptr,
+                                                                     w.arena, w.arena_chunks, t->p.theta, w.node_cap, l);
+        KCHECK(s, "k_walk_super");
+    }
+    k_walk<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, w.nmac, w.grp, w.srec, w.smap, w.arena, w.arena_chunks, t->p.theta, w.node_cap,
+                                                          (long long)t->N, w.group_cap);
     KCHECK(s, "k_walk");
-    petar_count_launch(5);
+    petar_count_launch(2 + 3 * PETAR_NSUP);
     stage_end(t, PETAR_STAGE_WALK, s);
     return cudaGetLastError();
 }
@@ -490,12 +517,17 @@ cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, 
 // ------------------------------------------------------------------------------------------------
 // list export (tests): flatten the chunk chains.
 // ------------------------------------------------------------------------------------------------
-__global__ void k_list_sizes(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const SuperRec* __restrict__ srec, int* __restrict__ sizes) {
+__device__ __forceinline__ int common_cells(const GroupRec* gr, const SuperRec* __restrict__ srec, int group_cap) {
+    int c = 0;
+    for (int l = 0; l < PETAR_NSUP; ++l) { const SuperRec* q = &srec[(size_t)l * group_cap + gr->sid[l]]; c += q->n_sp + q->n_spp; }
+    return c;
+}
+__global__ void k_list_sizes(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const SuperRec* __restrict__ srec, int group_cap, int* __restrict__ sizes) {
     int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= h->n_groups) return;
-    sizes[3 * g] = grp[g].n_sp + grp[g].n_spp + srec[grp[g].sid].n_sp + srec[grp[g].sid].n_spp; sizes[3 * g + 1] = 2 * grp[g].n_epn; sizes[3 * g + 2] = 2 * grp[g].n_epf;
+    sizes[3 * g] = grp[g].n_sp + grp[g].n_spp + common_cells(&grp[g], srec, group_cap); sizes[3 * g + 1] = 2 * grp[g].n_epn; sizes[3 * g + 2] = 2 * grp[g].n_epf;
 }
-__global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const SuperRec* __restrict__ srec, const int* __restrict__ arena,
+__global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const SuperRec* __restrict__ srec, int group_cap, const int* __restrict__ arena,
                                const long long* __restrict__ offs, int* __restrict__ out, long long out_entries) {
     const int lane = threadIdx.x & 31;
     long long wid = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -504,7 +536,7 @@ __global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* 
     int chunk = which == 0 ? grp[g].head_sp : which == 1 ? grp[g].head_epn : grp[g].head_epf;
     int remaining = which == 0 ? grp[g].n_sp : which == 1 ? 2 * grp[g].n_epn : 2 * grp[g].n_epf;
     long long o = offs[wid];
-    for (int part = 0; part < 4; ++part) {
+    for (int part = 0; part < 2 + 2 * PETAR_NSUP; ++part) {
         while (chunk >= 0 && remaining > 0) {
             const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
             int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
@@ -512,18 +544,25 @@ __global__ void k_list_flatten(const DevHeader* __restrict__ h, const GroupRec* 
             o += ne; remaining -= ne; chunk = cp[0];
         }
         if (which != 0) break;
-        // "SP" = own plain cells, own precise cells, then the super-group's common cells (plain, precise)
-        const SuperRec* sr = &srec[grp[g].sid];
+        // "SP" = own plain cells, own precise cells, then every level's common cells (plain, precise)
         if (part == 0) { chunk = grp[g].head_spp; remaining = grp[g].n_spp; }
-        else if (part == 1) { chunk = sr->head_sp; remaining = sr->n_sp; }
-        else if (part == 2) { chunk = sr->head_spp; remaining = sr->n_spp; }
+        else if (part < 1 + 2 * PETAR_NSUP) {
+            const SuperRec* sr = &srec[(size_t)((part - 1) >> 1) * group_cap + grp[g].sid[(part - 1) >> 1]];
+            if ((part - 1) & 1) { chunk = sr->head_spp; remaining = sr->n_spp; } else { chunk = sr->head_sp; remaining = sr->n_sp; }
+        }
     }
 }
-__global__ void k_group_cnt(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const SuperRec* __restrict__ srec, int* __restrict__ out, int what, int walked) {
+__global__ void k_group_cnt(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const SuperRec* __restrict__ srec, int group_cap, int* __restrict__ out, int what, int walked) {
     int g = blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= h->n_groups) return;
-    if (what == PETAR_DBG_GROUP_CNT) { out[4 * g] = grp[g].n_sp + grp[g].n_spp + (walked ? srec[grp[g].sid].n_sp + srec[grp[g].sid].n_spp : 0); out[4 * g + 1] = grp[g].n_epn; out[4 * g + 2] = grp[g].n_epf; out[4 * g + 3] = grp[g].n_ep_part; }
-    else if (what == PETAR_DBG_GROUP_SUPER) { const SuperRec* sr = &srec[grp[g].sid]; out[4 * g] = grp[g].sid; out[4 * g + 1] = sr->end - sr->begin; out[4 * g + 2] = sr->n_sp + sr->n_spp; out[4 * g + 3] = sr->n_def; }
+    if (what == PETAR_DBG_GROUP_CNT) { out[4 * g] = grp[g].n_sp + grp[g].n_spp + (walked ? common_cells(&grp[g], srec, group_cap) : 0); out[4 * g + 1] = grp[g].n_epn; out[4 * g + 2] = grp[g].n_epf; out[4 * g + 3] = grp[g].n_ep_part; }
+    else if (what == PETAR_DBG_GROUP_SUPER) {
+        for (int l = 0; l < 2; ++l) {
+            const int ll = l < PETAR_NSUP ? l : PETAR_NSUP - 1;
+            const SuperRec* sr = &srec[(size_t)ll * group_cap + grp[g].sid[ll]];
+            out[8 * g + 4 * l] = grp[g].sid[ll]; out[8 * g + 4 * l + 1] = sr->end - sr->begin; out[8 * g + 4 * l + 2] = sr->n_sp + sr->n_spp; out[8 * g + 4 * l + 3] = sr->n_def;
+        }
+    }
     else { out[2 * g] = grp[g].begin; out[2 * g + 1] = grp[g].end; }
 }
 __global__ void k_group_dbl(const DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, double* __restrict__ out) {
@@ -547,9 +586,9 @@ cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_b
     Workspace& w = t->w;
     int ng = t->pinned[1], nn = t->pinned[0];
     if (what == PETAR_DBG_GROUP_CNT || what == PETAR_DBG_GROUP_INT || what == PETAR_DBG_GROUP_SUPER) {
-        size_t need = (size_t)ng * (what == PETAR_DBG_GROUP_INT ? 8 : 16);
+        size_t need = (size_t)ng * (what == PETAR_DBG_GROUP_INT ? 8 : what == PETAR_DBG_GROUP_SUPER ? 32 : 16);
         if (dst_bytes < need) return cudaErrorInvalidValue;
-        if (ng) k_group_cnt<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, (int*)dst, what, t->walked ? 1 : 0);
+        if (ng) k_group_cnt<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, w.group_cap, (int*)dst, what, t->walked ? 1 : 0);
         KCHECK(s, "k_group_cnt");
     } else if (what == PETAR_DBG_GROUP_DBL) {
         if (dst_bytes < (size_t)ng * 56) return cudaErrorInvalidValue;
@@ -564,7 +603,7 @@ cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_b
         if (!ng) return cudaSuccess;
         int* sizes = w.exp_scratch;                                       // 3 ng ints
         long long* offs = (long long*)(w.exp_scratch + 4ll * (ng + 1));   // 3 ng + 1 int64 (16-byte aligned)
-        k_list_sizes<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, sizes);
+        k_list_sizes<<<cdiv(ng, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, w.group_cap, sizes);
         KCHECK(s, "k_list_sizes");
         cudaError_t e = launch_scan_i32_to_i64(sizes, offs, 3ll * ng, (long long*)w.scan_tmp, s);
         if (e != cudaSuccess) return e;
@@ -572,7 +611,7 @@ cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_b
             if (dst_bytes < (size_t)(3ll * ng + 1) * 8) return cudaErrorInvalidValue;
             return cudaMemcpyAsync(dst, offs, (size_t)(3ll * ng + 1) * 8, cudaMemcpyDeviceToDevice, s);
         }
-        k_list_flatten<<<cdiv(3ll * ng * 32, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, w.arena, offs, (int*)dst, (long long)(dst_bytes / 4));
+        k_list_flatten<<<cdiv(3ll * ng * 32, 256), 256, 0, s>>>(w.hdr, w.grp, w.srec, w.group_cap, w.arena, offs, (int*)dst, (long long)(dst_bytes / 4));
         KCHECK(s, "k_list_flatten");
     }
     return cudaGetLastError();
