@@ -32,6 +32,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 FLOP_NEWTON, FLOP_CUT, FLOP_QUAD = 20, 49, 53      # fixed flops-per-interaction convention
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/), bytes
+TRAFFIC_NCU = {"k_force_units": None, "k_force": None}
 
 
 def parse():
@@ -203,8 +205,11 @@ def main():
     cap = [torch.empty(int(nb_total * 1.1) + 1024, dtype=torch.int32, device=dev)]
     n_inter = counts.n_epep + counts.n_epsp
     quad = params.multipole >= 2
-    flops_step = (FLOP_CUT * counts.n_epep_near + FLOP_NEWTON * (counts.n_epep - counts.n_epep_near)
-                  + (FLOP_QUAD if quad else FLOP_NEWTON) * counts.n_epsp)
+    flop_sp = FLOP_QUAD if quad else FLOP_NEWTON
+    flops_units = flop_sp * counts.n_epsp_common                      # phase A: k_force_units (super-group-wide cells)
+    flops_groups = (FLOP_CUT * counts.n_epep_near + FLOP_NEWTON * (counts.n_epep - counts.n_epep_near)
+                    + flop_sp * (counts.n_epsp - counts.n_epsp_common))  # phase B: k_force (the groups' own lists)
+    flops_step = flops_units + flops_groups
 
     for _ in range(W):
         flush.fill_(1)
@@ -276,6 +281,17 @@ def main():
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(stream); fl = P.petar_probe_fp32(400000, scratch, stream); b.record(stream); b.synchronize()
     probe_tflops = fl / (a.elapsed_time(b) * 1e-3) / 1e12
+    # the same with three distinct register operands per FFMA, and the kernel's own cell term on register operands
+    probes = {}
+    for mode, name, iters in ((1, "ffma_3_distinct_registers", 400000), (2, "quadrupole_cell_term_loop", 2000)):
+        P.petar_probe_fp32_mode(mode, max(1, iters // 50), scratch, stream)
+        torch.cuda.synchronize()
+        a.record(stream); fl = P.petar_probe_fp32_mode(mode, iters, scratch, stream); b.record(stream); b.synchronize()
+        probes[name] = fl / (a.elapsed_time(b) * 1e-3) / 1e12
+
+    pk, pk_kind = peaks()
+    sm_max = float(pk.get("sm_max_mhz", 1965.0))
+    nominal_fp32 = 2 * 128 * 148 * sm_max * 1e6 / 1e12
 
     # ---- aggregate over ranks --------------------------------------------------------------------------
     ms_step = ms_total / K
@@ -290,12 +306,16 @@ def main():
     value = tot_inter / (ms_step * 1e-3)
     e2e_value = tot_inter / (e2e_ms * 1e-3)
 
-    pk, pk_kind = peaks()
-    sm_max = float(pk.get("sm_max_mhz", 1965.0))
-    nominal_fp32 = 2 * 128 * 148 * sm_max * 1e6 / 1e12
-    force_ms = stage_sum["force"] / K
-    achieved = flops_step / (force_ms * 1e-3) / 1e12
     stage_ms = {k: v / K for k, v in stage_sum.items()}
+    kern = [dict(kernel="k_force_units", ms=stage_ms["force_units"], flops_per_launch=float(flops_units)),
+            dict(kernel="k_force", ms=stage_ms["force"], flops_per_launch=float(flops_groups))]
+    for kd in kern:
+        kd["achieved"] = kd["flops_per_launch"] / (kd["ms"] * 1e-3) / 1e12 if kd["ms"] > 0 else 0.0
+        kd["frac"] = kd["achieved"] / nominal_fp32
+        kd["share_of_step"] = kd["ms"] / ms_step
+    dom = max(kern, key=lambda kd: kd["ms"])                  # the dominant kernel of the step
+    force_ms = stage_ms["force_units"] + stage_ms["force"]
+    achieved_both = flops_step / (force_ms * 1e-3) / 1e12
 
     if rank == 0:
         out = dict(
@@ -314,12 +334,16 @@ def main():
                      d2h_bytes_per_step=d2h_bytes, steps=Ke),
             gpu_launches=int(launches),
             clocks=clocks,
-            roofline=dict(bound="alu", kernel="k_force", achieved=achieved, peak=nominal_fp32, unit="TFLOP/s",
-                          frac=achieved / nominal_fp32, traffic=None,
+            roofline=dict(bound="alu", kernel=dom["kernel"], achieved=dom["achieved"], peak=nominal_fp32, unit="TFLOP/s",
+                          frac=dom["frac"], traffic=TRAFFIC_NCU.get(dom["kernel"]),
                           peak_kind=f"nominal CUDA-core FP32: 2 x 128 lanes x 148 SMs x {sm_max:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {pk_kind})",
-                          peak_measured_ffma_probe=probe_tflops, frac_of_probe=achieved / probe_tflops,
+                          peak_measured_ffma_probe=probe_tflops, frac_of_probe=dom["achieved"] / probe_tflops,
+                          probes_tflops=probes,
+                          frac_of_cell_term_probe=dom["achieved"] / probes["quadrupole_cell_term_loop"],
                           flops_convention=f"{FLOP_NEWTON}/{FLOP_CUT}/{FLOP_QUAD} flops per Newtonian / changeover / quadrupole interaction",
-                          flops_per_launch=float(flops_step), kernel_ms=force_ms, kernel_share_of_step=force_ms / ms_step,
+                          flops_per_launch=dom["flops_per_launch"], kernel_ms=dom["ms"], kernel_share_of_step=dom["share_of_step"],
+                          force_kernels=kern, both_force_kernels=dict(ms=force_ms, achieved=achieved_both, frac=achieved_both / nominal_fp32,
+                                                                      share_of_step=force_ms / ms_step),
                           hbm_peak_gbs=pk.get("hbm_gbs")),
             wall_s_timed_region=t_wall,
         )

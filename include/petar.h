@@ -72,6 +72,8 @@ typedef struct {
     int64_t n_ep_list;      /* sum over groups of EP leaf ranges                                    */
     int64_t n_sp_list;      /* sum over groups of accepted cells                                    */
     int64_t list_entries_used; /* 4-byte arena entries used                                         */
+    int64_t n_epsp_common;  /* part of n_epsp evaluated super-group-wide (cells every i-group of a
+                               super-group accepts; force phase A)             */
 } petar_counts;
 
 /* HOST-only query: bytes of device workspace petar_tree_build needs for N particles.
@@ -172,7 +174,8 @@ int petar_debug_export(petar_tree* t, int what, void* dst, size_t dst_bytes, voi
 #define PETAR_STAGE_WALK 6
 #define PETAR_STAGE_FORCE 7
 #define PETAR_STAGE_NEIGHBOR 8
-#define PETAR_N_STAGES 9
+#define PETAR_STAGE_FORCE_UNITS 9   /* force phase A (k_force_units); PETAR_STAGE_FORCE is phase B (k_force) */
+#define PETAR_N_STAGES 10
 int petar_set_profiling(int on);
 int petar_stage_times(petar_tree* t, float* stage_ms /* HOST */);
 /* Number of kernel launches the library has enqueued since process start (HOST counter).           */
@@ -183,6 +186,15 @@ int64_t petar_launch_count(void);
  * the caller times it with CUDA events to obtain this GPU's CUDA-core FP32 peak.
  * scratch_dev: DEVICE float[1].                                                                      */
 int petar_probe_fp32(int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream);
+/* The same with a choice of instruction stream ("operand bandwidth"):
+ *   mode 0: FFMA whose two other operands are the same for every chain (as petar_probe_fp32);
+ *   mode 1: FFMA with three distinct register operands per instruction;
+ *   mode 2: the force kernel's own quadrupole cell term (rule O8) on register operands, 4 i-particles
+ *           per thread, cells broadcast from shared memory -- *flops_out_host then counts 53 flops per
+ *           interaction (the convention of bench.py), so the result is the rate attainable by this
+ *           instruction mix with no list, staging or tail cost.
+ * Errors: PETAR_EINVAL (mode), PETAR_ECUDA.                                                          */
+int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -11,6 +11,6 @@ from .binding import (  # noqa: F401
     lib, library_path, exported_symbols,
     petar_workspace_bytes, petar_tree_build, petar_long_range_force, petar_neighbor_list,
     petar_tree_status, petar_tree_destroy, petar_strerror, petar_debug_export,
-    petar_set_profiling, petar_stage_times, petar_launch_count, petar_probe_fp32,
+    petar_set_profiling, petar_stage_times, petar_launch_count, petar_probe_fp32, petar_probe_fp32_mode,
     STAGE_NAMES,
 )

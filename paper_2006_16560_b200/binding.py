@@ -11,9 +11,9 @@ _LIB = None
 EXPORTS = [
     "petar_workspace_bytes", "petar_tree_build", "petar_long_range_force", "petar_neighbor_list",
     "petar_tree_status", "petar_tree_destroy", "petar_strerror", "petar_debug_export",
-    "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32",
+    "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32", "petar_probe_fp32_mode",
 ]
-STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor"]
+STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units"]
 DBG = dict(HEADER=0, ROOT=1, KEYS=2, PERM=3, NODE_INT=4, NODE_DBL=5, GROUP_INT=6, GROUP_DBL=7, GROUP_CNT=8,
            LIST_OFFS=9, LISTS=10, GROUP_SUPER=11)
 
@@ -42,7 +42,7 @@ class PetarParams(C.Structure):
 
 class PetarCounts(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("n_groups", "n_nodes", "n_epep", "n_epsp", "n_epep_near", "n_ep_list",
-                                         "n_sp_list", "list_entries_used")]
+                                         "n_sp_list", "list_entries_used", "n_epsp_common")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -84,6 +84,8 @@ def lib():
         L.petar_launch_count.restype = C.c_int64
         L.petar_probe_fp32.restype = C.c_int
         L.petar_probe_fp32.argtypes = [C.c_int64, C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
+        L.petar_probe_fp32_mode.restype = C.c_int
+        L.petar_probe_fp32_mode.argtypes = [C.c_int32, C.c_int64, C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
         _LIB = L
     return _LIB
 
@@ -175,6 +177,15 @@ def petar_probe_fp32(iters: int, scratch, stream=None) -> float:
     rc = lib().petar_probe_fp32(C.c_int64(iters), C.byref(fl), _ptr(scratch), _stream(stream))
     if rc:
         raise PetarError(rc, "petar_probe_fp32")
+    return float(fl.value)
+
+
+def petar_probe_fp32_mode(mode: int, iters: int, scratch, stream=None) -> float:
+    """Probe kernel of the given mode (see petar.h); returns the flops it executes (time it with CUDA events)."""
+    fl = C.c_double(0.0)
+    rc = lib().petar_probe_fp32_mode(C.c_int32(mode), C.c_int64(iters), C.byref(fl), _ptr(scratch), _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_probe_fp32_mode")
     return float(fl.value)
 
 

@@ -173,6 +173,7 @@ extern "C" int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_
         counts->n_epep = (int64_t)hh.n_epep; counts->n_epsp = (int64_t)hh.n_epsp; counts->n_epep_near = (int64_t)hh.n_epep_near;
         counts->n_ep_list = (int64_t)hh.n_ep_list; counts->n_sp_list = (int64_t)hh.n_sp_list;
         counts->list_entries_used = (int64_t)hh.arena_top * PETAR_CHUNK;
+        counts->n_epsp_common = (int64_t)hh.n_epsp_common;
         if (hh.status) return PETAR_ESTATUS;
     }
     return PETAR_OK;

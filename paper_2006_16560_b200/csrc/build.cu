@@ -45,7 +45,7 @@ __global__ void k_reset_header(DevHeader* h) {
         for (int k = 0; k < 3; ++k) { h->bbox[k] = ~0ull; h->bbox[3 + k] = 0ull; }
         h->n_nodes = 0; h->n_groups = 0; h->status = 0; h->arena_top = 0;
         h->group_ticket = 0; h->group_ticket2 = 0; h->group_ticket3 = 0; for (int l = 0; l < PETAR_NSUP; ++l) { h->n_super[l] = 0; h->super_ticket[l] = 0; }
-        h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = 0ull; h->nb_total = 0ull;
+        h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = h->n_epsp_common = 0ull; h->nb_total = 0ull;
         for (int l = 0; l < PETAR_NLEVELS + 2; ++l) h->level_off[l] = 0;
     }
 }

@@ -671,6 +671,8 @@ cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, doub
     if (quad) k_force_units<true><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, (long long)t->N);
     else k_force_units<false><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, (long long)t->N);
     KCHECK(s, "k_force_units");
+    stage_end(t, PETAR_STAGE_FORCE_UNITS, s);
+    stage_begin(t, s);
     // phase B: the groups' own lists
     if (quad) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<true>, FT, 0);
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<false>, FT, 0);
@@ -703,6 +705,68 @@ __global__ void __launch_bounds__(256) k_probe_fp32(float* __restrict__ out, lon
 #pragma unroll
     for (int k = 0; k < 16; ++k) s += v[k];
     if (s == 123.456f) out[0] = s;      // never true in practice; keeps the chains alive
+}
+
+// mode 1: FFMA with three distinct register operands per instruction
+__global__ void __launch_bounds__(256) k_probe_ffma3(float* __restrict__ out, long long iters) {
+    float a[8], b[8], c[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { a[k] = (float)(threadIdx.x + k) * 1e-3f; b[k] = 1.0f + 1e-6f * (float)(threadIdx.x + k); c[k] = 1e-3f * (float)(k + 1); }
+    for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { a[k] = fmaf(b[k], c[k], a[k]); c[k] = fmaf(a[k], b[k], c[k]); }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += a[k] + b[k] + c[k];
+    if (s == 123.456f) out[0] = s;
+}
+// mode 2: the quadrupole cell term of the force kernels on register operands (4 i-particles per thread)
+__global__ void __launch_bounds__(128, 4) k_probe_cell(float* __restrict__ out, long long iters) {
+    __shared__ float4 q0[64], q1[64];
+    __shared__ float2 q2[64];
+    const int t = threadIdx.x;
+    if (t < 64) {
+        q0[t] = make_float4(10.f + t, 20.f - t, 30.f + 0.5f * t, 1.f + 0.01f * t);
+        q1[t] = make_float4(1e-3f * t, -2e-3f * t, 1e-3f * t, 3e-4f * t);
+        q2[t] = make_float2(-1e-4f * t, 2e-4f * t);
+    }
+    __syncthreads();
+    float ix[4], iy[4], iz[4];
+    Acc32 p[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { ix[k] = t * 0.01f + k + out[0]; iy[k] = t * 0.02f - k; iz[k] = 0.5f * k + out[0]; p[k].ax = p[k].ay = p[k].az = p[k].pot = 0.f; }
+    for (long long it = 0; it < iters; ++it) {
+#pragma unroll 1
+        for (int j = 0; j < 64; ++j) {
+            const float4 a = q0[j], b = q1[j]; const float2 c = q2[j];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) cell_term<true>(p[k], a.x - ix[k], a.y - iy[k], a.z - iz[k], a.w, b.x, b.y, b.z, b.w, c.x, c.y);
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) s += p[k].ax + p[k].ay + p[k].az + p[k].pot;
+    if (s == 123.456f) out[0] = s;
+}
+
+extern "C" int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream) {
+    if (mode == 0) return petar_probe_fp32(iters, flops_out_host, scratch_dev, cuda_stream);
+    if (mode != 1 && mode != 2) return PETAR_EINVAL;
+    int dev = 0, sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return PETAR_ECUDA;
+    if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PETAR_ECUDA;
+    if (mode == 1) {
+        const int grid = sm * 8;
+        k_probe_ffma3<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(scratch_dev, (long long)iters);
+        if (flops_out_host) *flops_out_host = 2.0 * 16.0 * (double)iters * 256.0 * (double)grid;
+    } else {
+        const int grid = sm * 4;
+        k_probe_cell<<<grid, 128, 0, (cudaStream_t)cuda_stream>>>(scratch_dev, (long long)iters);
+        if (flops_out_host) *flops_out_host = 53.0 * 4.0 * 64.0 * (double)iters * 128.0 * (double)grid;
+    }
+    petar_count_launch(1);
+    return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;
 }
 
 extern "C" int petar_probe_fp32(int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream) {

@@ -46,7 +46,7 @@ struct DevHeader {
     int unit_fill[PETAR_UNIT_CLASSES];
     int unit_ticket;
     int pad_[2];
-    unsigned long long n_epep, n_epsp, n_epep_near, n_ep_list, n_sp_list;
+    unsigned long long n_epep, n_epsp, n_epep_near, n_ep_list, n_sp_list, n_epsp_common;
     unsigned long long nb_total;
 };
 

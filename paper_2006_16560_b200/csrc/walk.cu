@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
     const double rcx = h->c[0], rcy = h->c[1], rcz = h->c[2];
     if (threadIdx.x < PETAR_NLEVELS) s_lt[threadIdx.x] = (theta > 0.0) ? (float)(ldexp(twoh, -(int)threadIdx.x) / theta) : INFINITY;
     __syncthreads();
-    unsigned long long t_epep = 0, t_epsp = 0, t_near = 0, t_eplist = 0, t_splist = 0;
+    unsigned long long t_epep = 0, t_epsp = 0, t_near = 0, t_eplist = 0, t_splist = 0, t_common = 0;
     for (;;) {
         int g = 0;
         if (lane == 0) g = atomicAdd(&h->group_ticket, 1);
@@ -382,17 +382,18 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
         t_epep += (unsigned long long)n_i * (unsigned long long)n_ep_part;
         t_near += (unsigned long long)n_i * (unsigned long long)n_epn_part;
         t_epsp += (unsigned long long)n_i * (unsigned long long)(n_sp + n_spp + n_common);
+        t_common += (unsigned long long)n_i * (unsigned long long)n_common;
         t_eplist += (unsigned long long)(n_epn + n_epf);
         t_splist += (unsigned long long)(n_sp + n_spp + n_common);
     }
     if (lane == 0) {
         atomicAdd(&h->n_epep, t_epep); atomicAdd(&h->n_epsp, t_epsp); atomicAdd(&h->n_epep_near, t_near);
-        atomicAdd(&h->n_ep_list, t_eplist); atomicAdd(&h->n_sp_list, t_splist);
+        atomicAdd(&h->n_ep_list, t_eplist); atomicAdd(&h->n_sp_list, t_splist); atomicAdd(&h->n_epsp_common, t_common);
     }
 }
 
 __global__ void k_reset_ticket(DevHeader* h, int which) {
-    if (threadIdx.x == 0) { if (which == 0) { h->group_ticket = 0; h->arena_top = 0; for (int l = 0; l < PETAR_NSUP; ++l) { h->n_super[l] = 0; h->super_ticket[l] = 0; } h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = 0ull; } else h->group_ticket3 = 0; }
+    if (threadIdx.x == 0) { if (which == 0) { h->group_ticket = 0; h->arena_top = 0; for (int l = 0; l < PETAR_NSUP; ++l) { h->n_super[l] = 0; h->super_ticket[l] = 0; } h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = h->n_epsp_common = 0ull; } else h->group_ticket3 = 0; }
 }
 
 cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
