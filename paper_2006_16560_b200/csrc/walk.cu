@@ -4,7 +4,9 @@
 #include "internal.cuh"
 
 #define WALK_WARPS 8
+#ifndef WALK_STACK
 #define WALK_STACK 1504          // frontier entries per warp (shared memory)
+#endif
 
 // warp-uniform cursor of one chunked list
 struct ListCursor {
