@@ -33,7 +33,7 @@ sys.path.insert(0, ROOT)
 
 FLOP_NEWTON, FLOP_CUT, FLOP_QUAD = 20, 49, 53      # fixed flops-per-interaction convention
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/), bytes
-TRAFFIC_NCU = {"k_force_units": None, "k_force": None}
+TRAFFIC_NCU = {"k_force_units": 187.1e6, "k_force": 1246.6e6}     # profiles/ncu_r01_phaseAB.md
 
 
 def parse():
