@@ -113,6 +113,47 @@ def neighbors_direct(x, y, z, rs):
     return off, idx[: int(off[-1])]
 
 
+def search_radii(vx, vy, vz, rout, Cr: float, dt: float):
+    """Eq. 24 (PAPER.md:341): r_nb = r_out + C_r |v| dt_L."""
+    vx, vy, vz, rout = map(_f64, (vx, vy, vz, rout))
+    out = np.zeros_like(rout)
+    _lib().ora_search_radii(C.c_int64(rout.shape[0]), _p(vx, C.c_double), _p(vy, C.c_double), _p(vz, C.c_double),
+                            _p(rout, C.c_double), C.c_double(Cr), C.c_double(dt), _p(out, C.c_double))
+    return out
+
+
+def pericentre(d, w, mu: float) -> float:
+    """Kepler pericentre separation of a pair: relative position d[3], relative velocity w[3], mu = G (m_i + m_j)."""
+    L = _lib()
+    L.ora_pericentre.restype = C.c_double
+    L.ora_pericentre.argtypes = [C.c_double] * 7
+    return float(L.ora_pericentre(*[float(v) for v in d], *[float(v) for v in w], float(mu)))
+
+
+def neighbors_orbit_direct(x, y, z, vx, vy, vz, m, rnb, rout, G: float, Cv: float):
+    """O(N^2) definition of the two-stage neighbour criterion (rule O10c).  Rows ascending."""
+    a = list(map(_f64, (x, y, z, vx, vy, vz, m, rnb, rout)))
+    n = a[0].shape[0]
+    off = np.zeros(n + 1, dtype=np.int64)
+    args = [C.c_int64(n)] + [_p(v, C.c_double) for v in a] + [C.c_double(G), C.c_double(Cv), _p(off, C.c_int64)]
+    _lib().ora_neighbors_orbit_direct(*args, None)
+    idx = np.zeros(max(int(off[-1]), 1), dtype=np.int32)
+    _lib().ora_neighbors_orbit_direct(*args, _p(idx, C.c_int32))
+    return off, idx[: int(off[-1])]
+
+
+def clusters(offsets, indices):
+    """Connected components of the neighbour graph: (label int32[N] = smallest member, n_clusters)."""
+    off = np.ascontiguousarray(offsets, dtype=np.int64)
+    idx = np.ascontiguousarray(indices, dtype=np.int32)
+    n = off.shape[0] - 1
+    lab = np.zeros(max(n, 1), dtype=np.int32)
+    L = _lib()
+    L.ora_clusters.restype = C.c_int64
+    nc = int(L.ora_clusters(C.c_int64(n), _p(off, C.c_int64), _p(idx if idx.size else np.zeros(1, np.int32), C.c_int32), _p(lab, C.c_int32)))
+    return lab[:n], nc
+
+
 @dataclass
 class NodeTable:
     level: np.ndarray; begin: np.ndarray; end: np.ndarray; leaf: np.ndarray; nchild: np.ndarray
@@ -202,6 +243,23 @@ class OracleTree:
         _lib().ora_eval_lists(self._h, C.c_int64(gb), C.c_int64(ge), C.c_int64(sp.shape[0]), _p(sp, C.c_int64),
                               C.c_int64(ep.shape[0]), _p(ep, C.c_int64), *[_p(o, C.c_double) for o in out])
         return tuple(out)
+
+    def neighbors_orbit(self, vx, vy, vz, Cv: float, groups=None):
+        """Rule O10: orbit-filtered CSR neighbour list (velocities in the caller's order; rows ascending)."""
+        vx, vy, vz = map(_f64, (vx, vy, vz))
+        off = np.zeros(self.N + 1, dtype=np.int64)
+        if self.N == 0:
+            return off, np.zeros(0, dtype=np.int32)
+        if groups is None:
+            ns, sp = 0, None
+        else:
+            groups = np.ascontiguousarray(groups, dtype=np.int64)
+            ns, sp = groups.shape[0], _p(groups, C.c_int64)
+        a = [self._h, C.c_int64(ns), sp, _p(vx, C.c_double), _p(vy, C.c_double), _p(vz, C.c_double), C.c_double(Cv), _p(off, C.c_int64)]
+        _lib().ora_tree_neighbors_orbit_sel(*a, None)
+        idx = np.zeros(max(int(off[-1]), 1), dtype=np.int32)
+        _lib().ora_tree_neighbors_orbit_sel(*a, _p(idx, C.c_int32))
+        return off, idx[: int(off[-1])]
 
     def neighbors(self, groups=None):
         """CSR neighbour list (rows ascending).  groups: only the particles of these i-groups get rows."""

@@ -20,6 +20,9 @@
  * Pins (tests/test_oracle_*.py): Eq. 19 boundary values, Eq. 18 as a second formula,
  * long+short = Newton (Eq. 7), sum m_i a_i = 0, neighbour symmetry, theta=0 tree ==
  * direct sum, partition invariants of the walk, Plummer potential energy -1/2.
+ * Part (C): Eq. 24 search radii, the Kepler-pericentre filter and the
+ * clustering; pinned by conic closed forms (r_p = a(1-e), a(e-1), impact parameter), r_p <= r,
+ * symmetry, C_V -> infinity == rule O9, tree == O(N^2) definition, components against scipy.
  * Parity UNPINNED (the paper prints nothing to pin them to): interaction counts and
  * force error at theta > 0 (only monotonicity sanity checks).
  *
@@ -593,6 +596,141 @@ void ora_tree_neighbors_sel(const ora_tree *t, int64_t ns, const int64_t *sel, i
         free(l.sp); free(l.ep);
     }
     if (!indices) for (int64_t i = 0; i < N; ++i) offsets[i + 1] += offsets[i];
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* (C) orbit-dependent neighbour criterion and clustering (:325-335)  */
+/* ------------------------------------------------------------------------------------ */
+
+/* Eq. 24: r_nb,i = r_out,i + C_r |v_i| dt_L.  Operation order (rule O10a):
+ * v2 = fma(vz,vz, fma(vy,vy, vx*vx)); r_nb = r_out + (C_r * sqrt(v2)) * dt.                        */
+void ora_search_radii(int64_t N, const double *vx, const double *vy, const double *vz, const double *rout,
+                      double Cr, double dt, double *rnb) {
+    for (int64_t i = 0; i < N; ++i) {
+        double v2 = fma(vz[i], vz[i], fma(vy[i], vy[i], vx[i] * vx[i]));
+        rnb[i] = rout[i] + (Cr * sqrt(v2)) * dt;
+    }
+}
+
+/* Pericentre separation of the two-body Kepler orbit of a pair ("Kepler orbital
+ * pericentre separation r_p,ij"): relative position d, relative velocity w, mu = G (m_i + m_j).
+ * With h = d x w and 2 eps = w^2 - 2 mu / r the conic has r_p = h^2 / (mu + sqrt(mu^2 + 2 eps h^2))
+ * (= p / (1 + e); valid for bound, parabolic and unbound orbits; mu = 0 gives the impact parameter
+ * h / |w|).  Rule O10b, exactly these operations:
+ *   r2 = fma(dz,dz, fma(dy,dy, dx*dx)); v2 likewise; hx = dy*wz - dz*wy; hy = dz*wx - dx*wz;
+ *   hz = dx*wy - dy*wx; h2 = fma(hz,hz, fma(hy,hy, hx*hx)); r = sqrt(r2); r == 0 => r_p = 0;
+ *   e2 = v2 - (2 mu) / r; disc = max(0, fma(e2, h2, mu*mu)); den = mu + sqrt(disc);
+ *   r_p = den > 0 ? h2 / den : r.                                                                  */
+double ora_pericentre(double dx, double dy, double dz, double wx, double wy, double wz, double mu) {
+    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    double v2 = fma(wz, wz, fma(wy, wy, wx * wx));
+    double hx = dy * wz - dz * wy, hy = dz * wx - dx * wz, hz = dx * wy - dy * wx;
+    double h2 = fma(hz, hz, fma(hy, hy, hx * hx));
+    double r = sqrt(r2);
+    if (r == 0.0) return 0.0;
+    double e2 = v2 - (2.0 * mu) / r;
+    double disc = fma(e2, h2, mu * mu);
+    if (!(disc > 0.0)) disc = 0.0;
+    double den = mu + sqrt(disc);
+    return den > 0.0 ? h2 / den : r;
+}
+
+/* Two-stage criterion, rule O10c (reading P20).  j is a neighbour of i iff
+ *   stage (i)  j != i and r_ij < R_s, R_s = max(r_nb,i, r_nb,j) (the symmetric candidate rule O9 with the
+ *              Eq. 24 radii), and
+ *   stage (ii) r_p,ij < C_V min(r_nb,i, r_nb,j) -- the paper's "r_p,ij < C_V r_nb,i" required from both
+ *              sides, so that the relation stays symmetric (the clusters need a symmetric graph); with the
+ *              max instead, r_p <= r_ij < R_s would make the test vacuous for C_V >= 1 --
+ *              OR r_ij < R_o = max(r_out,i, r_out,j): a pair inside its changeover radius has a non-zero
+ *              short-range force now and is always kept.                                            */
+static int orbit_pair(double xi, double yi, double zi, double vxi, double vyi, double vzi, double mi, double ri, double roi,
+                      double xj, double yj, double zj, double vxj, double vyj, double vzj, double mj, double rj, double roj,
+                      double G, double Cv) {
+    double dx = xi - xj, dy = yi - yj, dz = zi - zj;
+    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    double Rs = ri > rj ? ri : rj;
+    if (!(r2 < Rs * Rs)) return 0;
+    double Ro = roi > roj ? roi : roj;
+    if (r2 < Ro * Ro) return 1;
+    double rp = ora_pericentre(dx, dy, dz, vxi - vxj, vyi - vyj, vzi - vzj, G * (mi + mj));
+    double Rm = ri < rj ? ri : rj;
+    return rp < Cv * Rm;
+}
+
+/* O(N^2) definition of the filtered list; two-phase like ora_neighbors_direct; rows ascending.     */
+void ora_neighbors_orbit_direct(int64_t N, const double *x, const double *y, const double *z,
+                                const double *vx, const double *vy, const double *vz, const double *m,
+                                const double *rnb, const double *rout, double G, double Cv, int64_t *offsets, int32_t *indices) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < N; ++i) {
+        int64_t c = 0, o = indices ? offsets[i] : 0;
+        for (int64_t j = 0; j < N; ++j) {
+            if (j == i) continue;
+            if (orbit_pair(x[i], y[i], z[i], vx[i], vy[i], vz[i], m[i], rnb[i], rout[i],
+                           x[j], y[j], z[j], vx[j], vy[j], vz[j], m[j], rnb[j], rout[j], G, Cv)) {
+                if (indices) indices[o + c] = (int32_t)j;
+                ++c;
+            }
+        }
+        if (!indices) offsets[i + 1] = c;
+    }
+    if (!indices) { offsets[0] = 0; for (int64_t i = 0; i < N; ++i) offsets[i + 1] += offsets[i]; }
+}
+
+/* Tree version (rule O10): the candidates are the walk's EP lists of a tree built with r_search = r_nb
+ * (so every pair inside R is an EP pair, rule O7); velocities vx, vy, vz are in the CALLER's order.
+ * Rows hold original indices, ascending.  sel as in ora_tree_neighbors_sel.                         */
+void ora_tree_neighbors_orbit_sel(const ora_tree *t, int64_t ns, const int64_t *sel, const double *vx, const double *vy,
+                                  const double *vz, double Cv, int64_t *offsets, int32_t *indices) {
+    int64_t N = t->N;
+    int64_t ng = sel ? ns : t->n_grp;
+    if (!indices) memset(offsets, 0, (size_t)(N + 1) * 8);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t gs = 0; gs < ng; ++gs) {
+        int64_t g = sel ? sel[gs] : gs;
+        ora_list l; memset(&l, 0, sizeof l); l.collect = 1;
+        visit(t, &t->grp[g], 0, &l);
+        for (int64_t i = t->grp[g].begin; i < t->grp[g].end; ++i) {
+            int32_t oi = t->perm[i];
+            int64_t c = 0, o = indices ? offsets[oi] : 0;
+            for (int64_t r = 0; r < l.n_ep_ranges; ++r)
+                for (int64_t j = l.ep[3 * r]; j < l.ep[3 * r + 1]; ++j) {
+                    if (j == i) continue;
+                    int32_t oj = t->perm[j];
+                    if (orbit_pair(t->x[i], t->y[i], t->z[i], vx[oi], vy[oi], vz[oi], t->m[i], t->rs[i], t->rout[i],
+                                   t->x[j], t->y[j], t->z[j], vx[oj], vy[oj], vz[oj], t->m[j], t->rs[j], t->rout[j], t->p.G, Cv)) {
+                        if (indices) indices[o + c] = oj;
+                        ++c;
+                    }
+                }
+            if (indices) qsort(indices + o, (size_t)c, 4, cmp_i32);
+            else offsets[oi + 1] = c;
+        }
+        free(l.sp); free(l.ep);
+    }
+    if (!indices) for (int64_t i = 0; i < N; ++i) offsets[i + 1] += offsets[i];
+}
+
+/* Clustering: "any member in one cluster have all its neighbours inside the same
+ * cluster" -- the clusters are the connected components of the (symmetric) neighbour graph.  Plain
+ * union-find with path halving; label[i] = smallest index of i's component (a particle without
+ * neighbours is its own cluster).  Returns the number of clusters.                                  */
+static int64_t uf_find(int64_t *parent, int64_t a) {
+    while (parent[a] != a) { parent[a] = parent[parent[a]]; a = parent[a]; }
+    return a;
+}
+int64_t ora_clusters(int64_t N, const int64_t *offsets, const int32_t *indices, int32_t *label) {
+    int64_t *parent = (int64_t *)xmalloc((size_t)N * 8);
+    for (int64_t i = 0; i < N; ++i) parent[i] = i;
+    for (int64_t i = 0; i < N; ++i)
+        for (int64_t e = offsets[i]; e < offsets[i + 1]; ++e) {
+            int64_t a = uf_find(parent, i), b = uf_find(parent, indices[e]);
+            if (a < b) parent[b] = a; else if (b < a) parent[a] = b;     /* the smaller index stays root */
+        }
+    int64_t nc = 0;
+    for (int64_t i = 0; i < N; ++i) { int64_t r = uf_find(parent, i); label[i] = (int32_t)r; nc += (r == i); }
+    free(parent);
+    return nc;
 }
 
 int ora_num_threads(void) {

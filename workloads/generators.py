@@ -43,6 +43,10 @@ class Workload:
     n_group_limit: int = 64
     G: float = 1.0
     meta: dict = field(default_factory=dict)
+    vx: np.ndarray | None = None      # velocities (make_workload(velocities=True)); None on the force path
+    vy: np.ndarray | None = None
+    vz: np.ndarray | None = None
+    dt_L: float | None = None         # tree time step that goes with r_out_ref (Eq. 41)
 
     @property
     def N(self) -> int:
@@ -117,9 +121,35 @@ def _random_rotations(n: int, rng: np.random.Generator) -> np.ndarray:
     return R
 
 
+def plummer_speeds(r: np.ndarray, rng: np.random.Generator, a: float = PLUMMER_A) -> np.ndarray:
+    """Speeds of a Plummer model (G = M = 1) at radii r: v = q v_esc(r), q drawn by rejection from
+    g(q) = q^2 (1 - q^2)^(7/2) (Aarseth, Henon & Wielen 1974)."""
+    n = r.shape[0]
+    q = np.empty(n)
+    todo = np.arange(n)
+    while todo.size:
+        xq = rng.random(todo.size)
+        yq = 0.1 * rng.random(todo.size)
+        ok = yq < xq * xq * (1.0 - xq * xq) ** 3.5
+        q[todo[ok]] = xq[ok]
+        todo = todo[~ok]
+    vesc = np.sqrt(2.0 / a) * (1.0 + (r / a) ** 2) ** -0.25
+    return q * vesc
+
+
+def _isotropic(speed: np.ndarray, rng: np.random.Generator) -> np.ndarray:
+    n = speed.shape[0]
+    cos_t = rng.uniform(-1.0, 1.0, n)
+    sin_t = np.sqrt(np.maximum(0.0, 1.0 - cos_t * cos_t))
+    phi = rng.uniform(0.0, 2.0 * np.pi, n)
+    return np.stack([speed * sin_t * np.cos(phi), speed * sin_t * np.sin(phi), speed * cos_t], axis=1)
+
+
 def _place_with_binaries(m: np.ndarray, n_pairs: int, a_lo: float, a_hi: float,
-                         rng: np.random.Generator) -> np.ndarray:
-    """Positions for stars of mass m where stars (2k, 2k+1), k < n_pairs, form binaries."""
+                         rng: np.random.Generator, vel_rng: np.random.Generator | None = None):
+    """Positions for stars of mass m where stars (2k, 2k+1), k < n_pairs, form binaries.
+    With vel_rng: returns (pos, vel); the velocities use their own generator and the orbital elements
+    already drawn, so the positions are the same with and without them."""
     n = m.shape[0]
     n_single = n - 2 * n_pairs
     cm = plummer_positions(n_pairs + n_single, rng)
@@ -131,14 +161,30 @@ def _place_with_binaries(m: np.ndarray, n_pairs: int, a_lo: float, a_hi: float,
         rel = np.zeros((n_pairs, 3))
         rel[:, 0] = semi * (np.cos(E) - ecc)                       # Eq. 32
         rel[:, 1] = semi * np.sqrt(1.0 - ecc * ecc) * np.sin(E)
-        rel = np.einsum("nij,nj->ni", _random_rotations(n_pairs, rng), rel)
+        rot = _random_rotations(n_pairs, rng)
+        rel = np.einsum("nij,nj->ni", rot, rel)
         m1 = m[0:2 * n_pairs:2]
         m2 = m[1:2 * n_pairs:2]
         mt = m1 + m2
         pos[0:2 * n_pairs:2] = cm[:n_pairs] - (m2 / mt)[:, None] * rel   # Eq. 33
         pos[1:2 * n_pairs:2] = cm[:n_pairs] + (m1 / mt)[:, None] * rel
     pos[2 * n_pairs:] = cm[n_pairs:]
-    return pos
+    if vel_rng is None:
+        return pos
+    vcm = _isotropic(plummer_speeds(np.linalg.norm(cm, axis=1), vel_rng), vel_rng)
+    vel = np.empty((n, 3))
+    if n_pairs:
+        # Kepler relative velocity in the orbital plane (G = 1), rotated like the relative position
+        nmean = np.sqrt(mt / semi ** 3)
+        fac = semi * nmean / (1.0 - ecc * np.cos(E))
+        relv = np.zeros((n_pairs, 3))
+        relv[:, 0] = -fac * np.sin(E)
+        relv[:, 1] = fac * np.sqrt(1.0 - ecc * ecc) * np.cos(E)
+        relv = np.einsum("nij,nj->ni", rot, relv)
+        vel[0:2 * n_pairs:2] = vcm[:n_pairs] - (m2 / mt)[:, None] * relv
+        vel[1:2 * n_pairs:2] = vcm[:n_pairs] + (m1 / mt)[:, None] * relv
+    vel[2 * n_pairs:] = vcm[n_pairs:]
+    return pos, vel
 
 
 # BASELINE.json configs 1..5 (index k-1); theta of config 4 is swept by the caller.
@@ -151,12 +197,22 @@ CONFIGS = {
 }
 
 
+def tree_time_step(r_out_ref: float) -> float:
+    """dt_L that goes with r_out_ref: Eq. 41 r_out = 10 dt_L sigma_1D with sigma_1D = 0.409
+    (Henon units), rounded to a power of two as in Table 3 (0.004 <-> 1/1024 for N1m, :666)."""
+    return float(2.0 ** np.round(np.log2(r_out_ref / 4.09)))
+
+
 def make_workload(config: int, N: int | None = None, seed: int | None = None, theta: float | None = None,
-                  uniform_radii: bool = False) -> Workload:
-    """Build BASELINE.json config `config` (1..5); N overrides the size (same recipe, for tests)."""
+                  uniform_radii: bool = False, velocities: bool = False) -> Workload:
+    """Build BASELINE.json config `config` (1..5); N overrides the size (same recipe, for tests).
+    velocities=True adds Plummer velocities (+ binary orbital motion) from a separate generator."""
     c = dict(CONFIGS[config])
     n = int(N if N is not None else c["N"])
-    rng = np.random.Generator(np.random.PCG64(SEED_BASE + config if seed is None else seed))
+    base_seed = SEED_BASE + config if seed is None else seed
+    rng = np.random.Generator(np.random.PCG64(base_seed))
+    vel_rng = np.random.Generator(np.random.PCG64([base_seed, 24])) if velocities else None
+    vel = None
     kind = c["masses"]
     if kind == "equal":
         m = np.full(n, 1.0 / n)
@@ -173,16 +229,24 @@ def make_workload(config: int, N: int | None = None, seed: int | None = None, th
         pos = np.empty((n, 3))
         pos[0] = 0.0
         pos[1:] = plummer_positions(n - 1, rng)
+        if velocities:
+            vel = np.zeros((n, 3))
+            vel[1:] = _isotropic(plummer_speeds(np.linalg.norm(pos[1:], axis=1), vel_rng), vel_rng)
     else:
         if n_pairs:
             perm = rng.permutation(n)       # "shuffle stars, pair consecutive ones"
             m = m[perm]
         a_lo, a_hi = c["a_range"] if c["a_range"] else (1.0, 1.0)
-        pos = _place_with_binaries(m, n_pairs, a_lo, a_hi, rng)
+        if velocities:
+            pos, vel = _place_with_binaries(m, n_pairs, a_lo, a_hi, rng, vel_rng)
+        else:
+            pos = _place_with_binaries(m, n_pairs, a_lo, a_hi, rng)
         # final shuffle so that the input order carries no structure
         perm2 = rng.permutation(n)
         pos = pos[perm2]
         m = m[perm2]
+        if vel is not None:
+            vel = vel[perm2]
     r_out_ref = c["r_out_ref"]
     r_out = np.full(n, r_out_ref) if uniform_radii else changeover_radii(m, r_out_ref)
     return Workload(
@@ -191,4 +255,8 @@ def make_workload(config: int, N: int | None = None, seed: int | None = None, th
         m=np.ascontiguousarray(m), r_out=np.ascontiguousarray(r_out),
         theta=float(c["theta"] if theta is None else theta), multipole=c["multipole"], r_out_ref=r_out_ref,
         meta=dict(config=config, n_pairs=n_pairs, masses=kind),
+        vx=None if vel is None else np.ascontiguousarray(vel[:, 0]),
+        vy=None if vel is None else np.ascontiguousarray(vel[:, 1]),
+        vz=None if vel is None else np.ascontiguousarray(vel[:, 2]),
+        dt_L=tree_time_step(r_out_ref),
     )
