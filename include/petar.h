@@ -119,6 +119,40 @@ int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_y, double* 
 int petar_neighbor_list(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity,
                         int32_t* status_dev, void* cuda_stream);
 
+/* ---- the consumers of the neighbour search --------------------------------
+ * Eq. 24: r_search_out[i] = r_out[i] + C_r |v_i| dt_L  (C_r = 3 in the paper); the result
+ * is what petar_tree_build takes as r_search.  All arrays DEVICE fp64[N]; r_search_out may not alias.
+ * Errors: PETAR_EINVAL (N < 0, C_r < 0, dt_L < 0, NULL), PETAR_ECUDA.                                */
+int petar_search_radii(const double* vx, const double* vy, const double* vz, const double* r_out,
+                       double C_r, double dt_L, int64_t N, double* r_search_out, void* cuda_stream);
+
+/* Orbit-dependent two-stage neighbour criterion (DESIGN.md rule O10, reading P20) on a
+ * tree built with r_search = the Eq. 24 radii:  j is a neighbour of i iff j != i,
+ *   (i)  r_ij < max(r_search,i, r_search,j)                       (the candidates of rule O9) and
+ *   (ii) r_ij < max(r_out,i, r_out,j)  or  r_p,ij < C_V min(r_search,i, r_search,j),
+ * r_p,ij = pericentre separation of the pair's two-body Kepler orbit, mu = G (m_i + m_j), fp64.
+ *   vx, vy, vz : DEVICE fp64[N], caller's particle order.   C_V >= 0 (1.5 in the paper).
+ * Output, two-phase protocol, ownership and errors as petar_neighbor_list.                          */
+int petar_neighbor_list_orbit(petar_tree* t, const double* vx, const double* vy, const double* vz, double C_V,
+                              int64_t* offsets, int32_t* indices, int64_t capacity, int32_t* status_dev,
+                              void* cuda_stream);
+
+/* Clustering: connected components of a symmetric neighbour list in CSR form.
+ *   offsets int64[N+1], indices int32[offsets[N]] : DEVICE, as written by petar_neighbor_list(_orbit).
+ *   label            : DEVICE int32[N]; label[i] = smallest particle index of i's cluster.
+ *   n_clusters_dev   : DEVICE int64[1] or NULL.
+ *   cluster_offsets  : DEVICE int64[N+1] or NULL.  If given, the clusters are numbered by ascending label,
+ *                      cluster c holds members[cluster_offsets[c] .. cluster_offsets[c+1]) in ascending
+ *                      particle index, cluster_offsets[n_clusters] = N (entries beyond are untouched).
+ *   members          : DEVICE int32[N] or NULL (needs cluster_offsets).
+ *   workspace        : DEVICE, 256-byte aligned, >= petar_clusters_workspace_bytes(N); only read when
+ *                      cluster_offsets is given.
+ * No host synchronisation.  Errors: PETAR_EINVAL, PETAR_EWORKSPACE, PETAR_ECUDA.                     */
+size_t petar_clusters_workspace_bytes(int64_t N);
+int petar_clusters(const int64_t* offsets, const int32_t* indices, int64_t N, int32_t* label,
+                   int64_t* n_clusters_dev, int64_t* cluster_offsets, int32_t* members,
+                   void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Synchronises the stream and returns the device status word (PETAR_ST_* bits) in *status_host.    */
 int petar_tree_status(petar_tree* t, int32_t* status_host /* HOST */, void* cuda_stream);
 

@@ -12,6 +12,7 @@ EXPORTS = [
     "petar_workspace_bytes", "petar_tree_build", "petar_long_range_force", "petar_neighbor_list",
     "petar_tree_status", "petar_tree_destroy", "petar_strerror", "petar_debug_export",
     "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32", "petar_probe_fp32_mode",
+    "petar_search_radii", "petar_neighbor_list_orbit", "petar_clusters_workspace_bytes", "petar_clusters",
 ]
 STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units"]
 DBG = dict(HEADER=0, ROOT=1, KEYS=2, PERM=3, NODE_INT=4, NODE_DBL=5, GROUP_INT=6, GROUP_DBL=7, GROUP_CNT=8,
@@ -69,6 +70,15 @@ def lib():
         L.petar_long_range_force.argtypes = [C.c_void_p] * 5 + [C.POINTER(PetarCounts), C.c_void_p]
         L.petar_neighbor_list.restype = C.c_int
         L.petar_neighbor_list.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+        L.petar_search_radii.restype = C.c_int
+        L.petar_search_radii.argtypes = [C.c_void_p] * 4 + [C.c_double, C.c_double, C.c_int64, C.c_void_p, C.c_void_p]
+        L.petar_neighbor_list_orbit.restype = C.c_int
+        L.petar_neighbor_list_orbit.argtypes = [C.c_void_p] * 4 + [C.c_double, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+        L.petar_clusters_workspace_bytes.restype = C.c_size_t
+        L.petar_clusters_workspace_bytes.argtypes = [C.c_int64]
+        L.petar_clusters.restype = C.c_int
+        L.petar_clusters.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                     C.c_size_t, C.c_void_p]
         L.petar_tree_status.restype = C.c_int
         L.petar_tree_status.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.c_void_p]
         L.petar_tree_destroy.restype = C.c_int
@@ -139,6 +149,32 @@ def petar_neighbor_list(tree, offsets, indices, capacity, status_dev=None, strea
     rc = lib().petar_neighbor_list(tree, _ptr(offsets), _ptr(indices), C.c_int64(capacity), _ptr(status_dev), _stream(stream))
     if rc:
         raise PetarError(rc, "petar_neighbor_list")
+
+
+def petar_search_radii(vx, vy, vz, r_out, C_r: float, dt_L: float, N: int, r_search_out, stream=None) -> None:
+    rc = lib().petar_search_radii(_ptr(vx), _ptr(vy), _ptr(vz), _ptr(r_out), C.c_double(C_r), C.c_double(dt_L), C.c_int64(N),
+                                  _ptr(r_search_out), _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_search_radii")
+
+
+def petar_neighbor_list_orbit(tree, vx, vy, vz, C_V: float, offsets, indices, capacity, status_dev=None, stream=None) -> None:
+    rc = lib().petar_neighbor_list_orbit(tree, _ptr(vx), _ptr(vy), _ptr(vz), C.c_double(C_V), _ptr(offsets), _ptr(indices),
+                                         C.c_int64(capacity), _ptr(status_dev), _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_neighbor_list_orbit")
+
+
+def petar_clusters_workspace_bytes(N: int) -> int:
+    return int(lib().petar_clusters_workspace_bytes(C.c_int64(N)))
+
+
+def petar_clusters(offsets, indices, N: int, label, n_clusters_dev=None, cluster_offsets=None, members=None, workspace=None,
+                   stream=None) -> None:
+    rc = lib().petar_clusters(_ptr(offsets), _ptr(indices), C.c_int64(N), _ptr(label), _ptr(n_clusters_dev), _ptr(cluster_offsets),
+                              _ptr(members), _ptr(workspace), C.c_size_t(0 if workspace is None else workspace.numel()), _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_clusters")
 
 
 def petar_tree_status(tree, stream=None) -> int:
@@ -241,6 +277,30 @@ class Tree:
             self.indices = t.empty(max(total, 1), dtype=t.int32, device=self.device)
         petar_neighbor_list(self.handle, self.offsets, self.indices, self.indices.numel(), self.nb_status, stream)
         return self.offsets, self.indices[:total]
+
+    def neighbors_orbit(self, vx, vy, vz, C_V: float = 1.5, stream=None):
+        """Two-phase output of the orbit-dependent criterion (velocities: CUDA fp64 tensors, caller's order)."""
+        t = self.torch
+        petar_neighbor_list_orbit(self.handle, vx, vy, vz, C_V, self.offsets, None, 0, None, stream)
+        total = int(self.offsets[-1].item()) if self.N else 0
+        if self.indices is None or self.indices.numel() < max(total, 1):
+            self.indices = t.empty(max(total, 1), dtype=t.int32, device=self.device)
+        petar_neighbor_list_orbit(self.handle, vx, vy, vz, C_V, self.offsets, self.indices, self.indices.numel(), self.nb_status, stream)
+        return self.offsets, self.indices[:total]
+
+    def clusters(self, offsets, indices, members: bool = True, stream=None):
+        """Connected components of a neighbour list: (label, n_clusters tensor, cluster_offsets, members)."""
+        t = self.torch
+        n = self.N
+        label = t.empty(max(n, 1), dtype=t.int32, device=self.device)
+        ncl = t.zeros(1, dtype=t.int64, device=self.device)
+        coff = mem = ws = None
+        if members:
+            coff = t.zeros(n + 1, dtype=t.int64, device=self.device)
+            mem = t.empty(max(n, 1), dtype=t.int32, device=self.device)
+            ws = t.empty(petar_clusters_workspace_bytes(n), dtype=t.uint8, device=self.device)
+        petar_clusters(offsets, indices, n, label, ncl, coff, mem, ws, stream)
+        return label[:n], ncl, coff, None if mem is None else mem[:n]
 
     def export(self, name: str):
         """Test hook: returns a torch tensor with the intermediate `name` (see petar_debug_export)."""

@@ -72,6 +72,7 @@ static size_t carve(Workspace* w, char* base, int64_t N, const petar_params* p) 
     W->sort_blk = (unsigned*)take((size_t)256 * nblk * 4);
     W->xs = (double*)take(n * 8); W->ys = (double*)take(n * 8); W->zs = (double*)take(n * 8);
     W->ms = (double*)take(n * 8); W->routs = (double*)take(n * 8); W->rss = (double*)take(n * 8);
+    W->vxs = (double*)take(n * 8); W->vys = (double*)take(n * 8); W->vzs = (double*)take(n * 8);
     W->pa = (float4*)take(n * 16); W->pb = (float4*)take(n * 16);
     W->D = (signed char*)take(n + 1); W->depth = (signed char*)take(n); W->glevel = (signed char*)take(n);
     W->gflag = (int*)take((2 * (n + 1)) * 4);
@@ -193,6 +194,51 @@ extern "C" int petar_neighbor_list(petar_tree* t, int64_t* offsets, int32_t* ind
     rc = ensure_walk(t, s);
     if (rc) return rc;
     CK(launch_neighbors(t, offsets, indices, capacity, status_dev, s));
+    return PETAR_OK;
+}
+
+extern "C" int petar_search_radii(const double* vx, const double* vy, const double* vz, const double* r_out, double C_r, double dt_L,
+                                  int64_t N, double* r_search_out, void* cuda_stream) {
+    if (N < 0 || !(C_r >= 0.0) || !(dt_L >= 0.0)) return PETAR_EINVAL;
+    if (N == 0) return PETAR_OK;
+    if (!vx || !vy || !vz || !r_out || !r_search_out) return PETAR_EINVAL;
+    CK(launch_search_radii(vx, vy, vz, r_out, C_r, dt_L, N, r_search_out, (cudaStream_t)cuda_stream));
+    return PETAR_OK;
+}
+
+extern "C" int petar_neighbor_list_orbit(petar_tree* t, const double* vx, const double* vy, const double* vz, double C_V,
+                                         int64_t* offsets, int32_t* indices, int64_t capacity, int32_t* status_dev, void* cuda_stream) {
+    int rc = check_tree(t);
+    if (rc) return rc;
+    if (!offsets || capacity < 0 || !(C_V >= 0.0)) return PETAR_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (t->N == 0) {
+        CK(cudaMemsetAsync(offsets, 0, 8, s));
+        if (status_dev) CK(cudaMemsetAsync(status_dev, 0, 4, s));
+        return PETAR_OK;
+    }
+    if (!vx || !vy || !vz) return PETAR_EINVAL;
+    rc = ensure_walk(t, s);
+    if (rc) return rc;
+    CK(launch_neighbors(t, offsets, indices, capacity, status_dev, s, vx, vy, vz, C_V));
+    return PETAR_OK;
+}
+
+extern "C" size_t petar_clusters_workspace_bytes(int64_t N) { return N < 0 ? 0 : clusters_workspace_bytes(N); }
+
+extern "C" int petar_clusters(const int64_t* offsets, const int32_t* indices, int64_t N, int32_t* label, int64_t* n_clusters_dev,
+                              int64_t* cluster_offsets, int32_t* members, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (N < 0 || N > 2000000000ll) return PETAR_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (N == 0) {
+        if (n_clusters_dev) CK(cudaMemsetAsync(n_clusters_dev, 0, 8, s));
+        if (cluster_offsets) CK(cudaMemsetAsync(cluster_offsets, 0, 8, s));
+        return PETAR_OK;
+    }
+    if (!offsets || !label) return PETAR_EINVAL;
+    if (members && !cluster_offsets) return PETAR_EINVAL;
+    if (cluster_offsets && (!workspace || workspace_bytes < clusters_workspace_bytes(N) || ((uintptr_t)workspace & 255u))) return PETAR_EWORKSPACE;
+    CK(launch_clusters((const long long*)offsets, indices, N, label, (long long*)n_clusters_dev, (long long*)cluster_offsets, members, workspace, s));
     return PETAR_OK;
 }
 

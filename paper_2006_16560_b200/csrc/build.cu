@@ -672,6 +672,46 @@ cudaError_t launch_scan_i32_to_i64(const int* in, long long* out, long long n, l
 // ------------------------------------------------------------------------------------------------
 // host-side launch sequences
 // ------------------------------------------------------------------------------------------------
+int radix_sort_blocks(long long n) { return cdiv(n, SORT_TILE); }
+
+cudaError_t launch_radix_sort(unsigned long long* key, unsigned long long* key_alt, unsigned* idx, unsigned* idx_alt,
+                              unsigned* hist, unsigned* blk, long long n, int npass, cudaStream_t s) {
+    const int nblk = cdiv(n, SORT_TILE);
+    cudaError_t e = cudaMemsetAsync(hist, 0, (size_t)npass * 256 * sizeof(unsigned), s);
+    if (e != cudaSuccess) return e;
+    unsigned long long *kin = key, *kout = key_alt;
+    unsigned *vin = idx, *vout = idx_alt;
+    for (int pass = 0; pass < npass; ++pass) {
+        int shift = 8 * pass;
+        k_sort_count<<<nblk, SORT_THREADS, 0, s>>>(kin, n, shift, blk, nblk, hist + 256 * pass);
+        KCHECK(s, "k_sort_count");
+        k_sort_scan<<<256, 256, 0, s>>>(blk, nblk, hist + 256 * pass);
+        KCHECK(s, "k_sort_scan");
+        k_sort_scatter<<<nblk, SORT_THREADS, 0, s>>>(kin, vin, kout, vout, blk, nblk, n, shift);
+        KCHECK(s, "k_sort_scatter");
+        unsigned long long* tk = kin; kin = kout; kout = tk;
+        unsigned* tv = vin; vin = vout; vout = tv;
+    }
+    petar_count_launch(3 * npass);
+    return cudaGetLastError();
+}
+
+// Eq. 24, rule O10a: r_nb = r_out + (C_r sqrt(v2)) dt, v2 = fma(vz,vz, fma(vy,vy, vx*vx))
+__global__ void __launch_bounds__(256) k_search_radii(const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
+                                                      const double* __restrict__ rout, double Cr, double dt, long long n, double* __restrict__ out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double v2 = fma(vz[i], vz[i], fma(vy[i], vy[i], vx[i] * vx[i]));
+    out[i] = rout[i] + (Cr * sqrt(v2)) * dt;
+}
+cudaError_t launch_search_radii(const double* vx, const double* vy, const double* vz, const double* r_out, double Cr, double dt,
+                                long long n, double* out, cudaStream_t s) {
+    if (n > 0) k_search_radii<<<cdiv(n, 256), 256, 0, s>>>(vx, vy, vz, r_out, Cr, dt, n, out);
+    KCHECK(s, "k_search_radii");
+    petar_count_launch(1);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s) {
     Workspace& w = t->w;
     const long long n = t->N;
@@ -689,25 +729,10 @@ cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s) {
     stage_end(t, PETAR_STAGE_BBOX_KEYS, s);
 
     stage_begin(t, s);
-    const int nblk = cdiv(n, SORT_TILE);
     {
-        cudaError_t e = cudaMemsetAsync(w.sort_hist, 0, 8 * 256 * sizeof(unsigned), s);
+        cudaError_t e = launch_radix_sort(w.key, w.key_alt, w.idx, w.idx_alt, w.sort_hist, w.sort_blk, n, 8, s);
         if (e != cudaSuccess) return e;
     }
-    unsigned long long *kin = w.key, *kout = w.key_alt;
-    unsigned *vin = w.idx, *vout = w.idx_alt;
-    for (int pass = 0; pass < 8; ++pass) {
-        int shift = 8 * pass;
-        k_sort_count<<<nblk, SORT_THREADS, 0, s>>>(kin, n, shift, w.sort_blk, nblk, w.sort_hist + 256 * pass);
-        KCHECK(s, "k_sort_count");
-        k_sort_scan<<<256, 256, 0, s>>>(w.sort_blk, nblk, w.sort_hist + 256 * pass);
-        KCHECK(s, "k_sort_scan");
-        k_sort_scatter<<<nblk, SORT_THREADS, 0, s>>>(kin, vin, kout, vout, w.sort_blk, nblk, n, shift);
-        KCHECK(s, "k_sort_scatter");
-        unsigned long long* tk = kin; kin = kout; kout = tk;
-        unsigned* tv = vin; vin = vout; vout = tv;
-    }
-    petar_count_launch(24);
     // 8 passes: the sorted data is back in (key, idx)
     stage_end(t, PETAR_STAGE_SORT, s);
 

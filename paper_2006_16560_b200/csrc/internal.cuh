@@ -100,6 +100,7 @@ struct Workspace {
     unsigned int *sort_blk;        // [256][nblk]
     // sorted particle data
     double *xs, *ys, *zs, *ms, *routs, *rss;
+    double *vxs, *vys, *vzs;       // sorted velocities (petar_neighbor_list_orbit only)
     float4 *pa, *pb;               // (xh,yh,zh,m) , (xl,yl,zl,1/r_out)
     signed char *D;                // [N+1] shared leading octal digits of keys i-1, i
     signed char *depth;            // [N] leaf level of particle i
@@ -143,8 +144,19 @@ cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s);
 cudaError_t launch_tree(petar_tree* t, cudaStream_t s);
 cudaError_t launch_walk(petar_tree* t, cudaStream_t s);
 cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s);
+// vx != nullptr: the orbit-dependent two-stage criterion (rule O10) with velocities in the caller's order
 cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity,
-                             int32_t* status_dev, cudaStream_t s);
+                             int32_t* status_dev, cudaStream_t s, const double* vx = nullptr, const double* vy = nullptr,
+                             const double* vz = nullptr, double Cv = 0.0);
+// stable LSD radix sort of (key, idx) pairs, 8 bits per pass, npass even: the result is back in (key, idx)
+cudaError_t launch_radix_sort(unsigned long long* key, unsigned long long* key_alt, unsigned* idx, unsigned* idx_alt,
+                              unsigned* hist /* [npass][256] */, unsigned* blk /* [256][nblk] */, long long n, int npass, cudaStream_t s);
+int radix_sort_blocks(long long n);
+cudaError_t launch_search_radii(const double* vx, const double* vy, const double* vz, const double* r_out, double Cr, double dt,
+                                long long n, double* out, cudaStream_t s);
+cudaError_t launch_clusters(const long long* offsets, const int* indices, long long n, int* label, long long* n_clusters_dev,
+                            long long* cluster_offsets, int* members, void* workspace, cudaStream_t s);
+size_t clusters_workspace_bytes(long long n);
 cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_bytes, cudaStream_t s);
 // device-wide exclusive scan: out[i] = sum_{j<i} in[j], out has n+1 entries (out[n] = total)
 cudaError_t launch_scan_i32(const int* in, int* out, int n, int* tmp, cudaStream_t s);

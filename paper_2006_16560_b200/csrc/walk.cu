@@ -431,12 +431,32 @@ cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
 // (a leaf that is not near has every pair at r >= R_ij, rule O7), fp64 test of rule O9.
 // Pass 1 counts into cnt[original index]; pass 2 (after the scan) fills.
 // ------------------------------------------------------------------------------------------------
-template <bool FILL>
+// Rule O10b: pericentre separation of the pair's Kepler orbit, exactly the operation order of
+// DESIGN.md (this file is compiled with -fmad=false; fma only where written).
+__device__ __forceinline__ double pericentre(double dx, double dy, double dz, double r2, double wx, double wy, double wz, double mu) {
+    const double v2 = fma(wz, wz, fma(wy, wy, wx * wx));
+    const double hx = dy * wz - dz * wy, hy = dz * wx - dx * wz, hz = dx * wy - dy * wx;
+    const double h2 = fma(hz, hz, fma(hy, hy, hx * hx));
+    const double r = sqrt(r2);
+    if (r == 0.0) return 0.0;
+    const double e2 = v2 - (2.0 * mu) / r;
+    double disc = fma(e2, h2, mu * mu);
+    if (!(disc > 0.0)) disc = 0.0;
+    const double den = mu + sqrt(disc);
+    return den > 0.0 ? h2 / den : r;
+}
+
+// ORBIT: the two-stage criterion of PAPER.md:346-348 (rule O10c): candidate as in O9 with the Eq. 24 radii,
+// kept iff the pair is inside its changeover radius or r_p < C_V min(r_nb,i, r_nb,j).
+struct OrbitArgs { const double *vxs, *vys, *vzs, *ms, *routs; double G, Cv; };
+
+template <bool FILL, bool ORBIT>
 __global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
                                                    const unsigned* __restrict__ perm,
                                                    const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
                                                    const double* __restrict__ rss, int* __restrict__ cnt,
-                                                   const long long* __restrict__ offsets, int* __restrict__ indices, long long capacity) {
+                                                   const long long* __restrict__ offsets, int* __restrict__ indices, long long capacity,
+                                                   const OrbitArgs oa) {
     const int lane = threadIdx.x & 31;
     const int ng = h->n_groups;
     for (;;) {
@@ -449,9 +469,13 @@ __global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, co
             const int i = ib + lane;
             const bool vi = i < gr.end;
             double xi = 0, yi = 0, zi = 0, ri = 0;
+            double vxi = 0, vyi = 0, vzi = 0, mi = 0, roi = 0;
             unsigned oi = 0;
             long long o = 0;
-            if (vi) { xi = xs[i]; yi = ys[i]; zi = zs[i]; ri = rss[i]; oi = perm[i]; if (FILL) o = offsets[oi]; }
+            if (vi) {
+                xi = xs[i]; yi = ys[i]; zi = zs[i]; ri = rss[i]; oi = perm[i]; if (FILL) o = offsets[oi];
+                if (ORBIT) { vxi = oa.vxs[i]; vyi = oa.vys[i]; vzi = oa.vzs[i]; mi = oa.ms[i]; roi = oa.routs[i]; }
+            }
             int c = 0;
             int chunk = gr.head_epn;
             int remaining = gr.n_epn * 2;       // entries
@@ -465,7 +489,15 @@ __global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, co
                         double dx = xi - xj, dy = yi - yj, dz = zi - zj;
                         double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
                         double R = fmax(ri, rj);
-                        if (vi && j != i && r2 < R * R) {
+                        bool keep = vi && j != i && r2 < R * R;
+                        if (ORBIT && keep) {
+                            const double Ro = fmax(roi, oa.routs[j]);
+                            if (!(r2 < Ro * Ro)) {
+                                const double rp = pericentre(dx, dy, dz, r2, vxi - oa.vxs[j], vyi - oa.vys[j], vzi - oa.vzs[j], oa.G * (mi + oa.ms[j]));
+                                keep = rp < oa.Cv * fmin(ri, rj);
+                            }
+                        }
+                        if (keep) {
                             if (FILL) { if (o + c < capacity) indices[o + c] = (int)perm[j]; }
                             ++c;
                         }
@@ -479,6 +511,15 @@ __global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, co
     }
 }
 
+__global__ void __launch_bounds__(256) k_gather_vel(const unsigned* __restrict__ perm, long long n, const double* __restrict__ vx,
+                                                    const double* __restrict__ vy, const double* __restrict__ vz,
+                                                    double* __restrict__ vxs, double* __restrict__ vys, double* __restrict__ vzs) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const unsigned o = perm[i];
+    vxs[i] = vx[o]; vys[i] = vy[o]; vzs[i] = vz[o];
+}
+
 __global__ void k_nb_status(const long long* __restrict__ offsets, long long n, long long capacity, int* __restrict__ status_dev,
                             DevHeader* __restrict__ h, int have_indices) {
     if (threadIdx.x == 0) {
@@ -490,15 +531,24 @@ __global__ void k_nb_status(const long long* __restrict__ offsets, long long n, 
     }
 }
 
-cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity, int32_t* status_dev, cudaStream_t s) {
+cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity, int32_t* status_dev, cudaStream_t s,
+                             const double* vx, const double* vy, const double* vz, double Cv) {
     Workspace& w = t->w;
     const long long n = t->N;
     const double* rss = t->r_search ? w.rss : w.routs;
+    const bool orbit = vx != nullptr;
+    OrbitArgs oa = {w.vxs, w.vys, w.vzs, w.ms, w.routs, t->p.G, Cv};
     stage_begin(t, s);
     int grid = t->sm_count * 8;
+    if (orbit) {
+        k_gather_vel<<<cdiv(n, 256), 256, 0, s>>>(w.idx, n, vx, vy, vz, w.vxs, w.vys, w.vzs);
+        KCHECK(s, "k_gather_vel");
+        petar_count_launch(1);
+    }
     k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 1);
     KCHECK(s, "k_reset_ticket");
-    k_neighbors<false><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, nullptr, nullptr, 0);
+    if (orbit) k_neighbors<false, true><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, nullptr, nullptr, 0, oa);
+    else k_neighbors<false, false><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, nullptr, nullptr, 0, oa);
     KCHECK(s, "k_neighbors");
     petar_count_launch(2);
     cudaError_t e = launch_scan_i32_to_i64(w.nb_cnt, (long long*)offsets, n, (long long*)w.scan_tmp, s);
@@ -506,7 +556,8 @@ cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, 
     if (indices) {
         k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 1);
         KCHECK(s, "k_reset_ticket");
-        k_neighbors<true><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, (const long long*)offsets, indices, capacity);
+        if (orbit) k_neighbors<true, true><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, (const long long*)offsets, indices, capacity, oa);
+        else k_neighbors<true, false><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, (const long long*)offsets, indices, capacity, oa);
         KCHECK(s, "k_neighbors");
         petar_count_launch(2);
     }
