@@ -274,6 +274,52 @@ def main():
     e2e_ms = (time.perf_counter() - t0) * 1e3 / Ke
     h2d_bytes = 5 * 8 * N
 
+    # ---- SURVEY 8(f) ranks 1-2, timed after the headline region (not part of `value`) -----------------------
+    # Eq. 24 radii -> tree with r_search -> two-stage orbit-dependent neighbour list -> clusters
+    next_rows = None
+    if world == 1:
+        wv = make_workload(cfg, N=args.N, velocities=True)
+        vdev = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (wv.vx, wv.vy, wv.vz)]
+        rs_dev = torch.empty(N, dtype=torch.float64, device=dev)
+        label = torch.empty(N, dtype=torch.int32, device=dev); ncl = torch.zeros(1, dtype=torch.int64, device=dev)
+        coff = torch.zeros(N + 1, dtype=torch.int64, device=dev); mem = torch.empty(N, dtype=torch.int32, device=dev)
+        cws = torch.empty(P.petar_clusters_workspace_bytes(N), dtype=torch.uint8, device=dev)
+        tree.inputs = tuple(dev_in) + (rs_dev,)
+        evn = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+        acc = np.zeros(4)
+        reps = max(3, min(K, 5))
+        for rep in range(reps + 1):
+            flush.fill_(rep & 255)
+            evn[0].record(stream)
+            P.petar_search_radii(*vdev, dev_in[4], 3.0, wv.dt_L, N, rs_dev, stream)
+            evn[1].record(stream)
+            tree.build(stream)
+            evn[2].record(stream)
+            P.petar_neighbor_list_orbit(tree.handle, *vdev, 1.5, tree.offsets, None, 0, None, stream)
+            tot_o = int(tree.offsets[-1].item())
+            if tot_o > cap[0].numel():
+                cap[0] = torch.empty(int(tot_o * 1.1), dtype=torch.int32, device=dev)
+            P.petar_neighbor_list_orbit(tree.handle, *vdev, 1.5, tree.offsets, cap[0], cap[0].numel(), tree.nb_status, stream)
+            evn[3].record(stream)
+            P.petar_clusters(tree.offsets, cap[0], N, label, ncl, coff, mem, cws, stream)
+            evn[4].record(stream)
+            evn[4].synchronize()
+            if rep:                                   # first repetition = warm-up
+                acc += np.array([evn[i].elapsed_time(evn[i + 1]) for i in range(4)])
+        acc /= reps
+        n_cl = int(ncl.item())
+        hbm = float(peaks()[0].get("hbm_gbs", 6545.6))
+        cl_bytes = 8 * (N + 1) + 4 * tot_o + 4 * N + 4 * (12 + 12) * N + 8 * N + 4 * N      # CSR read, labels, 4 sort passes, offsets, members
+        next_rows = {
+            "workload": "same config with Plummer velocities + binary orbital motion, C_r = 3, C_V = 1.5, dt_L = %g" % wv.dt_L,
+            "search_radii_ms": acc[0], "search_radii_gbs": 40.0 * N / (acc[0] * 1e-3) / 1e9 if acc[0] > 0 else None,
+            "tree_build_with_r_search_ms": acc[1],
+            "walk_plus_neighbor_list_orbit_ms": acc[2], "neighbours_orbit": tot_o,
+            "clusters_ms": acc[3], "n_clusters": n_cl, "clusters_algorithmic_gbs": cl_bytes / (acc[3] * 1e-3) / 1e9 if acc[3] > 0 else None,
+            "clusters_frac_of_hbm": cl_bytes / (acc[3] * 1e-3) / 1e9 / hbm if acc[3] > 0 else None,
+        }
+        tree.inputs = tuple(dev_in) + (None,)
+
     # ---- FP32 peak probe (FFMA only), timed alone ------------------------------------------------------
     scratch = torch.zeros(1, dtype=torch.float32, device=dev)
     P.petar_probe_fp32(20000, scratch, stream)
@@ -347,6 +393,8 @@ def main():
                           hbm_peak_gbs=pk.get("hbm_gbs")),
             wall_s_timed_region=t_wall,
         )
+        if next_rows is not None:
+            out["next_rows"] = next_rows
         if not args.no_cpu_baseline and world == 1:
             cb = cpu_oracle_sample(w, args.cpu_groups)
             out["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
