@@ -209,7 +209,8 @@ int petar_debug_export(petar_tree* t, int what, void* dst, size_t dst_bytes, voi
 #define PETAR_STAGE_FORCE 7
 #define PETAR_STAGE_NEIGHBOR 8
 #define PETAR_STAGE_FORCE_UNITS 9   /* force phase A (k_force_units); PETAR_STAGE_FORCE is phase B (k_force) */
-#define PETAR_N_STAGES 10
+#define PETAR_STAGE_WALK_SUPER 10   /* super-group walks; PETAR_STAGE_WALK is the per-group walk (k_walk)   */
+#define PETAR_N_STAGES 11
 int petar_set_profiling(int on);
 int petar_stage_times(petar_tree* t, float* stage_ms /* HOST */);
 /* Number of kernel launches the library has enqueued since process start (HOST counter).           */

@@ -14,7 +14,7 @@ EXPORTS = [
     "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32", "petar_probe_fp32_mode",
     "petar_search_radii", "petar_neighbor_list_orbit", "petar_clusters_workspace_bytes", "petar_clusters",
 ]
-STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units"]
+STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units", "walk_super"]
 DBG = dict(HEADER=0, ROOT=1, KEYS=2, PERM=3, NODE_INT=4, NODE_DBL=5, GROUP_INT=6, GROUP_DBL=7, GROUP_CNT=8,
            LIST_OFFS=9, LISTS=10, GROUP_SUPER=11)
 

@@ -637,24 +637,14 @@ __global__ void k_reset_ticket2(DevHeader* h) {
     if (threadIdx.x == 0) { h->group_ticket2 = 0; h->unit_ticket = 0; for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) h->unit_cnt[k] = 0; }
 }
 
-cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s) {
+// phase A: unit table, then the super-groups' common cells.  ctas_per_sm > 0 limits the grid (tuning
+// experiments).  Needs the super-group walks only.
+cudaError_t launch_force_units(petar_tree* t, cudaStream_t s, int ctas_per_sm) {
     Workspace& w = t->w;
-    const double rho = t->p.r_in_over_r_out;
-    const double lam = (1.0 - rho) / (1.0 + rho);
-    ForceConst fc;
-    fc.c1 = (float)(1.0 / (1.0 - rho)); fc.c0 = (float)(rho / (1.0 - rho));
-    fc.lam = (float)lam; fc.one_plus_lam = (float)(1.0 + lam);
-    fc.b0 = (float)(35.0 * (1.0 - lam));
-    fc.b1 = (float)(56.0 * lam - 84.0 * (1.0 - lam));
-    fc.b2 = (float)(70.0 * (1.0 - lam) - 140.0 * lam);
-    fc.b3 = (float)(120.0 * lam - 20.0 * (1.0 - lam));
-    fc.b4 = (float)(-35.0 * lam);
-    fc.a4 = (float)(35.0 * lam);
     stage_begin(t, s);
     k_reset_ticket2<<<1, 32, 0, s>>>(w.hdr);
     KCHECK(s, "k_reset_ticket2");
     const bool quad = t->p.multipole >= 2;
-    // phase A: unit table, then the super-groups' common cells
     const int nrec_blocks = cdiv(w.group_cap, 256);
     k_units_count<<<nrec_blocks, 256, 0, s>>>(w.hdr, w.srec, w.group_cap);
     KCHECK(s, "k_units_count");
@@ -668,12 +658,33 @@ cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, doub
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force_units<false>, UW * 32, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
+    if (ctas_per_sm > 0 && ctas_per_sm < per_sm) per_sm = ctas_per_sm;
     if (quad) k_force_units<true><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, (long long)t->N);
     else k_force_units<false><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, (long long)t->N);
     KCHECK(s, "k_force_units");
+    petar_count_launch(5);
     stage_end(t, PETAR_STAGE_FORCE_UNITS, s);
+    return cudaGetLastError();
+}
+
+// phase B: the groups' own lists (needs the per-group walk and phase A)
+cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s) {
+    Workspace& w = t->w;
+    const double rho = t->p.r_in_over_r_out;
+    const double lam = (1.0 - rho) / (1.0 + rho);
+    ForceConst fc;
+    fc.c1 = (float)(1.0 / (1.0 - rho)); fc.c0 = (float)(rho / (1.0 - rho));
+    fc.lam = (float)lam; fc.one_plus_lam = (float)(1.0 + lam);
+    fc.b0 = (float)(35.0 * (1.0 - lam));
+    fc.b1 = (float)(56.0 * lam - 84.0 * (1.0 - lam));
+    fc.b2 = (float)(70.0 * (1.0 - lam) - 140.0 * lam);
+    fc.b3 = (float)(120.0 * lam - 20.0 * (1.0 - lam));
+    fc.b4 = (float)(-35.0 * lam);
+    fc.a4 = (float)(35.0 * lam);
+    const bool quad = t->p.multipole >= 2;
     stage_begin(t, s);
-    // phase B: the groups' own lists
+    int per_sm = 0;
+    cudaError_t e;
     if (quad) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<true>, FT, 0);
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<false>, FT, 0);
     if (e != cudaSuccess) return e;
@@ -684,9 +695,15 @@ cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, doub
     else
         k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.part, (long long)t->N, ax, ay, az, pot, fc, t->p.G);
     KCHECK(s, "k_force");
-    petar_count_launch(6);
+    petar_count_launch(1);
     stage_end(t, PETAR_STAGE_FORCE, s);
     return cudaGetLastError();
+}
+
+cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s) {
+    cudaError_t e = launch_force_units(t, s, 0);
+    if (e != cudaSuccess) return e;
+    return launch_force_groups(t, ax, ay, az, pot, s);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -143,7 +143,11 @@ struct petar_tree {
 cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s);
 cudaError_t launch_tree(petar_tree* t, cudaStream_t s);
 cudaError_t launch_walk(petar_tree* t, cudaStream_t s);
+cudaError_t launch_walk_supers(petar_tree* t, cudaStream_t s);
+cudaError_t launch_walk_groups(petar_tree* t, cudaStream_t s, int ctas_per_sm);
 cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s);
+cudaError_t launch_force_units(petar_tree* t, cudaStream_t s, int ctas_per_sm);
+cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s);
 // vx != nullptr: the orbit-dependent two-stage criterion (rule O10) with velocities in the caller's order
 cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity,
                              int32_t* status_dev, cudaStream_t s, const double* vx = nullptr, const double* vy = nullptr,

@@ -398,13 +398,14 @@ __global__ void k_reset_ticket(DevHeader* h, int which) {
     if (threadIdx.x == 0) { if (which == 0) { h->group_ticket = 0; h->arena_top = 0; for (int l = 0; l < PETAR_NSUP; ++l) { h->n_super[l] = 0; h->super_ticket[l] = 0; } h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = h->n_epsp_common = 0ull; } else h->group_ticket3 = 0; }
 }
 
-cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
+// the super-group levels (everything the force phase A needs)
+cudaError_t launch_walk_supers(petar_tree* t, cudaStream_t s) {
     Workspace& w = t->w;
     stage_begin(t, s);
     k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 0);
     KCHECK(s, "k_reset_ticket");
     int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_walk, WALK_WARPS * 32, 0);
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_walk_super, WALK_WARPS * 32, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     for (int l = 0; l < PETAR_NSUP; ++l) {
@@ -418,12 +419,32 @@ cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
                                                                      w.arena, w.arena_chunks, t->p.theta, w.node_cap, l);
         KCHECK(s, "k_walk_super");
     }
+    petar_count_launch(1 + 3 * PETAR_NSUP);
+    stage_end(t, PETAR_STAGE_WALK_SUPER, s);
+    return cudaGetLastError();
+}
+
+// the per-group walks; ctas_per_sm > 0 limits the grid (tuning experiments)
+cudaError_t launch_walk_groups(petar_tree* t, cudaStream_t s, int ctas_per_sm) {
+    Workspace& w = t->w;
+    stage_begin(t, s);
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_walk, WALK_WARPS * 32, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    if (ctas_per_sm > 0 && ctas_per_sm < per_sm) per_sm = ctas_per_sm;
     k_walk<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, w.nmac, w.grp, w.srec, w.smap, w.arena, w.arena_chunks, t->p.theta, w.node_cap,
                                                           (long long)t->N, w.group_cap);
     KCHECK(s, "k_walk");
-    petar_count_launch(2 + 3 * PETAR_NSUP);
+    petar_count_launch(1);
     stage_end(t, PETAR_STAGE_WALK, s);
     return cudaGetLastError();
+}
+
+cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
+    cudaError_t e = launch_walk_supers(t, s);
+    if (e != cudaSuccess) return e;
+    return launch_walk_groups(t, s, 0);
 }
 
 // ------------------------------------------------------------------------------------------------
