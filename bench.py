@@ -285,8 +285,10 @@ def main():
         coff = torch.zeros(N + 1, dtype=torch.int64, device=dev); mem = torch.empty(N, dtype=torch.int32, device=dev)
         cws = torch.empty(P.petar_clusters_workspace_bytes(N), dtype=torch.uint8, device=dev)
         tree.inputs = tuple(dev_in) + (rs_dev,)
-        evn = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
-        acc = np.zeros(4)
+        sws = torch.empty(P.petar_short_range_workspace_bytes(N), dtype=torch.uint8, device=dev)
+        sr_out = [torch.empty(N, dtype=torch.float64, device=dev) for _ in range(7)]
+        evn = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+        acc = np.zeros(5)
         reps = max(3, min(K, 5))
         for rep in range(reps + 1):
             flush.fill_(rep & 255)
@@ -303,9 +305,12 @@ def main():
             evn[3].record(stream)
             P.petar_clusters(tree.offsets, cap[0], N, label, ncl, coff, mem, cws, stream)
             evn[4].record(stream)
-            evn[4].synchronize()
+            P.petar_short_range_force(*dev_in[:3], *vdev, dev_in[3], dev_in[4], tree.offsets, cap[0], N, params.G, params.r_in_over_r_out,
+                                      sr_out[0:3], sr_out[3:6], sr_out[6], sws, stream)
+            evn[5].record(stream)
+            evn[5].synchronize()
             if rep:                                   # first repetition = warm-up
-                acc += np.array([evn[i].elapsed_time(evn[i + 1]) for i in range(4)])
+                acc += np.array([evn[i].elapsed_time(evn[i + 1]) for i in range(5)])
         acc /= reps
         n_cl = int(ncl.item())
         hbm = float(peaks()[0].get("hbm_gbs", 6545.6))
@@ -317,6 +322,9 @@ def main():
             "walk_plus_neighbor_list_orbit_ms": acc[2], "neighbours_orbit": tot_o,
             "clusters_ms": acc[3], "n_clusters": n_cl, "clusters_algorithmic_gbs": cl_bytes / (acc[3] * 1e-3) / 1e9 if acc[3] > 0 else None,
             "clusters_frac_of_hbm": cl_bytes / (acc[3] * 1e-3) / 1e9 / hbm if acc[3] > 0 else None,
+            "short_range_force_ms": acc[4],
+            "short_range_algorithmic_gbs": (112.0 * N + 8.0 * (N + 1) + 68.0 * tot_o) / (acc[4] * 1e-3) / 1e9 if acc[4] > 0 else None,
+            "short_range_frac_of_hbm": (112.0 * N + 8.0 * (N + 1) + 68.0 * tot_o) / (acc[4] * 1e-3) / 1e9 / hbm if acc[4] > 0 else None,
         }
         tree.inputs = tuple(dev_in) + (None,)
 

@@ -153,6 +153,26 @@ int petar_clusters(const int64_t* offsets, const int32_t* indices, int64_t N, in
                    int64_t* n_clusters_dev, int64_t* cluster_offsets, int32_t* members,
                    void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Short-range part H_S of Eq. 11 over neighbour rows: for every i
+ *   a_S,i = -G sum_j m_j K(x) d/r^3,   j_S,i = d a_S,i / dt,   phi_S,i = -G sum_j m_j W(x)/r,   j in row i,
+ * d = x_i - x_j, K, W of Eq. 17 / Eq. 15 with R = max(r_out,i, r_out,j), r_in = r_in_over_r_out * R and
+ * K' = -280 Lambda (x+q) x^3 (1-x)^3 (from Eq. 18) in the jerk.  Entries at r >= R or r = 0 contribute nothing.
+ *   x..r_out      : DEVICE fp64[N], caller's order (the order the neighbour list refers to).
+ *   offsets, indices : DEVICE CSR neighbour list (petar_neighbor_list / _orbit).
+ *   acc_*, jerk_*, pot : DEVICE fp64[N]; any may be NULL (skipped).  fp64 throughout; rows are summed in
+ *                    list order (rows longer than 32 entries by one warp, in a fixed order).
+ *   workspace     : DEVICE, 256-byte aligned, >= petar_short_range_workspace_bytes(N).
+ * No host synchronisation.  Errors: PETAR_EINVAL, PETAR_EWORKSPACE, PETAR_ECUDA.                    */
+size_t petar_short_range_workspace_bytes(int64_t N);
+int petar_short_range_force(const double* x, const double* y, const double* z,
+                            const double* vx, const double* vy, const double* vz,
+                            const double* m, const double* r_out,
+                            const int64_t* offsets, const int32_t* indices, int64_t N,
+                            double G, double r_in_over_r_out,
+                            double* acc_x, double* acc_y, double* acc_z,
+                            double* jerk_x, double* jerk_y, double* jerk_z, double* pot,
+                            void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Synchronises the stream and returns the device status word (PETAR_ST_* bits) in *status_host.    */
 int petar_tree_status(petar_tree* t, int32_t* status_host /* HOST */, void* cuda_stream);
 

@@ -6,5 +6,5 @@ fp64, built with gcc at first use) through ctypes and imports nothing from the C
 """
 from .binding import (  # noqa: F401
     OracleParams, OracleTree, K, W, f, direct, neighbors_direct, build_library, num_threads,
-    search_radii, pericentre, neighbors_orbit_direct, clusters,
+    search_radii, pericentre, neighbors_orbit_direct, clusters, dK, short_range,
 )

@@ -142,6 +142,26 @@ def neighbors_orbit_direct(x, y, z, vx, vy, vz, m, rnb, rout, G: float, Cv: floa
     return off, idx[: int(off[-1])]
 
 
+def dK(x, lam, q):
+    L = _lib()
+    L.ora_dK.restype = C.c_double; L.ora_dK.argtypes = [C.c_double] * 3
+    return np.vectorize(lambda v: L.ora_dK(float(v), float(lam), float(q)))(np.asarray(x, dtype=np.float64))
+
+
+def short_range(x, y, z, vx, vy, vz, m, rout, offsets, indices, G: float, rho: float):
+    """H_S over the neighbour rows: (ax, ay, az, jx, jy, jz, pot), see ora_short_range."""
+    a = list(map(_f64, (x, y, z, vx, vy, vz, m, rout)))
+    n = a[0].shape[0]
+    off = np.ascontiguousarray(offsets, dtype=np.int64)
+    idx = np.ascontiguousarray(indices, dtype=np.int32)
+    if idx.size == 0:
+        idx = np.zeros(1, dtype=np.int32)
+    out = [np.zeros(n) for _ in range(7)]
+    _lib().ora_short_range(C.c_int64(n), *[_p(v, C.c_double) for v in a], _p(off, C.c_int64), _p(idx, C.c_int32),
+                           C.c_double(G), C.c_double(rho), *[_p(o, C.c_double) for o in out])
+    return tuple(out)
+
+
 def clusters(offsets, indices):
     """Connected components of the neighbour graph: (label int32[N] = smallest member, n_clusters)."""
     off = np.ascontiguousarray(offsets, dtype=np.int64)

@@ -23,6 +23,10 @@
  * Part (C): Eq. 24 search radii, the Kepler-pericentre filter and the
  * clustering; pinned by conic closed forms (r_p = a(1-e), a(e-1), impact parameter), r_p <= r,
  * symmetry, C_V -> infinity == rule O9, tree == O(N^2) definition, components against scipy.
+ * Part (D) (rank 4): short-range acceleration, jerk and potential over the neighbour rows; pinned by
+ * the O(N^2) short-range definition of part (A), dK/dx against a difference quotient of Eq. 17, the
+ * jerk against a difference quotient of the acceleration along x + v t, Newton's two-body jerk
+ * inside r_in, and sum m a = sum m j = 0.
  * Parity UNPINNED (the paper prints nothing to pin them to): interaction counts and
  * force error at theta > 0 (only monotonicity sanity checks).
  *
@@ -731,6 +735,60 @@ int64_t ora_clusters(int64_t N, const int64_t *offsets, const int32_t *indices, 
     for (int64_t i = 0; i < N; ++i) { int64_t r = uf_find(parent, i); label[i] = (int32_t)r; nc += (r == i); }
     free(parent);
     return nc;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* (D) short-range force, jerk and potential over the neighbour list  */
+/* ------------------------------------------------------------------------------------ */
+
+/* dK/dx of Eq. 17 for 0 < x < 1 (0 outside).  Differentiating Eq. 18,
+ * K = f - (x+q) f', gives K' = -(x+q) f'' with f'' = 280 Lambda x^3 (1-x)^3 (from Eq. 16) and
+ * q = r_in / (r_out - r_in); all of Eq. 19's boundary values follow from the x^3 (1-x)^3 factor.   */
+double ora_dK(double x, double Lam, double q) {
+    if (x <= 0.0 || x >= 1.0) return 0.0;
+    double y = 1.0 - x;
+    return -280.0 * Lam * (x + q) * (x * x * x) * (y * y * y);
+}
+
+/* H_S of Eq. 11 evaluated over the neighbour rows (the Hermite integrator's force
+ * evaluation, Eq. 40 :639 needs the acceleration and its first time derivative):
+ *   a_S,i   = -G sum_j m_j K(x) d / r^3,                       d = x_i - x_j, w = v_i - v_j
+ *   j_S,i   = -G sum_j m_j { K [ w / r^3 - 3 (d.w) d / r^5 ] + K'(x) xdot d / r^3 },  xdot = (d.w) / (r (R - r_in))
+ *   phi_S,i = -G sum_j m_j W(x) / r
+ * with R = max(r_out,i, r_out,j), r_in = rho R, x = (r - r_in)/(R - r_in).  Pairs at r >= R contribute
+ * nothing; coincident pairs (r = 0) are skipped (reading P4).  Rows are summed in list order.       */
+void ora_short_range(int64_t N, const double *x, const double *y, const double *z, const double *vx, const double *vy,
+                     const double *vz, const double *m, const double *rout, const int64_t *offsets, const int32_t *indices,
+                     double G, double rho, double *ax, double *ay, double *az, double *jx, double *jy, double *jz, double *pot) {
+    const double q = rho / (1.0 - rho);
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t i = 0; i < N; ++i) {
+        double a[3] = {0, 0, 0}, jk[3] = {0, 0, 0}, phi = 0.0;
+        for (int64_t e = offsets[i]; e < offsets[i + 1]; ++e) {
+            int64_t j = indices[e];
+            double dx = x[i] - x[j], dy = y[i] - y[j], dz = z[i] - z[j];
+            double wx = vx[i] - vx[j], wy = vy[i] - vy[j], wz = vz[i] - vz[j];
+            double r2 = dx * dx + dy * dy + dz * dz;
+            double r = sqrt(r2);
+            double R = rout[i] > rout[j] ? rout[i] : rout[j];
+            if (r == 0.0 || r >= R) continue;
+            double rin = rho * R;
+            double Lam = (R - rin) / (R + rin);
+            double xx = (r - rin) / (R - rin);
+            double K = ora_K(xx, Lam), W = ora_W(xx, Lam), dK = ora_dK(xx, Lam, q);
+            double dw = dx * wx + dy * wy + dz * wz;
+            double r3 = r2 * r;
+            double xdot = dw / (r * (R - rin));
+            double c0 = -G * m[j] * K / r3;                       /* coefficient of d in a, of w in the jerk */
+            double c1 = -G * m[j] * (-3.0 * K * dw / (r3 * r2) + dK * xdot / r3);
+            a[0] += c0 * dx; a[1] += c0 * dy; a[2] += c0 * dz;
+            jk[0] += c0 * wx + c1 * dx; jk[1] += c0 * wy + c1 * dy; jk[2] += c0 * wz + c1 * dz;
+            phi -= G * m[j] * W / r;
+        }
+        ax[i] = a[0]; ay[i] = a[1]; az[i] = a[2];
+        jx[i] = jk[0]; jy[i] = jk[1]; jz[i] = jk[2];
+        pot[i] = phi;
+    }
 }
 
 int ora_num_threads(void) {

@@ -13,5 +13,6 @@ from .binding import (  # noqa: F401
     petar_tree_status, petar_tree_destroy, petar_strerror, petar_debug_export,
     petar_set_profiling, petar_stage_times, petar_launch_count, petar_probe_fp32, petar_probe_fp32_mode,
     petar_search_radii, petar_neighbor_list_orbit, petar_clusters_workspace_bytes, petar_clusters,
+    petar_short_range_workspace_bytes, petar_short_range_force,
     STAGE_NAMES,
 )

@@ -13,6 +13,7 @@ EXPORTS = [
     "petar_tree_status", "petar_tree_destroy", "petar_strerror", "petar_debug_export",
     "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32", "petar_probe_fp32_mode",
     "petar_search_radii", "petar_neighbor_list_orbit", "petar_clusters_workspace_bytes", "petar_clusters",
+    "petar_short_range_workspace_bytes", "petar_short_range_force",
 ]
 STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units", "walk_super"]
 DBG = dict(HEADER=0, ROOT=1, KEYS=2, PERM=3, NODE_INT=4, NODE_DBL=5, GROUP_INT=6, GROUP_DBL=7, GROUP_CNT=8,
@@ -79,6 +80,11 @@ def lib():
         L.petar_clusters.restype = C.c_int
         L.petar_clusters.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_size_t, C.c_void_p]
+        L.petar_short_range_workspace_bytes.restype = C.c_size_t
+        L.petar_short_range_workspace_bytes.argtypes = [C.c_int64]
+        L.petar_short_range_force.restype = C.c_int
+        L.petar_short_range_force.argtypes = ([C.c_void_p] * 10 + [C.c_int64, C.c_double, C.c_double] + [C.c_void_p] * 7
+                                              + [C.c_void_p, C.c_size_t, C.c_void_p])
         L.petar_tree_status.restype = C.c_int
         L.petar_tree_status.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.c_void_p]
         L.petar_tree_destroy.restype = C.c_int
@@ -175,6 +181,20 @@ def petar_clusters(offsets, indices, N: int, label, n_clusters_dev=None, cluster
                               _ptr(members), _ptr(workspace), C.c_size_t(0 if workspace is None else workspace.numel()), _stream(stream))
     if rc:
         raise PetarError(rc, "petar_clusters")
+
+
+def petar_short_range_workspace_bytes(N: int) -> int:
+    return int(lib().petar_short_range_workspace_bytes(C.c_int64(N)))
+
+
+def petar_short_range_force(x, y, z, vx, vy, vz, m, r_out, offsets, indices, N: int, G: float, rho: float,
+                            acc, jerk, pot, workspace, stream=None) -> None:
+    """acc, jerk: 3-tuples of CUDA fp64 tensors (entries may be None); pot: tensor or None."""
+    rc = lib().petar_short_range_force(*[_ptr(a) for a in (x, y, z, vx, vy, vz, m, r_out, offsets, indices)], C.c_int64(N),
+                                       C.c_double(G), C.c_double(rho), *[_ptr(a) for a in acc], *[_ptr(a) for a in jerk], _ptr(pot),
+                                       _ptr(workspace), C.c_size_t(0 if workspace is None else workspace.numel()), _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_short_range_force")
 
 
 def petar_tree_status(tree, stream=None) -> int:

@@ -1,0 +1,121 @@
+// short.cu -- SURVEY.md 8(f) rank 4: the short-range part H_S of Eq. 11 over the
+// neighbour rows: acceleration, its first time derivative (the Hermite integrator's force evaluation,
+// PAPER.md:300, Eq. 40 :639) and potential, with the changeover functions K (Eq. 17), W (Eq. 15) and
+// K' = -280 Lambda (x+q) x^3 (1-x)^3 (from Eq. 18).  All fp64.
+//
+// Rows are short (the binary companion, rarely a few more) with a few very long ones (a massive
+// particle): rows of up to SHORT_ROW entries are summed by one thread in list order; longer rows are
+// queued and summed by one warp each (lanes take entries lane, lane+32, ..., then a fixed-order
+// shuffle reduction), so every result is deterministic.  HBM-bound: 56 B read + 56 B written per
+// particle and 64 B gathered per list entry.
+#include "internal.cuh"
+
+#define SHORT_ROW 32
+
+struct ShortArgs {
+    const double *x, *y, *z, *vx, *vy, *vz, *m, *rout;
+    const long long* offsets; const int* indices;
+    double *ax, *ay, *az, *jx, *jy, *jz, *pot;
+    double G, rho, lam, q;
+    long long n;
+};
+
+struct Sum7 { double a0, a1, a2, j0, j1, j2, p; };
+
+__device__ __forceinline__ void short_pair(const ShortArgs& A, const double xi, const double yi, const double zi, const double vxi,
+                                           const double vyi, const double vzi, const double ri, const int j, Sum7& s) {
+    const double dx = xi - A.x[j], dy = yi - A.y[j], dz = zi - A.z[j];
+    const double wx = vxi - A.vx[j], wy = vyi - A.vy[j], wz = vzi - A.vz[j];
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double r = sqrt(r2);
+    const double R = fmax(ri, A.rout[j]);
+    if (r == 0.0 || r >= R) return;
+    const double rin = A.rho * R;
+    const double xx = (r - rin) / (R - rin);
+    double K = 1.0, dK = 0.0, W;
+    if (xx > 0.0) {
+        const double xm = xx - 1.0, xm2 = xm * xm, x2 = xx * xx;
+        K = (xm2 * xm2) * (1.0 + 4.0 * xx + 10.0 * x2 + 20.0 * x2 * xx + 35.0 * A.lam * x2 * x2);      // Eq. 17
+        const double y = 1.0 - xx;
+        dK = -280.0 * A.lam * (xx + A.q) * (x2 * xx) * (y * y * y);
+        W = A.lam * (1.0 - 2.0 * xx) + A.lam * (x2 * x2 * xx) * (14.0 - 28.0 * xx + 20.0 * x2 - 5.0 * x2 * xx);   // Eq. 15: ... - 1 + f(x)
+    } else {
+        W = A.lam * (1.0 - 2.0 * xx);                                                                    // x <= 0, unclamped (reading P4)
+    }
+    const double mj = A.m[j];
+    const double dw = dx * wx + dy * wy + dz * wz;
+    const double r3 = r2 * r;
+    const double xdot = dw / (r * (R - rin));
+    const double c0 = -A.G * mj * K / r3;
+    const double c1 = -A.G * mj * (-3.0 * K * dw / (r3 * r2) + dK * xdot / r3);
+    s.a0 += c0 * dx; s.a1 += c0 * dy; s.a2 += c0 * dz;
+    s.j0 += c0 * wx + c1 * dx; s.j1 += c0 * wy + c1 * dy; s.j2 += c0 * wz + c1 * dz;
+    s.p -= A.G * mj * W / r;
+}
+
+__device__ __forceinline__ void short_store(const ShortArgs& A, const long long i, const Sum7& s) {
+    if (A.ax) A.ax[i] = s.a0; if (A.ay) A.ay[i] = s.a1; if (A.az) A.az[i] = s.a2;
+    if (A.jx) A.jx[i] = s.j0; if (A.jy) A.jy[i] = s.j1; if (A.jz) A.jz[i] = s.j2;
+    if (A.pot) A.pot[i] = s.p;
+}
+
+// queue[0] = number of long rows, queue[1..] = their particle indices
+__global__ void __launch_bounds__(256) k_short_rows(const ShortArgs A, int* __restrict__ queue) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= A.n) return;
+    const long long b = A.offsets[i], e = A.offsets[i + 1];
+    if (e - b > SHORT_ROW) { queue[1 + atomicAdd(&queue[0], 1)] = (int)i; return; }
+    Sum7 s = {0, 0, 0, 0, 0, 0, 0};
+    if (e > b) {
+        const double xi = A.x[i], yi = A.y[i], zi = A.z[i], vxi = A.vx[i], vyi = A.vy[i], vzi = A.vz[i], ri = A.rout[i];
+        for (long long k = b; k < e; ++k) short_pair(A, xi, yi, zi, vxi, vyi, vzi, ri, A.indices[k], s);
+    }
+    short_store(A, i, s);
+}
+
+__global__ void __launch_bounds__(256) k_short_long_rows(const ShortArgs A, const int* __restrict__ queue) {
+    const int lane = threadIdx.x & 31;
+    const int nq = queue[0];
+    for (int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < nq; w += (gridDim.x * blockDim.x) >> 5) {
+        const long long i = queue[1 + w];
+        const long long b = A.offsets[i], e = A.offsets[i + 1];
+        const double xi = A.x[i], yi = A.y[i], zi = A.z[i], vxi = A.vx[i], vyi = A.vy[i], vzi = A.vz[i], ri = A.rout[i];
+        Sum7 s = {0, 0, 0, 0, 0, 0, 0};
+        for (long long k = b + lane; k < e; k += 32) short_pair(A, xi, yi, zi, vxi, vyi, vzi, ri, A.indices[k], s);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            s.a0 += __shfl_down_sync(0xffffffffu, s.a0, o); s.a1 += __shfl_down_sync(0xffffffffu, s.a1, o); s.a2 += __shfl_down_sync(0xffffffffu, s.a2, o);
+            s.j0 += __shfl_down_sync(0xffffffffu, s.j0, o); s.j1 += __shfl_down_sync(0xffffffffu, s.j1, o); s.j2 += __shfl_down_sync(0xffffffffu, s.j2, o);
+            s.p += __shfl_down_sync(0xffffffffu, s.p, o);
+        }
+        if (lane == 0) short_store(A, i, s);
+    }
+}
+
+extern "C" size_t petar_short_range_workspace_bytes(int64_t N) { return N < 0 ? 0 : ((size_t)(N + 1) * 4 + 255) / 256 * 256; }
+
+extern "C" int petar_short_range_force(const double* x, const double* y, const double* z, const double* vx, const double* vy, const double* vz,
+                                       const double* m, const double* r_out, const int64_t* offsets, const int32_t* indices, int64_t N,
+                                       double G, double r_in_over_r_out, double* acc_x, double* acc_y, double* acc_z,
+                                       double* jerk_x, double* jerk_y, double* jerk_z, double* pot,
+                                       void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (N < 0 || N > 2000000000ll || !(r_in_over_r_out > 0.0 && r_in_over_r_out < 1.0) || !(G == G)) return PETAR_EINVAL;
+    if (N == 0) return PETAR_OK;
+    if (!x || !y || !z || !vx || !vy || !vz || !m || !r_out || !offsets) return PETAR_EINVAL;
+    if (!workspace || workspace_bytes < petar_short_range_workspace_bytes(N) || ((uintptr_t)workspace & 255u)) return PETAR_EWORKSPACE;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    ShortArgs A;
+    A.x = x; A.y = y; A.z = z; A.vx = vx; A.vy = vy; A.vz = vz; A.m = m; A.rout = r_out;
+    A.offsets = (const long long*)offsets; A.indices = indices;
+    A.ax = acc_x; A.ay = acc_y; A.az = acc_z; A.jx = jerk_x; A.jy = jerk_y; A.jz = jerk_z; A.pot = pot;
+    A.G = G; A.rho = r_in_over_r_out; A.lam = (1.0 - r_in_over_r_out) / (1.0 + r_in_over_r_out);
+    A.q = r_in_over_r_out / (1.0 - r_in_over_r_out); A.n = N;
+    int* queue = (int*)workspace;
+    if (cudaMemsetAsync(queue, 0, 4, s) != cudaSuccess) return PETAR_ECUDA;
+    k_short_rows<<<cdiv(N, 256), 256, 0, s>>>(A, queue);
+    KCHECK(s, "k_short_rows");
+    k_short_long_rows<<<148 * 4, 256, 0, s>>>(A, queue);
+    KCHECK(s, "k_short_long_rows");
+    petar_count_launch(2);
+    return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;
+}
