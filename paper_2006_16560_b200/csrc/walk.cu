@@ -478,7 +478,9 @@ __global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, co
                                                    const double* __restrict__ rss, int* __restrict__ cnt,
                                                    const long long* __restrict__ offsets, int* __restrict__ indices, long long capacity,
                                                    const OrbitArgs oa) {
-    const int lane = threadIdx.x & 31;
+    __shared__ double s_x[8][32], s_y[8][32], s_z[8][32], s_r[8][32];
+    __shared__ int s_j[8][32];
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
     const int ng = h->n_groups;
     for (;;) {
         int g = 0;
@@ -503,24 +505,48 @@ __global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, co
             while (chunk >= 0 && remaining > 0) {
                 const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
                 const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
-                for (int e = 0; e < ne; e += 2) {
-                    const int jb = cp[PETAR_CHUNK_HDR + e], je = cp[PETAR_CHUNK_HDR + e + 1];
-                    for (int j = jb; j < je; ++j) {
-                        double xj = xs[j], yj = ys[j], zj = zs[j], rj = rss[j];   // warp-uniform loads
-                        double dx = xi - xj, dy = yi - yj, dz = zi - zj;
-                        double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                        double R = fmax(ri, rj);
-                        bool keep = vi && j != i && r2 < R * R;
-                        if (ORBIT && keep) {
-                            const double Ro = fmax(roi, oa.routs[j]);
-                            if (!(r2 < Ro * Ro)) {
-                                const double rp = pericentre(dx, dy, dz, r2, vxi - oa.vxs[j], vyi - oa.vys[j], vzi - oa.vzs[j], oa.G * (mi + oa.ms[j]));
-                                keep = rp < oa.Cv * fmin(ri, rj);
-                            }
+                // 32 leaf ranges at a time: their particles are flattened (warp scan + search), staged 32 at a
+                // time in shared memory with one coalesced load per array, then tested by every lane
+                for (int e0 = 0; e0 < ne; e0 += 64) {
+                    int jb_l = 0, cnt_l = 0;
+                    if (e0 + 2 * lane < ne) { const int2 be = *reinterpret_cast<const int2*>(cp + PETAR_CHUNK_HDR + e0 + 2 * lane); jb_l = be.x; cnt_l = be.y - be.x; }
+                    int incl = cnt_l;
+#pragma unroll
+                    for (int o2 = 1; o2 < 32; o2 <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o2); if (lane >= o2) incl += v; }
+                    const int total = __shfl_sync(0xffffffffu, incl, 31);
+                    const int excl = incl - cnt_l;
+                    for (int p0 = 0; p0 < total; p0 += 32) {
+                        const int p = p0 + lane;
+                        int lo = 0;                               // smallest range whose inclusive count exceeds p
+#pragma unroll
+                        for (int step = 16; step > 0; step >>= 1) { const int v = __shfl_sync(0xffffffffu, incl, lo + step - 1); if (v <= p) lo += step; }
+                        lo = min(lo, 31);
+                        const int rjb = __shfl_sync(0xffffffffu, jb_l, lo), rex = __shfl_sync(0xffffffffu, excl, lo);
+                        __syncwarp();
+                        if (p < total) {
+                            const int j = rjb + (p - rex);
+                            s_x[wp][lane] = xs[j]; s_y[wp][lane] = ys[j]; s_z[wp][lane] = zs[j]; s_r[wp][lane] = rss[j]; s_j[wp][lane] = j;
                         }
-                        if (keep) {
-                            if (FILL) { if (o + c < capacity) indices[o + c] = (int)perm[j]; }
-                            ++c;
+                        __syncwarp();
+                        const int nb = min(32, total - p0);
+                        for (int k = 0; k < nb; ++k) {
+                            const int j = s_j[wp][k];
+                            const double xj = s_x[wp][k], yj = s_y[wp][k], zj = s_z[wp][k], rj = s_r[wp][k];
+                            double dx = xi - xj, dy = yi - yj, dz = zi - zj;
+                            double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                            double R = fmax(ri, rj);
+                            bool keep = vi && j != i && r2 < R * R;
+                            if (ORBIT && keep) {
+                                const double Ro = fmax(roi, oa.routs[j]);
+                                if (!(r2 < Ro * Ro)) {
+                                    const double rp = pericentre(dx, dy, dz, r2, vxi - oa.vxs[j], vyi - oa.vys[j], vzi - oa.vzs[j], oa.G * (mi + oa.ms[j]));
+                                    keep = rp < oa.Cv * fmin(ri, rj);
+                                }
+                            }
+                            if (keep) {
+                                if (FILL) { if (o + c < capacity) indices[o + c] = (int)perm[j]; }
+                                ++c;
+                            }
                         }
                     }
                 }
