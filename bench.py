@@ -326,6 +326,37 @@ def main():
             "short_range_algorithmic_gbs": (112.0 * N + 8.0 * (N + 1) + 68.0 * tot_o) / (acc[4] * 1e-3) / 1e9 if acc[4] > 0 else None,
             "short_range_frac_of_hbm": (112.0 * N + 8.0 * (N + 1) + 68.0 * tot_o) / (acc[4] * 1e-3) / 1e9 / hbm if acc[4] > 0 else None,
         }
+        # rank 3: kick, artificial particles of every binary (3rd-order measure points + pseudoparticles), tensor fit
+        pairs = wv.meta["pairs"]
+        nbin = int(pairs.shape[0])
+        if nbin:
+            na, nc = P.art_count(3), 16
+            pd = torch.from_numpy(np.ascontiguousarray(pairs)).to(dev)
+            art = [torch.empty(nbin * na, dtype=torch.float64, device=dev) for _ in range(4)]
+            elem = torch.empty(nbin * 8, dtype=torch.float64, device=dev)
+            Tt = torch.empty(nbin * nc, dtype=torch.float64, device=dev)
+            vk = [v.clone() for v in vdev]
+            ev3 = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            acc3 = np.zeros(3)
+            for rep in range(reps + 1):
+                flush.fill_(rep & 255)
+                ev3[0].record(stream)
+                P.petar_kick(*vk, tree.acc_x, tree.acc_y, tree.acc_z, 0.5 * wv.dt_L, N, stream)
+                ev3[1].record(stream)
+                P.petar_artificial_particles(*dev_in[:3], *vdev, dev_in[3], pd, nbin, params.G, 3, 2.0, *art, elem, stream)
+                ev3[2].record(stream)
+                P.petar_tidal_tensor_fit(art[0], art[1], art[2], elem, nbin, 3, Tt, stream)      # (positions stand in for accelerations: timing only)
+                ev3[3].record(stream)
+                ev3[3].synchronize()
+                if rep:
+                    acc3 += np.array([ev3[i].elapsed_time(ev3[i + 1]) for i in range(3)])
+            acc3 /= reps
+            next_rows.update({
+                "kick_ms": acc3[0], "kick_gbs": 72.0 * N / (acc3[0] * 1e-3) / 1e9,
+                "n_binaries": nbin, "artificial_particles_ms": acc3[1],
+                "artificial_particles_gbs": nbin * (2 * 56.0 + 8 + na * 32.0 + 64.0) / (acc3[1] * 1e-3) / 1e9,
+                "tidal_tensor_fit_ms": acc3[2], "tidal_tensor_fit_gbs": nbin * (9 * 24.0 + 64.0 + nc * 8.0) / (acc3[2] * 1e-3) / 1e9,
+            })
         tree.inputs = tuple(dev_in) + (None,)
 
     # ---- FP32 peak probe (FFMA only), timed alone ------------------------------------------------------

@@ -173,6 +173,40 @@ int petar_short_range_force(const double* x, const double* y, const double* z,
                             double* jerk_x, double* jerk_y, double* jerk_z, double* pot,
                             void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- P3T-kick and the artificial particles (section 6.4) -----------
+ * P3T-kick: v += a dt, in place.  All DEVICE fp64[N].                           */
+int petar_kick(double* vx, double* vy, double* vz, const double* ax, const double* ay, const double* az,
+               double dt, int64_t N, void* cuda_stream);
+
+/* Artificial particles of n_bin binaries.  pairs: DEVICE int32[n_bin][2], the particle indices
+ * of the two members.  For binary b the outputs hold PETAR_ART_COUNT(order) entries starting at
+ * b * PETAR_ART_COUNT(order):
+ *   [0, n_tt)       tidal-tensor measure points, mass 0: the corners of a regular tetrahedron (order 2, n_tt = 4)
+ *                   or of the paper's "cube" (order 3, n_tt = 8) around the centre of mass, coordinates of
+ *                   Table 1 part (3) times d_c = tt_scale * a (reading P24);
+ *   [n_tt]          the centre-of-mass point, mass 0 (it measures A(r_cm), Eq. 27);
+ *   [n_tt+1, +3)    the pseudoparticles of Eq. 38, mass (m1+m2)/3 each, in the orbital frame of Eq. 32 (x to
+ *                   the pericentre, z along the angular momentum) around the centre of mass.
+ *   elem : DEVICE fp64[n_bin][8] or NULL: a, e, d_c, cm[3], bound (1/0), m1+m2.
+ * An unbound or radial pair gets bound = 0, d_c = 0 and every entry at the centre of mass (the three masses
+ * still carry the monopole).  The caller appends the entries to the particle set for the tree build and gives the
+ * members zero mass there.  Errors: PETAR_EINVAL (order not 2 | 3, tt_scale <= 0, G <= 0, NULL), PETAR_ECUDA. */
+#define PETAR_ART_COUNT(order) ((order) == 2 ? 8 : 12)
+#define PETAR_TT_COEFFS(order) ((order) == 2 ? 6 : 16)
+int petar_artificial_particles(const double* x, const double* y, const double* z,
+                               const double* vx, const double* vy, const double* vz, const double* m,
+                               const int32_t* pairs, int64_t n_bin, double G, int32_t order, double tt_scale,
+                               double* art_x, double* art_y, double* art_z, double* art_m,
+                               double* elem, void* cuda_stream);
+
+/* Tidal-tensor coefficients (Eq. 25-26) from the long-range accelerations measured at the artificial particles
+ * (acc_*: DEVICE fp64, same layout as art_*): T[b] = M^-1 (A(r_k) - A(r_cm)), M^-1 the generalized inverse of
+ * Eq. 28 = the formulas of Table 1 part (1).  T: DEVICE fp64[n_bin][PETAR_TT_COEFFS(order)], order
+ * xx xy xz yy yz zz [xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz]; convention of Table 1 part (2):
+ * A_i(r) = A_i(r_cm) + A_ij r'_j + A_ijk r'_j r'_k.  Binaries with d_c = 0 get zeros.                 */
+int petar_tidal_tensor_fit(const double* acc_x, const double* acc_y, const double* acc_z, const double* elem,
+                           int64_t n_bin, int32_t order, double* T, void* cuda_stream);
+
 /* Synchronises the stream and returns the device status word (PETAR_ST_* bits) in *status_host.    */
 int petar_tree_status(petar_tree* t, int32_t* status_host /* HOST */, void* cuda_stream);
 

@@ -14,6 +14,7 @@ EXPORTS = [
     "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32", "petar_probe_fp32_mode",
     "petar_search_radii", "petar_neighbor_list_orbit", "petar_clusters_workspace_bytes", "petar_clusters",
     "petar_short_range_workspace_bytes", "petar_short_range_force",
+    "petar_kick", "petar_artificial_particles", "petar_tidal_tensor_fit",
 ]
 STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units", "walk_super"]
 DBG = dict(HEADER=0, ROOT=1, KEYS=2, PERM=3, NODE_INT=4, NODE_DBL=5, GROUP_INT=6, GROUP_DBL=7, GROUP_CNT=8,
@@ -85,6 +86,12 @@ def lib():
         L.petar_short_range_force.restype = C.c_int
         L.petar_short_range_force.argtypes = ([C.c_void_p] * 10 + [C.c_int64, C.c_double, C.c_double] + [C.c_void_p] * 7
                                               + [C.c_void_p, C.c_size_t, C.c_void_p])
+        L.petar_kick.restype = C.c_int
+        L.petar_kick.argtypes = [C.c_void_p] * 6 + [C.c_double, C.c_int64, C.c_void_p]
+        L.petar_artificial_particles.restype = C.c_int
+        L.petar_artificial_particles.argtypes = [C.c_void_p] * 8 + [C.c_int64, C.c_double, C.c_int32, C.c_double] + [C.c_void_p] * 6
+        L.petar_tidal_tensor_fit.restype = C.c_int
+        L.petar_tidal_tensor_fit.argtypes = [C.c_void_p] * 4 + [C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
         L.petar_tree_status.restype = C.c_int
         L.petar_tree_status.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.c_void_p]
         L.petar_tree_destroy.restype = C.c_int
@@ -195,6 +202,32 @@ def petar_short_range_force(x, y, z, vx, vy, vz, m, r_out, offsets, indices, N: 
                                        _ptr(workspace), C.c_size_t(0 if workspace is None else workspace.numel()), _stream(stream))
     if rc:
         raise PetarError(rc, "petar_short_range_force")
+
+
+def petar_kick(vx, vy, vz, ax, ay, az, dt: float, N: int, stream=None) -> None:
+    rc = lib().petar_kick(*[_ptr(a) for a in (vx, vy, vz, ax, ay, az)], C.c_double(dt), C.c_int64(N), _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_kick")
+
+
+def art_count(order: int) -> int:
+    return 8 if order == 2 else 12
+
+
+def petar_artificial_particles(x, y, z, vx, vy, vz, m, pairs, n_bin: int, G: float, order: int, tt_scale: float,
+                               art_x, art_y, art_z, art_m, elem=None, stream=None) -> None:
+    rc = lib().petar_artificial_particles(*[_ptr(a) for a in (x, y, z, vx, vy, vz, m, pairs)], C.c_int64(n_bin), C.c_double(G),
+                                          C.c_int32(order), C.c_double(tt_scale), *[_ptr(a) for a in (art_x, art_y, art_z, art_m, elem)],
+                                          _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_artificial_particles")
+
+
+def petar_tidal_tensor_fit(acc_x, acc_y, acc_z, elem, n_bin: int, order: int, T, stream=None) -> None:
+    rc = lib().petar_tidal_tensor_fit(_ptr(acc_x), _ptr(acc_y), _ptr(acc_z), _ptr(elem), C.c_int64(n_bin), C.c_int32(order), _ptr(T),
+                                      _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_tidal_tensor_fit")
 
 
 def petar_tree_status(tree, stream=None) -> int:

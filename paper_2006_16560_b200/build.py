@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("PETAR_B200_LIB_OUT", os.path.join(HERE, "libpetar_b200.so"))
-SOURCES = [("build.cu", ["-fmad=false"]), ("walk.cu", ["-fmad=false"]), ("force.cu", []), ("cluster.cu", []), ("short.cu", []), ("api.cu", [])]
+SOURCES = [("build.cu", ["-fmad=false"]), ("walk.cu", ["-fmad=false"]), ("force.cu", []), ("cluster.cu", []), ("short.cu", []), ("artificial.cu", []), ("api.cu", [])]
 COMMON = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 

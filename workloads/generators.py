@@ -247,6 +247,10 @@ def make_workload(config: int, N: int | None = None, seed: int | None = None, th
         m = m[perm2]
         if vel is not None:
             vel = vel[perm2]
+        inv2 = np.empty(n, dtype=np.int64); inv2[perm2] = np.arange(n)
+        pair_idx = np.stack([inv2[0:2 * n_pairs:2], inv2[1:2 * n_pairs:2]], axis=1).astype(np.int32)
+    if kind == "central":
+        pair_idx = np.zeros((0, 2), dtype=np.int32)
     r_out_ref = c["r_out_ref"]
     r_out = np.full(n, r_out_ref) if uniform_radii else changeover_radii(m, r_out_ref)
     return Workload(
@@ -254,7 +258,7 @@ def make_workload(config: int, N: int | None = None, seed: int | None = None, th
         x=np.ascontiguousarray(pos[:, 0]), y=np.ascontiguousarray(pos[:, 1]), z=np.ascontiguousarray(pos[:, 2]),
         m=np.ascontiguousarray(m), r_out=np.ascontiguousarray(r_out),
         theta=float(c["theta"] if theta is None else theta), multipole=c["multipole"], r_out_ref=r_out_ref,
-        meta=dict(config=config, n_pairs=n_pairs, masses=kind),
+        meta=dict(config=config, n_pairs=n_pairs, masses=kind, pairs=pair_idx),     # pairs: member indices of the binaries
         vx=None if vel is None else np.ascontiguousarray(vel[:, 0]),
         vy=None if vel is None else np.ascontiguousarray(vel[:, 1]),
         vz=None if vel is None else np.ascontiguousarray(vel[:, 2]),
