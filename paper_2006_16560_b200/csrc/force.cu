@@ -23,7 +23,9 @@
 // fp32 partial sums live only across one tile slice and are flushed into fp64 accumulators per tile.
 #include "internal.cuh"
 
+#ifndef FT
 #define FT 128                 // threads per CTA
+#endif
 #ifndef SP_REC
 #define SP_REC 2               // staged cells per thread per tile
 #endif
