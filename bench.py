@@ -46,6 +46,9 @@ def parse():
     ap.add_argument("--N", type=int, default=None, help="override the particle count (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-groups", type=int, default=40000, help="i-groups in the oracle's timed sample")
+    ap.add_argument("--theta-sweep", action="store_true",
+                    help="BASELINE.json configs[3]: after the headline run, sweep theta over 0.2, 0.3, 0.5, 0.7 (interactions/s and "
+                         "RMS force error against the direct long-range sum on a 4096-particle subsample, oracle on the host)")
     return ap.parse_args()
 
 
@@ -359,6 +362,36 @@ def main():
             })
         tree.inputs = tuple(dev_in) + (None,)
 
+    # ---- theta sweep (config 4 of BASELINE.json): interactions/s and RMS error vs the DEFINITION -----------------
+    theta_sweep = None
+    if args.theta_sweep and world == 1:
+        import oracle
+        tg = np.sort(np.random.default_rng(44).choice(N, size=min(4096, N), replace=False)).astype(np.int64)
+        dref = oracle.direct(w.x, w.y, w.z, w.m, w.r_out, oracle.OracleParams.from_workload(w), "long", targets=tg)
+        dn = np.sqrt(dref[0] ** 2 + dref[1] ** 2 + dref[2] ** 2)
+        theta_sweep = []
+        for th in (0.2, 0.3, 0.5, 0.7):
+            pt = P.PetarParams.from_workload(w, theta=th)
+            tt = P.Tree(N, pt, device=dev)
+            tt.inputs = tuple(dev_in) + (None,)
+            tt.build(stream)
+            cth = P.petar_long_range_force(tt.handle, tt.acc_x, tt.acc_y, tt.acc_z, tt.pot, True, stream)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ms_th = 0.0
+            for rep in range(3):
+                flush.fill_(rep)
+                a0.record(stream)
+                tt.build(stream)
+                P.petar_long_range_force(tt.handle, tt.acc_x, tt.acc_y, tt.acc_z, tt.pot, False, stream)
+                a1.record(stream); a1.synchronize()
+                ms_th += a0.elapsed_time(a1) / 3
+            g = [v[torch.from_numpy(tg).to(dev)].cpu().numpy() for v in (tt.acc_x, tt.acc_y, tt.acc_z)]
+            rel = np.sqrt(sum((g[k] - dref[k]) ** 2 for k in range(3))) / dn
+            theta_sweep.append(dict(theta=th, interactions=int(cth.n_epep + cth.n_epsp), build_plus_force_ms=ms_th,
+                                    interactions_per_s=(cth.n_epep + cth.n_epsp) / (ms_th * 1e-3),
+                                    rms_rel_force_error_vs_direct_sum=float(np.sqrt(np.mean(rel ** 2))), targets=int(len(tg))))
+            tt.close()
+
     # ---- FP32 peak probe (FFMA only), timed alone ------------------------------------------------------
     scratch = torch.zeros(1, dtype=torch.float32, device=dev)
     P.petar_probe_fp32(20000, scratch, stream)
@@ -434,6 +467,8 @@ def main():
         )
         if next_rows is not None:
             out["next_rows"] = next_rows
+        if theta_sweep is not None:
+            out["theta_sweep"] = theta_sweep
         if not args.no_cpu_baseline and world == 1:
             cb = cpu_oracle_sample(w, args.cpu_groups)
             out["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
