@@ -222,6 +222,9 @@ def test_degenerate_inputs():
         "coincident100": mk(np.tile([[0.5, -0.25, 2.0]], (100, 1)), np.full(100, 0.01), np.full(100, 0.1)),
         "coincident_plus": mk(np.concatenate([np.tile([[0.5, -0.25, 2.0]], (70, 1)), rng.normal(size=(300, 3))]),
                               np.full(370, 1 / 370), np.full(370, 0.05)),
+        # an over-full level-21 leaf larger than both super-group limits (it is its own super-group at every level)
+        "coincident5000_plus": mk(np.concatenate([np.tile([[0.25, 0.5, -1.0]], (5000, 1)), rng.normal(size=(3000, 3))]),
+                                  np.full(8000, 1 / 8000), np.full(8000, 0.05)),
         "zero_mass": mk(rng.normal(size=(200, 3)), np.where(np.arange(200) % 7 == 0, 0.0, 1 / 200), np.full(200, 0.05)),
         "all_zero_mass_cell": mk(np.concatenate([rng.normal(size=(100, 3)), 5 + 0.01 * rng.normal(size=(20, 3))]),
                                  np.concatenate([np.full(100, 0.01), np.zeros(20)]), np.full(120, 0.02)),
