@@ -199,6 +199,16 @@ int petar_artificial_particles(const double* x, const double* y, const double* z
                                double* art_x, double* art_y, double* art_z, double* art_m,
                                double* elem, void* cuda_stream);
 
+/* Orbit-sampling particles (Eq. 29): for binary b, out_*[b * 2 n_split ...] hold n_split samples
+ * of component 1 and then n_split of component 2, at eccentric anomalies E_k = k * 2 pi / n_split (reading P27),
+ * positions by Eq. 32-33 in the orbital frame around the centre of mass, masses m_i dM_k / (2 pi),
+ * dM_k = dE - 2 e cos(E_k) sin(dE / 2).  An unbound pair puts every sample at the centre of mass with mass
+ * m_i / n_split.  1 <= n_split <= 1024 (8 in the paper: "16 particles").  Errors as above.               */
+int petar_orbit_sampling(const double* x, const double* y, const double* z,
+                         const double* vx, const double* vy, const double* vz, const double* m,
+                         const int32_t* pairs, int64_t n_bin, double G, int32_t n_split,
+                         double* out_x, double* out_y, double* out_z, double* out_m, void* cuda_stream);
+
 /* Tidal-tensor coefficients (Eq. 25-26) from the long-range accelerations measured at the artificial particles
  * (acc_*: DEVICE fp64, same layout as art_*): T[b] = M^-1 (A(r_k) - A(r_cm)), M^-1 the generalized inverse of
  * Eq. 28 = the formulas of Table 1 part (1).  T: DEVICE fp64[n_bin][PETAR_TT_COEFFS(order)], order

@@ -7,6 +7,7 @@ P3T-kick and the artificial particles around the long-range force (SURVEY.md 8(f
   * Kepler elements of a pair (a, e and the orbital frame in which Eq. 32 holds)
   * pseudoparticles           Eq. 38 (:473-478): three particles of mass (m1+m2)/3 that carry the orbit-averaged
                               quadrupole of the binary, Eq. 36-37 (:457-470)
+  * orbit-sampling particles  Eq. 29 (:420-428): 2 n_split particles along the two orbits
   * tidal-tensor measure points: 4 at the corners of a regular tetrahedron (2nd order) or 8 at the corners of
                               the paper's "cube" (3rd order), coordinates of Table 1 part (3)
   * tidal-tensor fit          the generalized inverse of Eq. 28 (:404-406): least squares of the polynomial of
@@ -80,6 +81,21 @@ def pseudoparticles(m1, m2, a, e, P, Q, cm):
     loc = s * np.array([[0.0, by], [bx, -0.5 * by], [-bx, -0.5 * by]])
     pos = np.asarray(cm)[None, :] + loc[:, 0:1] * P[None, :] + loc[:, 1:2] * Q[None, :]
     return pos, mt / 3.0
+
+
+def orbit_sampling(m1, m2, a, e, P, Q, cm, n_split):
+    """Orbit-sampling particles (Eq. 29): n_split points per component at equal eccentric-anomaly
+    intervals dE = 2 pi / n_split, E_k = k dE (reading P27: the first sample at the pericentre), masses
+    m_i dM_k / (2 pi) with dM_k = dE - 2 e cos(E_k) sin(dE / 2).  Returns (pos (2 n_split x 3), mass (2 n_split)):
+    the samples of component 1, then those of component 2."""
+    dE = 2.0 * np.pi / n_split
+    E = np.arange(n_split) * dE
+    dM = dE - 2.0 * e * np.cos(E) * np.sin(0.5 * dE)
+    rel = (a * (np.cos(E) - e))[:, None] * P[None, :] + (a * np.sqrt(1.0 - e * e) * np.sin(E))[:, None] * Q[None, :]     # Eq. 32
+    mt = m1 + m2
+    pos = np.concatenate([np.asarray(cm)[None, :] - (m2 / mt) * rel, np.asarray(cm)[None, :] + (m1 / mt) * rel])      # Eq. 33
+    mass = np.concatenate([m1 * dM, m2 * dM]) / (2.0 * np.pi)
+    return pos, mass
 
 
 def tidal_points(order, cm, d_c):

@@ -14,6 +14,6 @@ from .binding import (  # noqa: F401
     petar_set_profiling, petar_stage_times, petar_launch_count, petar_probe_fp32, petar_probe_fp32_mode,
     petar_search_radii, petar_neighbor_list_orbit, petar_clusters_workspace_bytes, petar_clusters,
     petar_short_range_workspace_bytes, petar_short_range_force,
-    petar_kick, petar_artificial_particles, petar_tidal_tensor_fit, art_count,
+    petar_kick, petar_artificial_particles, petar_tidal_tensor_fit, petar_orbit_sampling, art_count,
     STAGE_NAMES,
 )

@@ -14,7 +14,7 @@ EXPORTS = [
     "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32", "petar_probe_fp32_mode",
     "petar_search_radii", "petar_neighbor_list_orbit", "petar_clusters_workspace_bytes", "petar_clusters",
     "petar_short_range_workspace_bytes", "petar_short_range_force",
-    "petar_kick", "petar_artificial_particles", "petar_tidal_tensor_fit",
+    "petar_kick", "petar_artificial_particles", "petar_tidal_tensor_fit", "petar_orbit_sampling",
 ]
 STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units", "walk_super"]
 DBG = dict(HEADER=0, ROOT=1, KEYS=2, PERM=3, NODE_INT=4, NODE_DBL=5, GROUP_INT=6, GROUP_DBL=7, GROUP_CNT=8,
@@ -90,6 +90,8 @@ def lib():
         L.petar_kick.argtypes = [C.c_void_p] * 6 + [C.c_double, C.c_int64, C.c_void_p]
         L.petar_artificial_particles.restype = C.c_int
         L.petar_artificial_particles.argtypes = [C.c_void_p] * 8 + [C.c_int64, C.c_double, C.c_int32, C.c_double] + [C.c_void_p] * 6
+        L.petar_orbit_sampling.restype = C.c_int
+        L.petar_orbit_sampling.argtypes = [C.c_void_p] * 8 + [C.c_int64, C.c_double, C.c_int32] + [C.c_void_p] * 5
         L.petar_tidal_tensor_fit.restype = C.c_int
         L.petar_tidal_tensor_fit.argtypes = [C.c_void_p] * 4 + [C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
         L.petar_tree_status.restype = C.c_int
@@ -221,6 +223,14 @@ def petar_artificial_particles(x, y, z, vx, vy, vz, m, pairs, n_bin: int, G: flo
                                           _stream(stream))
     if rc:
         raise PetarError(rc, "petar_artificial_particles")
+
+
+def petar_orbit_sampling(x, y, z, vx, vy, vz, m, pairs, n_bin: int, G: float, n_split: int, out_x, out_y, out_z, out_m,
+                         stream=None) -> None:
+    rc = lib().petar_orbit_sampling(*[_ptr(a) for a in (x, y, z, vx, vy, vz, m, pairs)], C.c_int64(n_bin), C.c_double(G),
+                                    C.c_int32(n_split), *[_ptr(a) for a in (out_x, out_y, out_z, out_m)], _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_orbit_sampling")
 
 
 def petar_tidal_tensor_fit(acc_x, acc_y, acc_z, elem, n_bin: int, order: int, T, stream=None) -> None:

@@ -27,6 +27,42 @@ extern "C" int petar_kick(double* vx, double* vy, double* vz, const double* ax, 
     return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;
 }
 
+// Kepler elements and orbital frame of a pair (reading P26): P to the pericentre, Q = W x P, W along d x w
+struct BinFrame { double a, e, inv_a, mt, cm[3], P[3], Q[3]; bool bound; };
+__device__ __forceinline__ BinFrame binary_frame(const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
+                                                 const double* __restrict__ vx, const double* __restrict__ vy, const double* __restrict__ vz,
+                                                 const double* __restrict__ m, const int i1, const int i2, const double G) {
+    BinFrame f;
+    const double m1 = m[i1], m2 = m[i2];
+    f.mt = m1 + m2;
+    const double x1[3] = {x[i1], y[i1], z[i1]}, x2[3] = {x[i2], y[i2], z[i2]};
+    const double d[3] = {x2[0] - x1[0], x2[1] - x1[1], x2[2] - x1[2]};
+    const double w[3] = {vx[i2] - vx[i1], vy[i2] - vy[i1], vz[i2] - vz[i1]};
+    for (int k = 0; k < 3; ++k) f.cm[k] = (m1 * x1[k] + m2 * x2[k]) / f.mt;
+    const double mu = G * f.mt;
+    const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    const double v2 = w[0] * w[0] + w[1] * w[1] + w[2] * w[2];
+    const double h[3] = {d[1] * w[2] - d[2] * w[1], d[2] * w[0] - d[0] * w[2], d[0] * w[1] - d[1] * w[0]};
+    const double hn = sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
+    f.inv_a = 2.0 / r - v2 / mu;
+    // eccentricity vector (w x h) / mu - d / r
+    const double ev[3] = {(w[1] * h[2] - w[2] * h[1]) / mu - d[0] / r, (w[2] * h[0] - w[0] * h[2]) / mu - d[1] / r, (w[0] * h[1] - w[1] * h[0]) / mu - d[2] / r};
+    f.e = sqrt(ev[0] * ev[0] + ev[1] * ev[1] + ev[2] * ev[2]);
+    f.bound = f.inv_a > 0.0 && hn > 0.0;
+    f.a = f.bound ? 1.0 / f.inv_a : 0.0;
+    for (int k = 0; k < 3; ++k) { f.P[k] = k == 0; f.Q[k] = k == 1; }
+    if (f.bound) {
+        const double W[3] = {h[0] / hn, h[1] / hn, h[2] / hn};
+        if (f.e > 1e-12) { f.P[0] = ev[0] / f.e; f.P[1] = ev[1] / f.e; f.P[2] = ev[2] / f.e; } else { f.P[0] = d[0] / r; f.P[1] = d[1] / r; f.P[2] = d[2] / r; }
+        const double pw = f.P[0] * W[0] + f.P[1] * W[1] + f.P[2] * W[2];
+        for (int k = 0; k < 3; ++k) f.P[k] -= W[k] * pw;
+        const double pn = sqrt(f.P[0] * f.P[0] + f.P[1] * f.P[1] + f.P[2] * f.P[2]);
+        for (int k = 0; k < 3; ++k) f.P[k] /= pn;
+        f.Q[0] = W[1] * f.P[2] - W[2] * f.P[1]; f.Q[1] = W[2] * f.P[0] - W[0] * f.P[2]; f.Q[2] = W[0] * f.P[1] - W[1] * f.P[0];
+    }
+    return f;
+}
+
 struct ArtArgs {
     const double *x, *y, *z, *vx, *vy, *vz, *m;
     const int* pairs;
@@ -40,50 +76,30 @@ __global__ void __launch_bounds__(128) k_artificial(const ArtArgs A) {
     const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= A.nb) return;
     const int i1 = A.pairs[2 * b], i2 = A.pairs[2 * b + 1];
-    const double m1 = A.m[i1], m2 = A.m[i2], mt = m1 + m2;
-    const double x1[3] = {A.x[i1], A.y[i1], A.z[i1]}, x2[3] = {A.x[i2], A.y[i2], A.z[i2]};
-    const double d[3] = {x2[0] - x1[0], x2[1] - x1[1], x2[2] - x1[2]};
-    const double w[3] = {A.vx[i2] - A.vx[i1], A.vy[i2] - A.vy[i1], A.vz[i2] - A.vz[i1]};
-    double cm[3];
-    for (int k = 0; k < 3; ++k) cm[k] = (m1 * x1[k] + m2 * x2[k]) / mt;
-    const double mu = A.G * mt;
-    const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-    const double v2 = w[0] * w[0] + w[1] * w[1] + w[2] * w[2];
-    const double h[3] = {d[1] * w[2] - d[2] * w[1], d[2] * w[0] - d[0] * w[2], d[0] * w[1] - d[1] * w[0]};
-    const double hn = sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
-    const double inv_a = 2.0 / r - v2 / mu;
-    // eccentricity vector (w x h) / mu - d / r
-    double ev[3] = {(w[1] * h[2] - w[2] * h[1]) / mu - d[0] / r, (w[2] * h[0] - w[0] * h[2]) / mu - d[1] / r, (w[0] * h[1] - w[1] * h[0]) / mu - d[2] / r};
-    const double e = sqrt(ev[0] * ev[0] + ev[1] * ev[1] + ev[2] * ev[2]);
-    const bool bound = inv_a > 0.0 && hn > 0.0;
+    const double m1 = A.m[i1], m2 = A.m[i2];
+    const BinFrame f = binary_frame(A.x, A.y, A.z, A.vx, A.vy, A.vz, A.m, i1, i2, A.G);
+    const double mt = f.mt, e = f.e, a = f.a, inv_a = f.inv_a;
+    const bool bound = f.bound;
+    const double* cm = f.cm;
     const int ntt = A.order == 2 ? 4 : 8;
     const int na = ntt + 4;
     double* ox = A.ox + b * na; double* oy = A.oy + b * na; double* oz = A.oz + b * na; double* om = A.om + b * na;
     for (int k = 0; k < na; ++k) { ox[k] = cm[0]; oy[k] = cm[1]; oz[k] = cm[2]; om[k] = k > ntt ? mt / 3.0 : 0.0; }
-    double a = bound ? 1.0 / inv_a : 0.0, d_c = 0.0;
+    double d_c = 0.0;
     if (bound) {
         d_c = A.tt_scale * a;
         for (int k = 0; k < ntt; ++k) {
             const double* p = A.order == 2 ? c_tt_points2[k] : c_tt_points3[k];
             ox[k] = cm[0] + d_c * p[0]; oy[k] = cm[1] + d_c * p[1]; oz[k] = cm[2] + d_c * p[2];
         }
-        // orbital frame of Eq. 32: W along d x w, P to the pericentre (along d for a circular orbit), Q = W x P
-        const double W[3] = {h[0] / hn, h[1] / hn, h[2] / hn};
-        double P[3];
-        if (e > 1e-12) { P[0] = ev[0] / e; P[1] = ev[1] / e; P[2] = ev[2] / e; } else { P[0] = d[0] / r; P[1] = d[1] / r; P[2] = d[2] / r; }
-        const double pw = P[0] * W[0] + P[1] * W[1] + P[2] * W[2];
-        for (int k = 0; k < 3; ++k) P[k] -= W[k] * pw;
-        const double pn = sqrt(P[0] * P[0] + P[1] * P[1] + P[2] * P[2]);
-        for (int k = 0; k < 3; ++k) P[k] /= pn;
-        const double Q[3] = {W[1] * P[2] - W[2] * P[1], W[2] * P[0] - W[0] * P[2], W[0] * P[1] - W[1] * P[0]};
         // Eq. 38
         const double s = a * sqrt((m1 * m2 / mt) / mt);
         const double bx = sqrt(3.0 * e * e + 0.75), by = sqrt(1.0 - e * e);
         const double lx[3] = {0.0, s * bx, -s * bx}, ly[3] = {s * by, -0.5 * s * by, -0.5 * s * by};
         for (int k = 0; k < 3; ++k) {
-            ox[ntt + 1 + k] = cm[0] + lx[k] * P[0] + ly[k] * Q[0];
-            oy[ntt + 1 + k] = cm[1] + lx[k] * P[1] + ly[k] * Q[1];
-            oz[ntt + 1 + k] = cm[2] + lx[k] * P[2] + ly[k] * Q[2];
+            ox[ntt + 1 + k] = cm[0] + lx[k] * f.P[0] + ly[k] * f.Q[0];
+            oy[ntt + 1 + k] = cm[1] + lx[k] * f.P[1] + ly[k] * f.Q[1];
+            oz[ntt + 1 + k] = cm[2] + lx[k] * f.P[2] + ly[k] * f.Q[2];
         }
     }
     if (A.elem) {
@@ -102,6 +118,44 @@ extern "C" int petar_artificial_particles(const double* x, const double* y, cons
     if (!x || !y || !z || !vx || !vy || !vz || !m || !pairs || !art_x || !art_y || !art_z || !art_m) return PETAR_EINVAL;
     ArtArgs A = {x, y, z, vx, vy, vz, m, pairs, art_x, art_y, art_z, art_m, elem, G, tt_scale, n_bin, order};
     k_artificial<<<cdiv(n_bin, 128), 128, 0, (cudaStream_t)cuda_stream>>>(A);
+    petar_count_launch(1);
+    return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;
+}
+
+// Orbit-sampling particles (Eq. 29; reading P27): n_split samples per component at E_k = k dE
+__global__ void __launch_bounds__(128) k_orbit_sampling(const ArtArgs A, const int n_split) {
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= A.nb) return;
+    const int i1 = A.pairs[2 * b], i2 = A.pairs[2 * b + 1];
+    const double m1 = A.m[i1], m2 = A.m[i2];
+    const BinFrame f = binary_frame(A.x, A.y, A.z, A.vx, A.vy, A.vz, A.m, i1, i2, A.G);
+    const double twopi = 6.283185307179586476925;
+    const double dE = twopi / (double)n_split, shalf = sin(0.5 * dE), by = sqrt(fmax(0.0, 1.0 - f.e * f.e));
+    double* ox = A.ox + b * 2 * n_split; double* oy = A.oy + b * 2 * n_split; double* oz = A.oz + b * 2 * n_split; double* om = A.om + b * 2 * n_split;
+    for (int k = 0; k < n_split; ++k) {
+        double rel[3] = {0.0, 0.0, 0.0}, dM = dE;
+        if (f.bound) {
+            double sE, cE;
+            sincos((double)k * dE, &sE, &cE);
+            dM = dE - 2.0 * f.e * cE * shalf;
+            const double lx = f.a * (cE - f.e), ly = f.a * by * sE;                       // Eq. 32
+            for (int c = 0; c < 3; ++c) rel[c] = lx * f.P[c] + ly * f.Q[c];
+        }
+        const double q1 = m2 / f.mt, q2 = m1 / f.mt;                                         // Eq. 33
+        ox[k] = f.cm[0] - q1 * rel[0]; oy[k] = f.cm[1] - q1 * rel[1]; oz[k] = f.cm[2] - q1 * rel[2];
+        ox[n_split + k] = f.cm[0] + q2 * rel[0]; oy[n_split + k] = f.cm[1] + q2 * rel[1]; oz[n_split + k] = f.cm[2] + q2 * rel[2];
+        om[k] = m1 * dM / twopi; om[n_split + k] = m2 * dM / twopi;
+    }
+}
+
+extern "C" int petar_orbit_sampling(const double* x, const double* y, const double* z, const double* vx, const double* vy,
+                                    const double* vz, const double* m, const int32_t* pairs, int64_t n_bin, double G,
+                                    int32_t n_split, double* out_x, double* out_y, double* out_z, double* out_m, void* cuda_stream) {
+    if (n_bin < 0 || n_split < 1 || n_split > 1024 || !(G > 0.0)) return PETAR_EINVAL;
+    if (n_bin == 0) return PETAR_OK;
+    if (!x || !y || !z || !vx || !vy || !vz || !m || !pairs || !out_x || !out_y || !out_z || !out_m) return PETAR_EINVAL;
+    ArtArgs A = {x, y, z, vx, vy, vz, m, pairs, out_x, out_y, out_z, out_m, nullptr, G, 1.0, n_bin, 2};
+    k_orbit_sampling<<<cdiv(n_bin, 128), 128, 0, (cudaStream_t)cuda_stream>>>(A, n_split);
     petar_count_launch(1);
     return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;
 }

@@ -163,3 +163,34 @@ def test_artificial_particles_through_the_long_range_force():
     # trace condition holds.)  The measured differences A(r_k) - A(r_cm) are ~d_c/R of the fp32-accurate accelerations: percent-level agreement
     assert np.median(rel) < 0.05
     t.close()
+
+
+def test_orbit_sampling():
+    import torch
+    P = _P()
+    w = make_workload(2, N=20000, velocities=True)
+    pairs = np.concatenate([w.meta["pairs"][:3000], [[0, w.N - 1]]]).astype(np.int32)       # + one unbound pair
+    nb, ns = len(pairs), 8
+    ins = [_dev(q) for q in (w.x, w.y, w.z, w.vx, w.vy, w.vz, w.m)]
+    out = [torch.empty(nb * 2 * ns, dtype=torch.float64, device="cuda") for _ in range(4)]
+    P.petar_orbit_sampling(*ins, _dev(pairs), nb, w.G, ns, *out)
+    gx, gy, gz, gm = (o.cpu().numpy().reshape(nb, 2 * ns) for o in out)
+    for b in range(0, nb, 13):
+        i, j = pairs[b]
+        x1 = np.array([w.x[i], w.y[i], w.z[i]]); x2 = np.array([w.x[j], w.y[j], w.z[j]])
+        v1 = np.array([w.vx[i], w.vy[i], w.vz[i]]); v2 = np.array([w.vx[j], w.vy[j], w.vz[j]])
+        el = A.kepler_elements(x2 - x1, v2 - v1, w.G * (w.m[i] + w.m[j]))
+        cm = (w.m[i] * x1 + w.m[j] * x2) / (w.m[i] + w.m[j])
+        assert el["bound"]
+        pos, mass = A.orbit_sampling(w.m[i], w.m[j], el["a"], el["e"], el["P"], el["Q"], cm, ns)
+        g = np.stack([gx[b], gy[b], gz[b]], axis=1)
+        tol = 1e-9 if el["e"] > 1e-3 else 1e-6
+        assert np.max(np.abs(g - pos)) < tol * el["a"] + 1e-15 * np.abs(cm).max()
+        assert np.allclose(gm[b], mass, rtol=1e-12)
+    # every binary keeps its mass; the unbound pair sits at its centre of mass
+    assert np.allclose(gm.sum(axis=1), w.m[pairs[:, 0]] + w.m[pairs[:, 1]], rtol=1e-13)
+    b = nb - 1
+    cm = (w.m[0] * np.array([w.x[0], w.y[0], w.z[0]]) + w.m[-1] * np.array([w.x[-1], w.y[-1], w.z[-1]])) / (w.m[0] + w.m[-1])
+    assert np.allclose(np.stack([gx[b], gy[b], gz[b]], axis=1), cm)
+    with pytest.raises(P.PetarError):
+        P.petar_orbit_sampling(*ins, _dev(pairs), nb, w.G, 0, *out)

@@ -143,3 +143,25 @@ def test_kepler_elements_and_artificial_particles():
     art = A.artificial_particles([0, 0, 0], [0, 0, 0], 1.0, [1, 0, 0], [0, 5.0, 0], 1.0, 1.0, 2, 2.0)
     assert not art["bound"] and np.allclose(art["pos"], art["cm"])
     assert np.array_equal(A.kick(np.array([1.0, 2.0]), np.array([0.5, -1.0]), 0.25), np.array([1.125, 1.75]))
+
+
+@pytest.mark.parametrize("e", [0.0, 0.5, 0.9])
+def test_orbit_sampling_eq29(e):
+    m1, m2, a = 0.7, 0.2, 1.3
+    P, Q, cm = np.array([1.0, 0, 0]), np.array([0, 1.0, 0]), np.array([0.3, -0.2, 0.1])
+    pos, mass = A.orbit_sampling(m1, m2, a, e, P, Q, cm, 8)
+    assert pos.shape == (16, 3)                                              # "dE = pi/4, 16 particles"
+    # the mean-anomaly intervals tile the orbit: the samples of a component carry exactly its mass
+    assert mass[:8].sum() == pytest.approx(m1, rel=1e-14) and mass[8:].sum() == pytest.approx(m2, rel=1e-14)
+    # Eq. 29's two forms agree: dE - e [sin(E + dE/2) - sin(E - dE/2)] = dE - 2 e cos E sin(dE/2)
+    dE = np.pi / 4; E = np.arange(8) * dE
+    assert np.allclose(mass[:8] * 2 * np.pi / m1, dE - e * (np.sin(E + dE / 2) - np.sin(E - dE / 2)), rtol=1e-13)
+    # no dipole about the centre of mass pair by pair, and the sampled quadrupole converges to Eq. 36
+    assert np.allclose(m1 * (pos[:8] - cm) + m2 * (pos[8:] - cm), 0, atol=1e-15)
+    mu = m1 * m2 / (m1 + m2)
+    eq36 = mu * a * a * np.diag([2 * e * e + 0.5, 0.5 - 0.5 * e * e, 0.0])
+    errs = []
+    for n in (8, 64):
+        p_, m_ = A.orbit_sampling(m1, m2, a, e, P, Q, np.zeros(3), n)
+        errs.append(np.abs(np.einsum("n,ni,nj->ij", m_, p_, p_) - eq36).max())
+    assert errs[1] < 1e-2 * mu * a * a and errs[1] <= errs[0] + 1e-15
