@@ -326,8 +326,8 @@ def main():
             "clusters_ms": acc[3], "n_clusters": n_cl, "clusters_algorithmic_gbs": cl_bytes / (acc[3] * 1e-3) / 1e9 if acc[3] > 0 else None,
             "clusters_frac_of_hbm": cl_bytes / (acc[3] * 1e-3) / 1e9 / hbm if acc[3] > 0 else None,
             "short_range_force_ms": acc[4],
-            "short_range_algorithmic_gbs": (112.0 * N + 8.0 * (N + 1) + 68.0 * tot_o) / (acc[4] * 1e-3) / 1e9 if acc[4] > 0 else None,
-            "short_range_frac_of_hbm": (112.0 * N + 8.0 * (N + 1) + 68.0 * tot_o) / (acc[4] * 1e-3) / 1e9 / hbm if acc[4] > 0 else None,
+            "short_range_algorithmic_gbs": (240.0 * N + 8.0 * (N + 1) + 68.0 * tot_o) / (acc[4] * 1e-3) / 1e9 if acc[4] > 0 else None,
+            "short_range_frac_of_hbm": (240.0 * N + 8.0 * (N + 1) + 68.0 * tot_o) / (acc[4] * 1e-3) / 1e9 / hbm if acc[4] > 0 else None,
         }
         # rank 3: kick, artificial particles of every binary (3rd-order measure points + pseudoparticles), tensor fit
         pairs = wv.meta["pairs"]

@@ -6,14 +6,19 @@
 // Rows are short (the binary companion, rarely a few more) with a few very long ones (a massive
 // particle): rows of up to SHORT_ROW entries are summed by one thread in list order; longer rows are
 // queued and summed by one warp each (lanes take entries lane, lane+32, ..., then a fixed-order
-// shuffle reduction), so every result is deterministic.  HBM-bound: 56 B read + 56 B written per
-// particle and 64 B gathered per list entry.
+// shuffle reduction), so every result is deterministic.  HBM-bound: the inputs are first packed into one
+// 64-byte record per particle (64 B read + 64 B written), then 64 B read + 56 B written per particle and one
+// 64-byte record gathered per list entry.
 #include "internal.cuh"
 
 #define SHORT_ROW 32
 
+// packed copy of the inputs: one 64-byte record per particle, so a gathered neighbour costs two sectors, not eight
+struct __align__(16) ShortRec { double x, y, z, vx, vy, vz, m, rout; };
+
 struct ShortArgs {
     const double *x, *y, *z, *vx, *vy, *vz, *m, *rout;
+    const ShortRec* rec;
     const long long* offsets; const int* indices;
     double *ax, *ay, *az, *jx, *jy, *jz, *pot;
     double G, rho, lam, q;
@@ -24,11 +29,13 @@ struct Sum7 { double a0, a1, a2, j0, j1, j2, p; };
 
 __device__ __forceinline__ void short_pair(const ShortArgs& A, const double xi, const double yi, const double zi, const double vxi,
                                            const double vyi, const double vzi, const double ri, const int j, Sum7& s) {
-    const double dx = xi - A.x[j], dy = yi - A.y[j], dz = zi - A.z[j];
-    const double wx = vxi - A.vx[j], wy = vyi - A.vy[j], wz = vzi - A.vz[j];
+    const double2* rp = reinterpret_cast<const double2*>(&A.rec[j]);
+    const double2 q0 = rp[0], q1 = rp[1], q2 = rp[2], q3 = rp[3];         // (x, y) (z, vx) (vy, vz) (m, rout)
+    const double dx = xi - q0.x, dy = yi - q0.y, dz = zi - q1.x;
+    const double wx = vxi - q1.y, wy = vyi - q2.x, wz = vzi - q2.y;
     const double r2 = dx * dx + dy * dy + dz * dz;
     const double r = sqrt(r2);
-    const double R = fmax(ri, A.rout[j]);
+    const double R = fmax(ri, q3.y);
     if (r == 0.0 || r >= R) return;
     const double rin = A.rho * R;
     const double xx = (r - rin) / (R - rin);
@@ -42,7 +49,7 @@ __device__ __forceinline__ void short_pair(const ShortArgs& A, const double xi, 
     } else {
         W = A.lam * (1.0 - 2.0 * xx);                                                                    // x <= 0, unclamped (reading P4)
     }
-    const double mj = A.m[j];
+    const double mj = q3.x;
     const double dw = dx * wx + dy * wy + dz * wz;
     const double r3 = r2 * r;
     const double xdot = dw / (r * (R - rin));
@@ -57,6 +64,13 @@ __device__ __forceinline__ void short_store(const ShortArgs& A, const long long 
     if (A.ax) A.ax[i] = s.a0; if (A.ay) A.ay[i] = s.a1; if (A.az) A.az[i] = s.a2;
     if (A.jx) A.jx[i] = s.j0; if (A.jy) A.jy[i] = s.j1; if (A.jz) A.jz[i] = s.j2;
     if (A.pot) A.pot[i] = s.p;
+}
+
+__global__ void __launch_bounds__(256) k_short_pack(const ShortArgs A, ShortRec* __restrict__ rec) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= A.n) return;
+    ShortRec r = {A.x[i], A.y[i], A.z[i], A.vx[i], A.vy[i], A.vz[i], A.m[i], A.rout[i]};
+    rec[i] = r;
 }
 
 // queue[0] = number of long rows, queue[1..] = their particle indices
@@ -92,7 +106,8 @@ __global__ void __launch_bounds__(256) k_short_long_rows(const ShortArgs A, cons
     }
 }
 
-extern "C" size_t petar_short_range_workspace_bytes(int64_t N) { return N < 0 ? 0 : ((size_t)(N + 1) * 4 + 255) / 256 * 256; }
+static size_t short_queue_bytes(int64_t N) { return ((size_t)(N + 1) * 4 + 255) / 256 * 256; }
+extern "C" size_t petar_short_range_workspace_bytes(int64_t N) { return N < 0 ? 0 : short_queue_bytes(N) + (size_t)N * sizeof(ShortRec); }
 
 extern "C" int petar_short_range_force(const double* x, const double* y, const double* z, const double* vx, const double* vy, const double* vz,
                                        const double* m, const double* r_out, const int64_t* offsets, const int32_t* indices, int64_t N,
@@ -111,11 +126,15 @@ extern "C" int petar_short_range_force(const double* x, const double* y, const d
     A.G = G; A.rho = r_in_over_r_out; A.lam = (1.0 - r_in_over_r_out) / (1.0 + r_in_over_r_out);
     A.q = r_in_over_r_out / (1.0 - r_in_over_r_out); A.n = N;
     int* queue = (int*)workspace;
+    ShortRec* rec = (ShortRec*)((char*)workspace + short_queue_bytes(N));
+    A.rec = rec;
     if (cudaMemsetAsync(queue, 0, 4, s) != cudaSuccess) return PETAR_ECUDA;
+    k_short_pack<<<cdiv(N, 256), 256, 0, s>>>(A, rec);
+    KCHECK(s, "k_short_pack");
     k_short_rows<<<cdiv(N, 256), 256, 0, s>>>(A, queue);
     KCHECK(s, "k_short_rows");
     k_short_long_rows<<<148 * 4, 256, 0, s>>>(A, queue);
     KCHECK(s, "k_short_long_rows");
-    petar_count_launch(2);
+    petar_count_launch(3);
     return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;
 }
