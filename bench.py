@@ -479,8 +479,15 @@ def main():
         if theta_sweep is not None:
             out["theta_sweep"] = theta_sweep
         if not args.no_cpu_baseline and world == 1:
+            import oracle
             cb = cpu_oracle_sample(w, args.cpu_groups)
             out["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+            ncores = oracle.num_threads()
+            oracle.set_num_threads(1)                      # the same oracle on ONE core, on a 16 times smaller sample
+            c1 = cpu_oracle_sample(w, max(50, args.cpu_groups // 16), seed=2)
+            oracle.set_num_threads(ncores)
+            out["cpu_baseline"]["single_thread_value"] = c1["value"]
+            out["cpu_baseline"]["single_thread_sample"] = c1["sample"]
         print(json.dumps(out), flush=True)
     if dist:
         dist.barrier()

@@ -6,6 +6,6 @@ fp64, built with gcc at first use) through ctypes and imports nothing from the C
 """
 from . import artificial  # noqa: F401  (part (E): kick, pseudoparticles, tidal tensors; numpy)
 from .binding import (  # noqa: F401
-    OracleParams, OracleTree, K, W, f, direct, neighbors_direct, build_library, num_threads,
+    OracleParams, OracleTree, K, W, f, direct, neighbors_direct, build_library, num_threads, set_num_threads,
     search_radii, pericentre, neighbors_orbit_direct, clusters, dK, short_range,
 )

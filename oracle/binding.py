@@ -80,6 +80,11 @@ def f(x, lam):
     return _lib().ora_f(float(x), float(lam))
 
 
+def set_num_threads(n: int) -> None:
+    """Number of OpenMP threads of the following calls (bench.py's single-thread baseline)."""
+    _lib().ora_set_num_threads(C.c_int(int(n)))
+
+
 def num_threads() -> int:
     return int(_lib().ora_num_threads())
 

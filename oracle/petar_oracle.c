@@ -791,6 +791,14 @@ void ora_short_range(int64_t N, const double *x, const double *y, const double *
     }
 }
 
+void ora_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int ora_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();
