@@ -92,6 +92,7 @@ static size_t carve(Workspace* w, char* base, int64_t N, const petar_params* p) 
     W->units = (ForceUnit*)take((size_t)W->unit_cap * sizeof(ForceUnit));
     W->part = (double*)take((size_t)PETAR_NSUP * n * 4 * 8);
     W->nb_cnt = (int*)take(n * 4);
+    W->nb_queue = (int*)take(((size_t)W->group_cap + 1) * 4);
     W->exp_scratch = (int*)take((10 * (n + 1) + 8) * 4);
     long long chunks = arena_chunks_for(N, p);
     W->arena_chunks = (int)chunks;

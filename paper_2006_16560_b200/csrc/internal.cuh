@@ -121,6 +121,7 @@ struct Workspace {
     int* arena; int arena_chunks;
     // neighbour temporaries
     int* nb_cnt;                   // [N] counts in caller's order
+    int* nb_queue;                 // [group_cap + 1] groups with a long near list (k_neighbors_big)
     int* exp_scratch;              // [10 (N+1) + 8] list-export scratch (tests)
 };
 

@@ -448,7 +448,8 @@ cudaError_t launch_walk(petar_tree* t, cudaStream_t s) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// S9: neighbours.  One warp per group; lanes own i-particles; j runs over the NEAR EP ranges only
+// S9: neighbours.  One warp per group (one CTA for the few groups with a very long near list); lanes own
+// i-particles; j runs over the NEAR EP ranges only
 // (a leaf that is not near has every pair at r >= R_ij, rule O7), fp64 test of rule O9.
 // Pass 1 counts into cnt[original index]; pass 2 (after the scan) fills.
 // ------------------------------------------------------------------------------------------------
@@ -471,15 +472,91 @@ __device__ __forceinline__ double pericentre(double dx, double dy, double dz, do
 // kept iff the pair is inside its changeover radius or r_p < C_V min(r_nb,i, r_nb,j).
 struct OrbitArgs { const double *vxs, *vys, *vzs, *ms, *routs; double G, Cv; };
 
+struct NbArgs {
+    const int* arena; const unsigned* perm;
+    const double *xs, *ys, *zs, *rss;
+    int* cnt; const long long* offsets; int* indices; long long capacity;
+    OrbitArgs oa;
+};
+struct NbTile { double x[32], y[32], z[32], r[32]; int j[32]; };
+
+// One warp, one block of <= 32 i-particles (lane = particle) of group gr, against the blocks of 32 leaf ranges
+// number wsel, wsel + nwarps, ... of the group's near list.  The particles of 32 ranges are flattened (warp scan +
+// search), staged 32 at a time in shared memory with one coalesced load per array, then tested by every lane.
+// Returns the lane's count; FILL writes the kept neighbours from position o on.
 template <bool FILL, bool ORBIT>
-__global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
-                                                   const unsigned* __restrict__ perm,
-                                                   const double* __restrict__ xs, const double* __restrict__ ys, const double* __restrict__ zs,
-                                                   const double* __restrict__ rss, int* __restrict__ cnt,
-                                                   const long long* __restrict__ offsets, int* __restrict__ indices, long long capacity,
-                                                   const OrbitArgs oa) {
-    __shared__ double s_x[8][32], s_y[8][32], s_z[8][32], s_r[8][32];
-    __shared__ int s_j[8][32];
+__device__ __forceinline__ int nb_sweep(const NbArgs& A, const GroupRec& gr, const int i, const bool vi, const long long o,
+                                        const int lane, NbTile& tl, const int wsel, const int nwarps) {
+    double xi = 0, yi = 0, zi = 0, ri = 0;
+    double vxi = 0, vyi = 0, vzi = 0, mi = 0, roi = 0;
+    if (vi) {
+        xi = A.xs[i]; yi = A.ys[i]; zi = A.zs[i]; ri = A.rss[i];
+        if (ORBIT) { vxi = A.oa.vxs[i]; vyi = A.oa.vys[i]; vzi = A.oa.vzs[i]; mi = A.oa.ms[i]; roi = A.oa.routs[i]; }
+    }
+    int c = 0, blk = 0;
+    int chunk = gr.head_epn;
+    int remaining = gr.n_epn * 2;       // entries
+    while (chunk >= 0 && remaining > 0) {
+        const int* cp = A.arena + (size_t)chunk * PETAR_CHUNK;
+        const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+        for (int e0 = 0; e0 < ne; e0 += 64, ++blk) {
+            if (blk % nwarps != wsel) continue;
+            int jb_l = 0, cnt_l = 0;
+            if (e0 + 2 * lane < ne) { const int2 be = *reinterpret_cast<const int2*>(cp + PETAR_CHUNK_HDR + e0 + 2 * lane); jb_l = be.x; cnt_l = be.y - be.x; }
+            int incl = cnt_l;
+#pragma unroll
+            for (int o2 = 1; o2 < 32; o2 <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o2); if (lane >= o2) incl += v; }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            const int excl = incl - cnt_l;
+            for (int p0 = 0; p0 < total; p0 += 32) {
+                const int p = p0 + lane;
+                int lo = 0;                               // smallest range whose inclusive count exceeds p
+#pragma unroll
+                for (int step = 16; step > 0; step >>= 1) { const int v = __shfl_sync(0xffffffffu, incl, lo + step - 1); if (v <= p) lo += step; }
+                lo = min(lo, 31);
+                const int rjb = __shfl_sync(0xffffffffu, jb_l, lo), rex = __shfl_sync(0xffffffffu, excl, lo);
+                __syncwarp();
+                if (p < total) {
+                    const int j = rjb + (p - rex);
+                    tl.x[lane] = A.xs[j]; tl.y[lane] = A.ys[j]; tl.z[lane] = A.zs[j]; tl.r[lane] = A.rss[j]; tl.j[lane] = j;
+                }
+                __syncwarp();
+                const int nb = min(32, total - p0);
+                for (int k = 0; k < nb; ++k) {
+                    const int j = tl.j[k];
+                    const double xj = tl.x[k], yj = tl.y[k], zj = tl.z[k], rj = tl.r[k];
+                    double dx = xi - xj, dy = yi - yj, dz = zi - zj;
+                    double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+                    double R = fmax(ri, rj);
+                    bool keep = vi && j != i && r2 < R * R;
+                    if (ORBIT && keep) {
+                        const double Ro = fmax(roi, A.oa.routs[j]);
+                        if (!(r2 < Ro * Ro)) {
+                            const double rp = pericentre(dx, dy, dz, r2, vxi - A.oa.vxs[j], vyi - A.oa.vys[j], vzi - A.oa.vzs[j], A.oa.G * (mi + A.oa.ms[j]));
+                            keep = rp < A.oa.Cv * fmin(ri, rj);
+                        }
+                    }
+                    if (keep) {
+                        if (FILL) { if (o + c < A.capacity) A.indices[o + c] = (int)A.perm[j]; }
+                        ++c;
+                    }
+                }
+            }
+        }
+        remaining -= ne;
+        chunk = cp[0];
+    }
+    return c;
+}
+
+// groups whose near list is long (a massive particle's r_out reaches thousands of others) go to k_neighbors_big
+#define NB_BIG_WORK 32768
+__device__ __forceinline__ bool nb_is_big(const GroupRec& gr) { return (long long)gr.n_epn_part * (long long)(gr.end - gr.begin) > NB_BIG_WORK; }
+
+// One warp per group.  queue[0] = number of big groups, queue[1..] = their ids (filled by the count pass).
+template <bool FILL, bool ORBIT>
+__global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const NbArgs A, int* __restrict__ queue) {
+    __shared__ NbTile s_tile[8];
     const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
     const int ng = h->n_groups;
     for (;;) {
@@ -488,72 +565,49 @@ __global__ void __launch_bounds__(256) k_neighbors(DevHeader* __restrict__ h, co
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g >= ng) break;
         const GroupRec gr = grp[g];
+        if (nb_is_big(gr)) {
+            if (!FILL && lane == 0) queue[1 + atomicAdd(&queue[0], 1)] = g;
+            continue;
+        }
         for (int ib = gr.begin; ib < gr.end; ib += 32) {
             const int i = ib + lane;
             const bool vi = i < gr.end;
-            double xi = 0, yi = 0, zi = 0, ri = 0;
-            double vxi = 0, vyi = 0, vzi = 0, mi = 0, roi = 0;
             unsigned oi = 0;
             long long o = 0;
-            if (vi) {
-                xi = xs[i]; yi = ys[i]; zi = zs[i]; ri = rss[i]; oi = perm[i]; if (FILL) o = offsets[oi];
-                if (ORBIT) { vxi = oa.vxs[i]; vyi = oa.vys[i]; vzi = oa.vzs[i]; mi = oa.ms[i]; roi = oa.routs[i]; }
+            if (vi) { oi = A.perm[i]; if (FILL) o = A.offsets[oi]; }
+            const int c = nb_sweep<FILL, ORBIT>(A, gr, i, vi, o, lane, s_tile[wp], 0, 1);
+            if (!FILL && vi) A.cnt[oi] = c;
+        }
+    }
+}
+
+// One CTA (8 warps) per big group: the warps share out the blocks of 32 leaf ranges.  Every warp counts its share
+// first, so the rows are filled at fixed positions (warp 0's neighbours, then warp 1's, ...): deterministic.
+template <bool FILL, bool ORBIT>
+__global__ void __launch_bounds__(256) k_neighbors_big(const GroupRec* __restrict__ grp, const NbArgs A, const int* __restrict__ queue) {
+    __shared__ NbTile s_tile[8];
+    __shared__ int s_cnt[8][32];
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    const int nq = queue[0];
+    for (int q = blockIdx.x; q < nq; q += gridDim.x) {
+        const GroupRec gr = grp[queue[1 + q]];
+        for (int ib = gr.begin; ib < gr.end; ib += 32) {
+            const int i = ib + lane;
+            const bool vi = i < gr.end;
+            unsigned oi = 0;
+            long long o = 0;
+            if (vi) { oi = A.perm[i]; if (FILL) o = A.offsets[oi]; }
+            __syncthreads();                                     // s_cnt of the previous block consumed
+            s_cnt[wp][lane] = nb_sweep<false, ORBIT>(A, gr, i, vi, 0, lane, s_tile[wp], wp, 8);
+            __syncthreads();
+            if (FILL) {
+                for (int w2 = 0; w2 < wp; ++w2) o += s_cnt[w2][lane];
+                nb_sweep<true, ORBIT>(A, gr, i, vi, o, lane, s_tile[wp], wp, 8);
+            } else if (wp == 0 && vi) {
+                int c = 0;
+                for (int w2 = 0; w2 < 8; ++w2) c += s_cnt[w2][lane];
+                A.cnt[oi] = c;
             }
-            int c = 0;
-            int chunk = gr.head_epn;
-            int remaining = gr.n_epn * 2;       // entries
-            while (chunk >= 0 && remaining > 0) {
-                const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
-                const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
-                // 32 leaf ranges at a time: their particles are flattened (warp scan + search), staged 32 at a
-                // time in shared memory with one coalesced load per array, then tested by every lane
-                for (int e0 = 0; e0 < ne; e0 += 64) {
-                    int jb_l = 0, cnt_l = 0;
-                    if (e0 + 2 * lane < ne) { const int2 be = *reinterpret_cast<const int2*>(cp + PETAR_CHUNK_HDR + e0 + 2 * lane); jb_l = be.x; cnt_l = be.y - be.x; }
-                    int incl = cnt_l;
-#pragma unroll
-                    for (int o2 = 1; o2 < 32; o2 <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o2); if (lane >= o2) incl += v; }
-                    const int total = __shfl_sync(0xffffffffu, incl, 31);
-                    const int excl = incl - cnt_l;
-                    for (int p0 = 0; p0 < total; p0 += 32) {
-                        const int p = p0 + lane;
-                        int lo = 0;                               // smallest range whose inclusive count exceeds p
-#pragma unroll
-                        for (int step = 16; step > 0; step >>= 1) { const int v = __shfl_sync(0xffffffffu, incl, lo + step - 1); if (v <= p) lo += step; }
-                        lo = min(lo, 31);
-                        const int rjb = __shfl_sync(0xffffffffu, jb_l, lo), rex = __shfl_sync(0xffffffffu, excl, lo);
-                        __syncwarp();
-                        if (p < total) {
-                            const int j = rjb + (p - rex);
-                            s_x[wp][lane] = xs[j]; s_y[wp][lane] = ys[j]; s_z[wp][lane] = zs[j]; s_r[wp][lane] = rss[j]; s_j[wp][lane] = j;
-                        }
-                        __syncwarp();
-                        const int nb = min(32, total - p0);
-                        for (int k = 0; k < nb; ++k) {
-                            const int j = s_j[wp][k];
-                            const double xj = s_x[wp][k], yj = s_y[wp][k], zj = s_z[wp][k], rj = s_r[wp][k];
-                            double dx = xi - xj, dy = yi - yj, dz = zi - zj;
-                            double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                            double R = fmax(ri, rj);
-                            bool keep = vi && j != i && r2 < R * R;
-                            if (ORBIT && keep) {
-                                const double Ro = fmax(roi, oa.routs[j]);
-                                if (!(r2 < Ro * Ro)) {
-                                    const double rp = pericentre(dx, dy, dz, r2, vxi - oa.vxs[j], vyi - oa.vys[j], vzi - oa.vzs[j], oa.G * (mi + oa.ms[j]));
-                                    keep = rp < oa.Cv * fmin(ri, rj);
-                                }
-                            }
-                            if (keep) {
-                                if (FILL) { if (o + c < capacity) indices[o + c] = (int)perm[j]; }
-                                ++c;
-                            }
-                        }
-                    }
-                }
-                remaining -= ne;
-                chunk = cp[0];
-            }
-            if (!FILL && vi) cnt[oi] = c;
         }
     }
 }
@@ -584,29 +638,32 @@ cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, 
     const long long n = t->N;
     const double* rss = t->r_search ? w.rss : w.routs;
     const bool orbit = vx != nullptr;
-    OrbitArgs oa = {w.vxs, w.vys, w.vzs, w.ms, w.routs, t->p.G, Cv};
+    NbArgs A = {w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, nullptr, nullptr, 0, {w.vxs, w.vys, w.vzs, w.ms, w.routs, t->p.G, Cv}};
     stage_begin(t, s);
-    int grid = t->sm_count * 8;
+    const int grid = t->sm_count * 8, grid_big = t->sm_count;
     if (orbit) {
         k_gather_vel<<<cdiv(n, 256), 256, 0, s>>>(w.idx, n, vx, vy, vz, w.vxs, w.vys, w.vzs);
         KCHECK(s, "k_gather_vel");
         petar_count_launch(1);
     }
+    cudaError_t e = cudaMemsetAsync(w.nb_queue, 0, 4, s);
+    if (e != cudaSuccess) return e;
     k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 1);
     KCHECK(s, "k_reset_ticket");
-    if (orbit) k_neighbors<false, true><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, nullptr, nullptr, 0, oa);
-    else k_neighbors<false, false><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, nullptr, nullptr, 0, oa);
+    if (orbit) { k_neighbors<false, true><<<grid, 256, 0, s>>>(w.hdr, w.grp, A, w.nb_queue); k_neighbors_big<false, true><<<grid_big, 256, 0, s>>>(w.grp, A, w.nb_queue); }
+    else { k_neighbors<false, false><<<grid, 256, 0, s>>>(w.hdr, w.grp, A, w.nb_queue); k_neighbors_big<false, false><<<grid_big, 256, 0, s>>>(w.grp, A, w.nb_queue); }
     KCHECK(s, "k_neighbors");
-    petar_count_launch(2);
-    cudaError_t e = launch_scan_i32_to_i64(w.nb_cnt, (long long*)offsets, n, (long long*)w.scan_tmp, s);
+    petar_count_launch(3);
+    e = launch_scan_i32_to_i64(w.nb_cnt, (long long*)offsets, n, (long long*)w.scan_tmp, s);
     if (e != cudaSuccess) return e;
     if (indices) {
+        A.offsets = (const long long*)offsets; A.indices = indices; A.capacity = capacity;
         k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 1);
         KCHECK(s, "k_reset_ticket");
-        if (orbit) k_neighbors<true, true><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, (const long long*)offsets, indices, capacity, oa);
-        else k_neighbors<true, false><<<grid, 256, 0, s>>>(w.hdr, w.grp, w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, (const long long*)offsets, indices, capacity, oa);
+        if (orbit) { k_neighbors<true, true><<<grid, 256, 0, s>>>(w.hdr, w.grp, A, w.nb_queue); k_neighbors_big<true, true><<<grid_big, 256, 0, s>>>(w.grp, A, w.nb_queue); }
+        else { k_neighbors<true, false><<<grid, 256, 0, s>>>(w.hdr, w.grp, A, w.nb_queue); k_neighbors_big<true, false><<<grid_big, 256, 0, s>>>(w.grp, A, w.nb_queue); }
         KCHECK(s, "k_neighbors");
-        petar_count_launch(2);
+        petar_count_launch(3);
     }
     k_nb_status<<<1, 32, 0, s>>>((const long long*)offsets, n, capacity, status_dev, w.hdr, indices ? 1 : 0);
     KCHECK(s, "k_nb_status");
