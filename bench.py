@@ -434,6 +434,14 @@ def main():
     e2e_value = tot_inter / (e2e_ms * 1e-3)
 
     stage_ms = {k: v / K for k, v in stage_sum.items()}
+    # HBM-side stages: algorithmic bytes per particle against the measured copy bandwidth
+    hbm_peak = float(pk.get("hbm_gbs", 6545.6))
+    stage_bytes = {"bbox_keys": 36.0, "sort": 256.0, "gather": 116.0, "tree": 20.0, "moments": 115.0, "groups": 40.0}
+    hbm_stages = {}
+    for name, bpp in stage_bytes.items():
+        if stage_ms.get(name, 0.0) > 0.0:
+            gbs = bpp * N / (stage_ms[name] * 1e-3) / 1e9
+            hbm_stages[name] = dict(ms=stage_ms[name], bytes_per_particle=bpp, achieved_gbs=gbs, frac_of_hbm=gbs / hbm_peak)
     kern = [dict(kernel="k_force_units", ms=stage_ms["force_units"], flops_per_launch=float(flops_units)),
             dict(kernel="k_force", ms=stage_ms["force"], flops_per_launch=float(flops_groups))]
     for kd in kern:
@@ -457,6 +465,9 @@ def main():
                     "n_epep_changeover": int(counts.n_epep_near), "neighbours": nb_total, "n_groups": int(counts.n_groups),
                     "n_nodes": int(counts.n_nodes), "status": status, "multi_gpu": "replicas only (no data-path collective)"},
             stage_ms=stage_ms,
+            hbm_stages=dict(peak_gbs=hbm_peak, note="keys / sort / tree stages: algorithmic bytes over stage time; at N = 2^20 the working "
+                            "set (12-116 MB) sits in the 126 MB L2 and the stages are launch- and latency-bound, the fraction of HBM "
+                            "bandwidth only means something at --config 5 (N = 10^7)", stages=hbm_stages),
             e2e=dict(value=e2e_value, unit="interactions/s", ms_per_step=e2e_ms, h2d_bytes_per_step=h2d_bytes,
                      d2h_bytes_per_step=d2h_bytes, steps=Ke),
             gpu_launches=int(launches),
