@@ -391,3 +391,41 @@ def test_rms_error_vs_direct_sum_config4():
         t.close()
     print("RMS relative force error vs direct sum, theta 0.3 / 0.7:", errs)
     assert errs[0] < errs[1] < 5e-3 and errs[0] < 5e-4
+
+
+def test_scale_and_translation():
+    """Properties that hold at any size: a power-of-two rescaling leaves every integer result unchanged and scales the
+    forces exactly as Newton's law says; a large translation (tight binaries far from the origin) still meets 1e-5."""
+    import copy
+    w = make_workload(2, N=30011)
+    t0 = _gpu_tree(w)
+    c0 = t0.force(want_counts=True)
+    g0 = [_np(v).copy() for v in (t0.acc_x, t0.acc_y, t0.acc_z, t0.pot)]
+    off0, idx0 = (_np(v).copy() for v in t0.neighbors())
+    t0.close()
+    s = 2.0 ** 10
+    ws = copy.copy(w)
+    ws.x, ws.y, ws.z, ws.r_out = w.x * s, w.y * s, w.z * s, w.r_out * s
+    t1 = _gpu_tree(ws)
+    c1 = t1.force(want_counts=True)
+    assert (c1.n_epep, c1.n_epsp, c1.n_epep_near, c1.n_groups, c1.n_nodes) == (c0.n_epep, c0.n_epsp, c0.n_epep_near, c0.n_groups, c0.n_nodes)
+    g1 = [_np(v) for v in (t1.acc_x, t1.acc_y, t1.acc_z, t1.pot)]
+    ea, ep = _rel_err([g1[0] * s * s, g1[1] * s * s, g1[2] * s * s, g1[3] * s], g0, sel=np.ones(w.N, bool))
+    assert ea.max() < 1e-6 and ep.max() < 1e-6          # the same arithmetic up to fp32 exponent shifts
+    off1, idx1 = (_np(v) for v in t1.neighbors())
+    assert np.array_equal(off1, off0)
+    rows = np.repeat(np.arange(w.N), np.diff(off0))
+    assert np.array_equal(idx1[np.lexsort((idx1, rows))], idx0[np.lexsort((idx0, rows))])
+    t1.close()
+    # translation: the whole cluster 1000 length units away from the origin
+    wt = copy.copy(w)
+    wt.x, wt.y, wt.z = w.x + 1000.0, w.y - 700.0, w.z + 333.0
+    t2, T2 = _gpu_tree(wt), _ora_tree(wt)
+    check_structures(t2, T2, wt)
+    c2 = t2.force(want_counts=True)
+    check_counts_and_lists(t2, T2, c2, sample=10)
+    g2 = [_np(v) for v in (t2.acc_x, t2.acc_y, t2.acc_z, t2.pot)]
+    ea, ep = _rel_err(g2, T2.force())
+    assert ea.max() < TOL and ep.max() < TOL, (ea.max(), ep.max())
+    check_neighbors(t2, T2, wt.N)
+    t2.close()
