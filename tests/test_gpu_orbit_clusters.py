@@ -139,3 +139,29 @@ def test_clusters_edge_cases():
         P.petar_clusters(off, idx, n, lab, ncl, torch.zeros(n + 1, dtype=torch.int64, device="cuda"), None, None)    # no workspace
     with pytest.raises(P.PetarError):
         P.petar_search_radii(lab, lab, lab, lab, -1.0, 0.1, n, lab)
+
+
+def test_orbit_list_degenerate_cases():
+    """At rest r_nb = r_out and stage (ii) keeps every candidate (all are inside their changeover radius): the orbit
+    list equals the plain one.  N = 0 and bad arguments."""
+    import torch
+    P = _P()
+    w = make_workload(2, N=9001)
+    z = torch.zeros(w.N, dtype=torch.float64, device="cuda")
+    t = P.Tree(w.N, P.PetarParams.from_workload(w))
+    t.upload(w.x, w.y, w.z, w.m, w.r_out)
+    t.build()
+    off0, idx0 = (_np(v).copy() for v in t.neighbors())
+    off1, idx1 = (_np(v).copy() for v in t.neighbors_orbit(z, z, z, 0.0))
+    assert np.array_equal(off0, off1) and np.array_equal(_sorted_rows(off0, idx0, w.N), _sorted_rows(off1, idx1, w.N))
+    with pytest.raises(P.PetarError):
+        P.petar_neighbor_list_orbit(t.handle, z, z, z, -1.0, t.offsets, None, 0)
+    with pytest.raises(P.PetarError):
+        P.petar_neighbor_list_orbit(t.handle, None, z, z, 1.5, t.offsets, None, 0)
+    t.close()
+    h = P.petar_tree_build(None, None, None, None, None, None, 0, P.PetarParams.make(theta=0.3, multipole=2), None)
+    off = torch.full((1,), 7, dtype=torch.int64, device="cuda")
+    P.petar_neighbor_list_orbit(h, None, None, None, 1.5, off, None, 0)
+    torch.cuda.synchronize()
+    assert int(off[0]) == 0
+    P.petar_tree_destroy(h)
