@@ -1,17 +1,21 @@
 // force.cu -- step S8: fp32 pairwise force + potential over the walk's lists (rule O8), with the
 // changeover weights 1-K (Eq. 17) and 1-W (Eq. 15) on near EP pairs.
 //
-// One CTA (128 threads) per i-group, groups pulled from a device ticket (persistent CTAs).
-// Thread mapping: the group's n_i particles are taken two per thread ("pair slot" p = t % P,
-// P = ceil(n_i/2)); S = 128 / P slices split every staged j-tile (slice s handles j = s, s+S, ...),
-// so >= 80 % of the lanes are busy for any n_i in 1..64 and every shared-memory j-record feeds two
-// interactions.
+// Two kernels:
+//   PHASE A, k_force_units: the cells COMMON to a super-group (accepted once for all of its i-groups by
+//     k_walk_super) against all of its particles, in units of 128 / 64 / 32 / < 32 particles, four
+//     i-particles per lane, warps that stage their own tiles without CTA barriers; sums go to `part`.
+//   PHASE B, k_force: one CTA (128 threads) per i-group for the group's OWN cells and particles, groups
+//     pulled from a device ticket (persistent CTAs).  Thread mapping: the group's n_i particles are taken
+//     two per thread ("pair slot" p = t % P, P = ceil(n_i/2)); S = 128 / P slices split every staged
+//     j-tile (slice s handles j = s, s+S, ...), so >= 80 % of the lanes are busy for any n_i in 1..64 and
+//     every shared-memory j-record feeds two interactions.  It adds `part`, scales by G and scatters.
 //
-// The kernel is ISSUE-bound ("force kernel"): on B200 scalar FFMA/FADD/FMUL issue at one
-// warp instruction per clock per sub-partition, the packed fp32x2 forms measured slower per flop for
-// distinct operands, so the design minimises instructions per interaction:
-//   * cells farther from the group than the group's own size (the bulk) are evaluated with
-//     GROUP-RELATIVE single floats: the j-record is translated to the group centre once when its tile
+// The kernels are bound by FP32 instruction issue, more precisely by the register-operand bandwidth of
+// the sub-partition (an FFMA with three distinct register sources issues at 0.61 per clock, the packed
+// fp32x2 forms gain nothing), so the design minimises instructions per interaction:
+//   * cells farther from the (super-)group than its own size (the bulk) are evaluated with
+//     GROUP-RELATIVE single floats: the j-record is translated to the box centre once when its tile
 //     is staged, the displacement is then one FADD per axis (33 fp32 instructions + 1 MUFU per
 //     quadrupole interaction);
 //   * cells closer than that, and all particles, keep float-float coordinates (hi + lo, relative to
@@ -19,8 +23,8 @@
 //     separation whatever the distance from the origin (needed for tight binaries in sparse groups).
 // Super-particle tiles are gathered through a 3-stage software pipeline (ids two tiles ahead,
 // 48-byte records one tile ahead in registers, current tile in double-buffered shared memory), so
-// the dependent id -> record loads overlap the arithmetic and there is one barrier per tile.
-// fp32 partial sums live only across one tile slice and are flushed into fp64 accumulators per tile.
+// the dependent id -> record loads overlap the arithmetic.
+// fp32 partial sums live only across one tile slice and are flushed into fp64 accumulators.
 #include "internal.cuh"
 
 #ifndef FT

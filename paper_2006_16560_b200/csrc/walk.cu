@@ -1,5 +1,5 @@
-// walk.cu -- step S7 (per-group interaction-list walk, rule O7), step S9 (neighbour-list writer,
-// rule O9) and the list export used by the tests.  Compiled with -fmad=false: the MAC and the
+// walk.cu -- step S7 (interaction-list walk, rule O7: two super-group levels, then the i-groups), step S9
+// (neighbour-list writer, rules O9 / O10) and the list export used by the tests.  Compiled with -fmad=false: the MAC and the
 // neighbour test are fp64 with exactly the operation order of DESIGN.md O7 / O9 (fma where written).
 #include "internal.cuh"
 
