@@ -88,7 +88,7 @@ static size_t carve(Workspace* w, char* base, int64_t N, const petar_params* p) 
     W->grp = (GroupRec*)take((size_t)W->group_cap * sizeof(GroupRec));
     W->srec = (SuperRec*)take((size_t)PETAR_NSUP * W->group_cap * sizeof(SuperRec));
     W->smap = (int*)take((size_t)PETAR_NSUP * n * 4);
-    W->unit_cap = (int)(PETAR_NSUP * (N + N / 16 + 64));
+    W->unit_cap = (int)(PETAR_NSUP * (N + 64));             // every unit holds at least one particle
     W->units = (ForceUnit*)take((size_t)W->unit_cap * sizeof(ForceUnit));
     W->part = (double*)take((size_t)PETAR_NSUP * n * 4 * 8);
     W->nb_cnt = (int*)take(n * 4);

@@ -92,19 +92,65 @@ __device__ __forceinline__ void cell_term(Acc32& p, const float dx, const float 
     }
 }
 
+// ---- packed fp32x2 arithmetic (Blackwell FFMA2 / FMUL2 / FADD2) ------------------------------------
+// Two i-particles share one instruction: the halves of a float2 are particles i0 and i1, a j-operand is a
+// scalar that the instruction broadcasts to both halves (SASS operand form R.F32, one 32-bit register read).
+// A packed instruction keeps the FMA pipe busy for two cycles and reads a register PAIR (one even, one odd
+// register) per operand, so it cannot suffer the even/odd register-bank conflicts that hold the scalar
+// instruction stream at ~1.22 cycles per instruction (profiles/fp32_issue_model_r02.md).
+typedef float2 f2;
+__device__ __forceinline__ f2 fma2(const f2 a, const f2 b, const f2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ f2 mul2(const f2 a, const f2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ f2 add2(const f2 a, const f2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ f2 bc(const float v) { return make_float2(v, v); }
+struct Acc2 { f2 ax, ay, az, pot; };            // .x = first particle of the pair, .y = second
+__device__ __forceinline__ void flush(Acc2& p, Acc64& a0, Acc64& a1) {
+    a0.ax += (double)p.ax.x; a0.ay += (double)p.ay.x; a0.az += (double)p.az.x; a0.pot += (double)p.pot.x;
+    a1.ax += (double)p.ax.y; a1.ay += (double)p.ay.y; a1.az += (double)p.az.y; a1.pot += (double)p.pot.y;
+    p.ax = p.ay = p.az = p.pot = make_float2(0.f, 0.f);
+}
+// cell_term for a pair of i-particles (same algebra, see above)
+template <bool QUAD>
+__device__ __forceinline__ void cell_term2(Acc2& p, const f2 dx, const f2 dy, const f2 dz, const float M,
+                                           const float bxx, const float byy, const float bzz, const float bxy, const float bxz, const float byz) {
+    const f2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+    f2 rinv; rinv.x = rsqrt_ftz(r2.x); rinv.y = rsqrt_ftz(r2.y);
+    const f2 rinv2 = mul2(rinv, rinv);
+    const f2 mr = mul2(bc(M), rinv);
+    if (!QUAD) {
+        const f2 f = mul2(mr, rinv2);
+        p.pot = add2(p.pot, mr);
+        p.ax = fma2(f, dx, p.ax); p.ay = fma2(f, dy, p.ay); p.az = fma2(f, dz, p.az);
+    } else {
+        const f2 bdx = fma2(bc(bxx), dx, fma2(bc(bxy), dy, mul2(bc(bxz), dz)));
+        const f2 bdy = fma2(bc(bxy), dx, fma2(bc(byy), dy, mul2(bc(byz), dz)));
+        const f2 bdz = fma2(bc(bxz), dx, fma2(bc(byz), dy, mul2(bc(bzz), dz)));
+        const f2 dbd = fma2(dx, bdx, fma2(dy, bdy, mul2(dz, bdz)));
+        const f2 rinv4 = mul2(rinv2, rinv2);
+        const f2 rinv5 = mul2(rinv4, rinv);
+        const f2 u = mul2(dbd, rinv5);
+        p.pot = fma2(u, bc(-0.5f), add2(p.pot, mr));
+        const f2 f = mul2(fma2(u, bc(-2.5f), mr), rinv2);
+        p.ax = fma2(f, dx, fma2(rinv5, bdx, p.ax));
+        p.ay = fma2(f, dy, fma2(rinv5, bdy, p.ay));
+        p.az = fma2(f, dz, fma2(rinv5, bdz, p.az));
+    }
+}
+
 struct IFF { float nxh, nyh, nzh, nxl, nyl, nzl, inv_ro; };     // negated float-float position of an i-particle
 
-// one far particle: plain Newtonian (every pair of a far leaf has r >= R_ij > 0, rule O7)
-__device__ __forceinline__ void ep_far_one(Acc32& p, const IFF& i, const float4 a, const float4 b) {
-    const float dx = (a.x + i.nxh) + (b.x + i.nxl);
-    const float dy = (a.y + i.nyh) + (b.y + i.nyl);
-    const float dz = (a.z + i.nzh) + (b.z + i.nzl);
-    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const float rinv = rsqrt_ftz(r2);
-    const float mr = a.w * rinv;
-    const float f = mr * (rinv * rinv);
-    p.pot += mr;
-    p.ax = fmaf(f, dx, p.ax); p.ay = fmaf(f, dy, p.ay); p.az = fmaf(f, dz, p.az);
+// one far particle against a pair of i-particles: plain Newtonian (every pair of a far leaf has r >= R_ij > 0, rule O7)
+struct IFF2 { f2 nxh, nyh, nzh, nxl, nyl, nzl; };      // negated float-float positions of the two i-particles
+__device__ __forceinline__ void ep_far_pair(Acc2& p, const IFF2& i, const float4 a, const float4 b) {
+    const f2 dx = add2(add2(bc(a.x), i.nxh), add2(bc(b.x), i.nxl));
+    const f2 dy = add2(add2(bc(a.y), i.nyh), add2(bc(b.y), i.nyl));
+    const f2 dz = add2(add2(bc(a.z), i.nzh), add2(bc(b.z), i.nzl));
+    const f2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+    f2 rinv; rinv.x = rsqrt_ftz(r2.x); rinv.y = rsqrt_ftz(r2.y);
+    const f2 mr = mul2(bc(a.w), rinv);
+    const f2 f = mul2(mr, mul2(rinv, rinv));
+    p.pot = add2(p.pot, mr);
+    p.ax = fma2(f, dx, p.ax); p.ay = fma2(f, dy, p.ay); p.az = fma2(f, dz, p.az);
 }
 
 // one near particle: changeover weights (Eq. 15-17).  self = the list entry is the i-particle itself.
@@ -185,17 +231,18 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
                                          const float4 ia0, const float4 ib0, const float4 ia1, const float4 ib1,
                                          const float3 gh, const float3 gl, Acc64& acc0, Acc64& acc1) {
     if (n + n2 <= 0) return;        // uniform
-    // i-particles in the representation of this path
-    float ix0, iy0, iz0, ix1, iy1, iz1;                 // PLAIN: group-relative; PRECISE: -hi
-    float lx0 = 0.f, ly0 = 0.f, lz0 = 0.f, lx1 = 0.f, ly1 = 0.f, lz1 = 0.f;     // PRECISE: -lo
+    // the thread's two i-particles as a packed pair, NEGATED, in the representation of this path
+    f2 nx, ny, nz;                                      // PLAIN: group-relative; PRECISE: hi parts
+    f2 lx = make_float2(0.f, 0.f), ly = lx, lz = lx;    // PRECISE: lo parts
     if (PRECISE) {
-        ix0 = -ia0.x; iy0 = -ia0.y; iz0 = -ia0.z; lx0 = -ib0.x; ly0 = -ib0.y; lz0 = -ib0.z;
-        ix1 = -ia1.x; iy1 = -ia1.y; iz1 = -ia1.z; lx1 = -ib1.x; ly1 = -ib1.y; lz1 = -ib1.z;
+        nx = make_float2(-ia0.x, -ia1.x); ny = make_float2(-ia0.y, -ia1.y); nz = make_float2(-ia0.z, -ia1.z);
+        lx = make_float2(-ib0.x, -ib1.x); ly = make_float2(-ib0.y, -ib1.y); lz = make_float2(-ib0.z, -ib1.z);
     } else {
-        ix0 = (ia0.x - gh.x) + (ib0.x - gl.x); iy0 = (ia0.y - gh.y) + (ib0.y - gl.y); iz0 = (ia0.z - gh.z) + (ib0.z - gl.z);
-        ix1 = (ia1.x - gh.x) + (ib1.x - gl.x); iy1 = (ia1.y - gh.y) + (ib1.y - gl.y); iz1 = (ia1.z - gh.z) + (ib1.z - gl.z);
+        nx = make_float2(-((ia0.x - gh.x) + (ib0.x - gl.x)), -((ia1.x - gh.x) + (ib1.x - gl.x)));
+        ny = make_float2(-((ia0.y - gh.y) + (ib0.y - gl.y)), -((ia1.y - gh.y) + (ib1.y - gl.y)));
+        nz = make_float2(-((ia0.z - gh.z) + (ib0.z - gl.z)), -((ia1.z - gh.z) + (ib1.z - gl.z)));
     }
-    Acc32 p0 = {0.f, 0.f, 0.f, 0.f}, p1 = {0.f, 0.f, 0.f, 0.f};
+    Acc2 p = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
     TileCursor cur; cur.init(arena, head, n, head2, n2);
     int tn0 = 0, tn1 = 0, tn2 = 0;
     int id2[SP_REC];
@@ -250,16 +297,15 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
                     const float4 b = bf.q1[j];
                     float4 c = make_float4(0.f, 0.f, 0.f, 0.f); float byz = 0.f;
                     if (QUAD) { c = bf.q2[j]; byz = bf.q3[j]; }
-                    cell_term<QUAD>(p0, (a.x + ix0) + (b.x + lx0), (a.y + iy0) + (b.y + ly0), (a.z + iz0) + (b.z + lz0), a.w, b.w, c.x, c.y, c.z, c.w, byz);
-                    cell_term<QUAD>(p1, (a.x + ix1) + (b.x + lx1), (a.y + iy1) + (b.y + ly1), (a.z + iz1) + (b.z + lz1), a.w, b.w, c.x, c.y, c.z, c.w, byz);
+                    cell_term2<QUAD>(p, add2(add2(bc(a.x), nx), add2(bc(b.x), lx)), add2(add2(bc(a.y), ny), add2(bc(b.y), ly)),
+                                     add2(add2(bc(a.z), nz), add2(bc(b.z), lz)), a.w, b.w, c.x, c.y, c.z, c.w, byz);
                 } else {
                     float4 b = make_float4(0.f, 0.f, 0.f, 0.f); float2 c = make_float2(0.f, 0.f);
                     if (QUAD) { b = bf.q1[j]; c = *reinterpret_cast<const float2*>(&bf.q2[j]); }
-                    cell_term<QUAD>(p0, a.x - ix0, a.y - iy0, a.z - iz0, a.w, b.x, b.y, b.z, b.w, c.x, c.y);
-                    cell_term<QUAD>(p1, a.x - ix1, a.y - iy1, a.z - iz1, a.w, b.x, b.y, b.z, b.w, c.x, c.y);
+                    cell_term2<QUAD>(p, add2(bc(a.x), nx), add2(bc(a.y), ny), add2(bc(a.z), nz), a.w, b.x, b.y, b.z, b.w, c.x, c.y);
                 }
             }
-            flush(p0, acc0); flush(p1, acc1);
+            flush(p, acc0, acc1);
         }
         store_recs(sm.sp[cb ^ 1]); tn0 = tn1;    // tile k+1 (its loads overlapped the loop above)
         load_recs();                             // tile k+2 records (their ids arrived a tile ago)
@@ -313,7 +359,10 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
         {
             IFF i0 = {-ia0.x, -ia0.y, -ia0.z, -ib0.x, -ib0.y, -ib0.z, ib0.w};
             IFF i1 = {-ia1.x, -ia1.y, -ia1.z, -ib1.x, -ib1.y, -ib1.z, ib1.w};
+            const IFF2 i2 = {make_float2(i0.nxh, i1.nxh), make_float2(i0.nyh, i1.nyh), make_float2(i0.nzh, i1.nzh),
+                             make_float2(i0.nxl, i1.nxl), make_float2(i0.nyl, i1.nyl), make_float2(i0.nzl, i1.nzl)};
             Acc32 p0 = {0.f, 0.f, 0.f, 0.f}, p1 = {0.f, 0.f, 0.f, 0.f};
+            Acc2 pf = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll 1
             for (int pass = 0; pass < 2; ++pass) {
                 int chunk = pass == 0 ? gr->head_epn : gr->head_epf;
@@ -357,11 +406,11 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
 #pragma unroll 2
                                     for (int j = slice; j < tn; j += S) {
                                         const float4 a = sm.ep.a[j], b = sm.ep.b[j];
-                                        ep_far_one(p0, i0, a, b);
-                                        ep_far_one(p1, i1, a, b);
+                                        ep_far_pair(pf, i2, a, b);
                                     }
+                                    flush(pf, acc0, acc1);
                                 }
-                                flush(p0, acc0); flush(p1, acc1);
+                                if (pass == 0) { flush(p0, acc0); flush(p1, acc1); }
                             }
                         }
                     }
@@ -443,29 +492,40 @@ struct WarpTileCursor {
 };
 
 // fp64 accumulators of phase A live in shared memory (s_acc[component][thread], conflict-free): 16 per lane
-__device__ __forceinline__ void flush_smem(Acc32& p, double* __restrict__ a) {
-    a[0] += (double)p.ax; a[UW * 32] += (double)p.ay; a[2 * UW * 32] += (double)p.az; a[3 * UW * 32] += (double)p.pot;
-    p.ax = p.ay = p.az = p.pot = 0.0f;
+// (a: the accumulators of the pair's first particle; the second particle's follow 4 components later)
+__device__ __forceinline__ void flush_smem(Acc2& p, double* __restrict__ a) {
+    a[0] += (double)p.ax.x; a[UW * 32] += (double)p.ay.x; a[2 * UW * 32] += (double)p.az.x; a[3 * UW * 32] += (double)p.pot.x;
+    a[4 * UW * 32] += (double)p.ax.y; a[5 * UW * 32] += (double)p.ay.y; a[6 * UW * 32] += (double)p.az.y; a[7 * UW * 32] += (double)p.pot.y;
+    p.ax = p.ay = p.az = p.pot = make_float2(0.f, 0.f);
 }
 
-template <bool QUAD, bool PRECISE>
+template <bool QUAD, bool PRECISE, int NIv>
 __device__ __forceinline__ void unit_phase(UBuf* __restrict__ bufs, const int* __restrict__ arena, const NodeSp* __restrict__ nsp,
                                            const int head, const int n, const int w, const int lane, const int slice, const int S, const bool active,
                                            const float4* __restrict__ pa, const float4* __restrict__ pb, const int i0, const int ilast,
                                            const float3 gh, double* __restrict__ sacc) {
     if (n <= 0) return;             // warp-uniform
-    float ix[NI], iy[NI], iz[NI], lx[NI], ly[NI], lz[NI];
-    float4 ia[NI], ib[NI];
+    // the lane's NI i-particles as NI/2 packed pairs, NEGATED: PLAIN group-relative floats, PRECISE hi and lo parts
+    f2 nx[NIv / 2], ny[NIv / 2], nz[NIv / 2], lx[NIv / 2], ly[NIv / 2], lz[NIv / 2];
+    {
+        float4 ia[NIv], ib[NIv];
+        float ix[NIv], iy[NIv], iz[NIv], jx[NIv], jy[NIv], jz[NIv];
 #pragma unroll
-    for (int k = 0; k < NI; ++k) { const int i = min(i0 + k, ilast); ia[k] = pa[i]; ib[k] = pb[i]; }
+        for (int k = 0; k < NIv; ++k) { const int i = min(i0 + k, ilast); ia[k] = pa[i]; ib[k] = pb[i]; }
 #pragma unroll
-    for (int k = 0; k < NI; ++k) {
-        if (PRECISE) { ix[k] = -ia[k].x; iy[k] = -ia[k].y; iz[k] = -ia[k].z; lx[k] = -ib[k].x; ly[k] = -ib[k].y; lz[k] = -ib[k].z; }
-        else { ix[k] = (ia[k].x - gh.x) + ib[k].x; iy[k] = (ia[k].y - gh.y) + ib[k].y; iz[k] = (ia[k].z - gh.z) + ib[k].z; lx[k] = ly[k] = lz[k] = 0.f; }
+        for (int k = 0; k < NIv; ++k) {
+            if (PRECISE) { ix[k] = -ia[k].x; iy[k] = -ia[k].y; iz[k] = -ia[k].z; jx[k] = -ib[k].x; jy[k] = -ib[k].y; jz[k] = -ib[k].z; }
+            else { ix[k] = -((ia[k].x - gh.x) + ib[k].x); iy[k] = -((ia[k].y - gh.y) + ib[k].y); iz[k] = -((ia[k].z - gh.z) + ib[k].z); jx[k] = jy[k] = jz[k] = 0.f; }
+        }
+#pragma unroll
+        for (int k = 0; k < NIv / 2; ++k) {
+            nx[k] = make_float2(ix[2 * k], ix[2 * k + 1]); ny[k] = make_float2(iy[2 * k], iy[2 * k + 1]); nz[k] = make_float2(iz[2 * k], iz[2 * k + 1]);
+            lx[k] = make_float2(jx[2 * k], jx[2 * k + 1]); ly[k] = make_float2(jy[2 * k], jy[2 * k + 1]); lz[k] = make_float2(jz[2 * k], jz[2 * k + 1]);
+        }
     }
-    Acc32 p[NI];
+    Acc2 p[NIv / 2];
 #pragma unroll
-    for (int k = 0; k < NI; ++k) p[k].ax = p[k].ay = p[k].az = p[k].pot = 0.f;
+    for (int k = 0; k < NIv / 2; ++k) p[k].ax = p[k].ay = p[k].az = p[k].pot = make_float2(0.f, 0.f);
     WarpTileCursor cur; cur.start(arena, head, n, w);
     int tn0 = 0, tn1 = 0, tn2 = 0;
     int id2[UREC];
@@ -522,20 +582,21 @@ __device__ __forceinline__ void unit_phase(UBuf* __restrict__ bufs, const int* _
                     float4 c = make_float4(0.f, 0.f, 0.f, 0.f); float byz = 0.f;
                     if (QUAD) { c = bf.q2[j]; byz = bf.q3[j]; }
 #pragma unroll
-                    for (int k = 0; k < NI; ++k)
-                        cell_term<QUAD>(p[k], (a.x + ix[k]) + (b.x + lx[k]), (a.y + iy[k]) + (b.y + ly[k]), (a.z + iz[k]) + (b.z + lz[k]), a.w, b.w, c.x, c.y, c.z, c.w, byz);
+                    for (int k = 0; k < NIv / 2; ++k)
+                        cell_term2<QUAD>(p[k], add2(add2(bc(a.x), nx[k]), add2(bc(b.x), lx[k])), add2(add2(bc(a.y), ny[k]), add2(bc(b.y), ly[k])),
+                                         add2(add2(bc(a.z), nz[k]), add2(bc(b.z), lz[k])), a.w, b.w, c.x, c.y, c.z, c.w, byz);
                 } else {
                     float4 b = make_float4(0.f, 0.f, 0.f, 0.f); float2 c = make_float2(0.f, 0.f);
                     if (QUAD) { b = bf.q1[j]; c = *reinterpret_cast<const float2*>(&bf.q2[j]); }
 #pragma unroll
-                    for (int k = 0; k < NI; ++k)
-                        cell_term<QUAD>(p[k], a.x - ix[k], a.y - iy[k], a.z - iz[k], a.w, b.x, b.y, b.z, b.w, c.x, c.y);
+                    for (int k = 0; k < NIv / 2; ++k)
+                        cell_term2<QUAD>(p[k], add2(bc(a.x), nx[k]), add2(bc(a.y), ny[k]), add2(bc(a.z), nz[k]), a.w, b.x, b.y, b.z, b.w, c.x, c.y);
                 }
             }
             if (++fl >= fl_every) {
                 fl = 0;
 #pragma unroll
-                for (int k = 0; k < NI; ++k) flush_smem(p[k], sacc + 4 * k * (UW * 32));
+                for (int k = 0; k < NIv / 2; ++k) flush_smem(p[k], sacc + 8 * k * (UW * 32));
             }
         }
         store_recs(bufs[cb ^ 1]); tn0 = tn1;
@@ -546,14 +607,39 @@ __device__ __forceinline__ void unit_phase(UBuf* __restrict__ bufs, const int* _
     }
     if (active) {
 #pragma unroll
-        for (int k = 0; k < NI; ++k) flush_smem(p[k], sacc + 4 * k * (UW * 32));
+        for (int k = 0; k < NIv / 2; ++k) flush_smem(p[k], sacc + 8 * k * (UW * 32));
     }
+}
+
+// one unit with NIv i-particles per lane (slot = lane % P, P = ceil(cnt / NIv); S = 32 / P slices)
+template <bool QUAD, int NIv>
+__device__ __forceinline__ void unit_run(UBuf* __restrict__ bufs, const int* __restrict__ arena, const NodeSp* __restrict__ nsp,
+                                         const int head_sp, const int n_sp, const int head_spp, const int n_spp, const int w, const int lane,
+                                         const float4* __restrict__ pa, const float4* __restrict__ pb, const int ibeg, const int cnt,
+                                         const float3 gh, double* __restrict__ sacc) {
+    const int P = (cnt + NIv - 1) / NIv, S = 32 / P;
+    const int slot = lane % P, slice = lane / P;
+    const bool active = slice < S;
+    const int i0 = ibeg + NIv * slot, ilast = ibeg + cnt - 1;
+#pragma unroll
+    for (int c = 0; c < 4 * NIv; ++c) sacc[c * (UW * 32)] = 0.0;
+    unit_phase<QUAD, false, NIv>(bufs, arena, nsp, head_sp, n_sp, w, lane, slice, S, active, pa, pb, i0, ilast, gh, sacc);
+    unit_phase<QUAD, true, NIv>(bufs, arena, nsp, head_spp, n_spp, w, lane, slice, S, active, pa, pb, i0, ilast, gh, sacc);
+}
+
+// i-particles per lane of a unit of cnt particles: 4 (two packed pairs in flight), or 2 where that keeps clearly more
+// lanes busy (busy fraction of a warp = S * cnt / (32 * NI))
+__device__ __forceinline__ int unit_ni(const int cnt) {
+    if (cnt > 64) return 4;
+    const int s4 = 32 / ((cnt + 3) >> 2), s2 = 32 / ((cnt + 1) >> 1);
+    return (200 * s2 > 108 * s4) ? 2 : 4;
 }
 
 template <bool QUAD>
 __global__ void __launch_bounds__(UW * 32, UNITS_MIN_CTAS) k_force_units(DevHeader* __restrict__ h, const ForceUnit* __restrict__ units, const SuperRec* __restrict__ srec,
-                                                            const int group_cap, const NodeW* __restrict__ nw, const int* __restrict__ arena,
-                                                            const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
+                                                            const int group_cap, const NodeW* __restrict__ nw,
+                                                            const int* __restrict__ arena, const NodeSp* __restrict__ nsp,
+                                                            const float4* __restrict__ pa, const float4* __restrict__ pb,
                                                             double* __restrict__ part, const long long n_part) {
     __shared__ __align__(16) UBuf s_buf[UW][2];
     __shared__ double s_acc[4 * NI][UW * 32];
@@ -568,52 +654,65 @@ __global__ void __launch_bounds__(UW * 32, UNITS_MIN_CTAS) k_force_units(DevHead
         const int u = s_u;
         if (u >= nu) break;
         const ForceUnit fu = units[u];
-        const SuperRec* sr = &srec[(size_t)fu.level * group_cap + fu.rec];
         const int cnt = fu.cnt;
-        const int P = (cnt + NI - 1) / NI, S = 32 / P;
-        const int slot = lane % P, slice = lane / P;
-        const bool active = slice < S;
-        const int i0 = fu.ibeg + NI * slot, ilast = fu.ibeg + cnt - 1;
+        const SuperRec* sr = &srec[(size_t)fu.level * group_cap + fu.rec];
+        const int head_sp = sr->head_sp, n_sp = sr->n_sp, head_spp = sr->head_spp, n_spp = sr->n_spp;
         // any fp32 point inside the super-group's box serves as the origin of the group-relative floats
         const float4 ba = nw[sr->node].a, bb = nw[sr->node].b;
         const float3 gh = make_float3(0.5f * (ba.x + ba.w), 0.5f * (ba.y + bb.x), 0.5f * (ba.z + bb.y));
-#pragma unroll
-        for (int c = 0; c < 4 * NI; ++c) sacc[c * (UW * 32)] = 0.0;
-        unit_phase<QUAD, false>(s_buf[w], arena, nsp, sr->head_sp, sr->n_sp, w, lane, slice, S, active, pa, pb, i0, ilast, gh, sacc);
-        unit_phase<QUAD, true>(s_buf[w], arena, nsp, sr->head_spp, sr->n_spp, w, lane, slice, S, active, pa, pb, i0, ilast, gh, sacc);
+        const int ni = unit_ni(cnt);
+        if (ni == 4) unit_run<QUAD, 4>(s_buf[w], arena, nsp, head_sp, n_sp, head_spp, n_spp, w, lane, pa, pb, fu.ibeg, cnt, gh, sacc);
+        else unit_run<QUAD, 2>(s_buf[w], arena, nsp, head_sp, n_sp, head_spp, n_spp, w, lane, pa, pb, fu.ibeg, cnt, gh, sacc);
         // ordered reduction over the warps and their slices
         __syncthreads();
+        const int P = (cnt + ni - 1) / ni, S = 32 / P;
         double* out = part + ((size_t)fu.level * n_part + fu.ibeg) * 4;
         for (int e = threadIdx.x; e < cnt * 4; e += UW * 32) {
             const int i = e >> 2, comp = e & 3;
             double sum = 0.0;
             for (int ww = 0; ww < UW; ++ww)
-                for (int sl = 0; sl < S; ++sl) sum += s_acc[(i % NI) * 4 + comp][ww * 32 + sl * P + (i / NI)];
+                for (int sl = 0; sl < S; ++sl) sum += s_acc[(i % ni) * 4 + comp][ww * 32 + sl * P + (i / ni)];
             out[e] = sum;
         }
     }
 }
 
-// unit table: every super-group is cut into units of 128 particles, then at most one of 64, one of 32 and
-// one of < 32; units are stored by size class (largest first) so the ticket order ends with the small ones
+// unit table: every super-group is cut into units of 128 particles, then at most one each of 64, 32 and < 32;
+// units are stored by size class (largest first) so the ticket order ends with the small ones
 template <class F>
 __device__ __forceinline__ void for_units(const int begin, const int n, F f) {
     int b = begin, r = n;
     while (r >= UNIT_MAX) { f(0, b, UNIT_MAX); b += UNIT_MAX; r -= UNIT_MAX; }
-    if (r >= UNIT_MAX / 2) { f(1, b, UNIT_MAX / 2); b += UNIT_MAX / 2; r -= UNIT_MAX / 2; }
-    if (r >= UNIT_MAX / 4) { f(2, b, UNIT_MAX / 4); b += UNIT_MAX / 4; r -= UNIT_MAX / 4; }
-    if (r > 0) f(3, b, r);
+#pragma unroll
+    for (int c = 1; c < PETAR_UNIT_CLASSES - 1; ++c) {
+        const int sz = UNIT_MAX >> c;
+        if (r >= sz) { f(c, b, sz); b += sz; r -= sz; }
+    }
+    if (r > 0) f(PETAR_UNIT_CLASSES - 1, b, r);
+}
+// particle range of super-group `id` of level l (false: no such record)
+__device__ __forceinline__ bool unit_range(const DevHeader* __restrict__ h, const SuperRec* __restrict__ srec, const int group_cap, const int l, const int id,
+                                           int& begin, int& n) {
+    if (id >= h->n_super[l]) return false;
+    const SuperRec* sr = &srec[(size_t)l * group_cap + id];
+    begin = sr->begin; n = sr->end - sr->begin;
+    return true;
 }
 __global__ void __launch_bounds__(256) k_units_count(DevHeader* __restrict__ h, const SuperRec* __restrict__ srec, const int group_cap) {
     const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    int c[PETAR_UNIT_CLASSES];
+#pragma unroll
+    for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) c[k] = 0;
 #pragma unroll
     for (int l = 0; l < PETAR_NSUP; ++l) {
-        if (id >= h->n_super[l]) continue;
-        const SuperRec* sr = &srec[(size_t)l * group_cap + id];
-        int c[PETAR_UNIT_CLASSES] = {0, 0, 0, 0};
-        for_units(sr->begin, sr->end - sr->begin, [&](int cls, int, int) { ++c[cls]; });
+        int begin, n;
+        if (!unit_range(h, srec, group_cap, l, id, begin, n)) continue;
+        for_units(begin, n, [&](int cls, int, int) { ++c[cls]; });
+    }
 #pragma unroll
-        for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) if (c[k]) atomicAdd(&h->unit_cnt[k], c[k]);
+    for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) {          // one atomic per class and warp
+        const int tot = __reduce_add_sync(0xffffffffu, c[k]);
+        if ((threadIdx.x & 31) == 0 && tot) atomicAdd(&h->unit_cnt[k], tot);
     }
 }
 __global__ void k_units_offsets(DevHeader* h, const int unit_cap) {
@@ -629,9 +728,9 @@ __global__ void __launch_bounds__(256) k_units_fill(DevHeader* __restrict__ h, c
     if (h->unit_off[PETAR_UNIT_CLASSES] == 0) return;
 #pragma unroll
     for (int l = 0; l < PETAR_NSUP; ++l) {
-        if (id >= h->n_super[l]) continue;
-        const SuperRec* sr = &srec[(size_t)l * group_cap + id];
-        for_units(sr->begin, sr->end - sr->begin, [&](int cls, int b, int cnt) {
+        int begin, n;
+        if (!unit_range(h, srec, group_cap, l, id, begin, n)) continue;
+        for_units(begin, n, [&](int cls, int b, int cnt) {
             const int at = h->unit_off[cls] + atomicAdd(&h->unit_fill[cls], 1);
             ForceUnit fu; fu.rec = id; fu.ibeg = b; fu.cnt = cnt; fu.level = l;
             units[at] = fu;
