@@ -32,8 +32,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 FLOP_NEWTON, FLOP_CUT, FLOP_QUAD = 20, 49, 53      # fixed flops-per-interaction convention
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures (profiles/), bytes
-TRAFFIC_NCU = {"k_force_units": 187.1e6, "k_force": 1246.6e6}     # profiles/ncu_r01_phaseAB.md
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the force kernels, from the committed `ncu --set full` capture of
+# THIS round's build at config 3 (profiles/ncu_r02_force.md).  Emitted only for that configuration; any other run reports null.
+TRAFFIC_NCU = {"capture": "profiles/ncu_r02_force.md", "config": 3, "k_force_units": 187.2e6, "k_force": 1237.5e6}
 
 
 def parse():
@@ -115,17 +116,13 @@ def cpu_oracle_sample(w, n_groups_sample: int, seed: int = 1):
     t0 = time.perf_counter()
     T.force(sel)
     t_force = time.perf_counter() - t0
-    # interactions of the sample (counted by a second, untimed walk of the same groups)
-    n_int = 0
-    gb, ge, *_ = T.groups()
-    for g in sel[:: max(1, len(sel) // 200)]:
-        sp, ep = T.walk_lists(int(g))
-        n_int += (ge[g] - gb[g]) * (len(sp) + int((ep[:, 1] - ep[:, 0]).sum()))
-    n_int = n_int * len(sel) / len(sel[:: max(1, len(sel) // 200)])
+    # interactions of the sample, counted exactly by the oracle's own (untimed) count walk: sum over the sampled groups of
+    # n_i * (n_ep + n_sp), rule O7
+    oc, _, _ = T.walk_counts()
+    n_int = int((oc[sel, 0] * (oc[sel, 1] + oc[sel, 2])).sum())
     return dict(value=n_int / t_force, unit="interactions/s", cores=oracle.num_threads(), kind="oracle",
                 sample=f"fp64 oracle (oracle/petar_oracle.c, OpenMP): tree build of all N={w.N} particles ({t_build:.2f} s, untimed in value) "
-                       f"+ walk and force of {len(sel)} of {ng} i-groups ({t_force:.2f} s, ~{n_int:.3g} interactions, "
-                       f"counted on a 1/{max(1, len(sel) // 200)} subsample)",
+                       f"+ walk and force of {len(sel)} of {ng} i-groups ({t_force:.2f} s, {n_int} interactions, counted exactly)",
                 seconds=t_force, build_seconds=t_build)
 
 
@@ -153,6 +150,20 @@ def run_reference(args):
                cpu_baseline=dict(value=v, unit="interactions/s", cores=base["cores"], kind="oracle", sample=base["sample"]),
                e2e=dict(value=v, unit="interactions/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))
     print(json.dumps(out), flush=True)
+
+
+def aggregate_ranks(ms_step: float, e2e_ms: float, interactions: float, dist=None, device="cpu"):
+    """Whole-job figures of N independent replicas: time = MAX over ranks, interactions = SUM over ranks
+    (tests/test_multi_rank.py runs this very function on two gloo ranks)."""
+    if dist is not None:
+        import torch
+        t = torch.tensor([ms_step, e2e_ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step, e2e_ms = float(t[0]), float(t[1])
+        s = torch.tensor([interactions], dtype=torch.float64, device=device)
+        dist.all_reduce(s, op=dist.ReduceOp.SUM)
+        interactions = float(s[0])
+    return ms_step, e2e_ms, interactions
 
 
 def main():
@@ -277,7 +288,7 @@ def main():
 
     step_e2e()
     torch.cuda.synchronize()
-    Ke = max(3, min(K, 10))
+    Ke = K
     if dist: dist.barrier()
     t0 = time.perf_counter()
     for _ in range(Ke):
@@ -418,30 +429,30 @@ def main():
 
     pk, pk_kind = peaks()
     sm_max = float(pk.get("sm_max_mhz", 1965.0))
-    nominal_fp32 = 2 * 128 * 148 * sm_max * 1e6 / 1e12
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    nominal_fp32 = 2 * 128 * n_sm * sm_max * 1e6 / 1e12
 
     # ---- aggregate over ranks --------------------------------------------------------------------------
-    ms_step = ms_total / K
-    tot_inter = float(n_inter)
-    if dist:
-        t = torch.tensor([ms_step, e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step, e2e_ms = float(t[0]), float(t[1])
-        s = torch.tensor([tot_inter], dtype=torch.float64, device=dev)
-        dist.all_reduce(s, op=dist.ReduceOp.SUM)
-        tot_inter = float(s[0])
+    # headline time per step: the MEDIAN of the K per-step CUDA-event times; the mean is kept beside it
+    step_ms = sorted(a.elapsed_time(b) for a, b in ev)
+    ms_median = step_ms[K // 2] if K % 2 else 0.5 * (step_ms[K // 2 - 1] + step_ms[K // 2])
+    ms_mean = ms_total / K
+    ms_step, e2e_ms, tot_inter = aggregate_ranks(ms_median, e2e_ms, float(n_inter), dist, dev)
     value = tot_inter / (ms_step * 1e-3)
     e2e_value = tot_inter / (e2e_ms * 1e-3)
 
     stage_ms = {k: v / K for k, v in stage_sum.items()}
     # HBM-side stages: algorithmic bytes per particle against the measured copy bandwidth
     hbm_peak = float(pk.get("hbm_gbs", 6545.6))
-    stage_bytes = {"bbox_keys": 36.0, "sort": 256.0, "gather": 116.0, "tree": 20.0, "moments": 115.0, "groups": 40.0}
+    # keys 36 B, sort ~200 B (8 + 8 x 24), gather 84 B per particle, S4-S6 (tree + moments + groups) ~100 B together
+    stage_bytes = {"bbox_keys": (36.0, ("bbox_keys",)), "sort": (200.0, ("sort",)), "gather": (84.0, ("gather",)),
+                   "tree_moments_groups": (100.0, ("tree", "moments", "groups"))}
     hbm_stages = {}
-    for name, bpp in stage_bytes.items():
-        if stage_ms.get(name, 0.0) > 0.0:
-            gbs = bpp * N / (stage_ms[name] * 1e-3) / 1e9
-            hbm_stages[name] = dict(ms=stage_ms[name], bytes_per_particle=bpp, achieved_gbs=gbs, frac_of_hbm=gbs / hbm_peak)
+    for name, (bpp, parts) in stage_bytes.items():
+        ms_st = sum(stage_ms.get(q, 0.0) for q in parts)
+        if ms_st > 0.0:
+            gbs = bpp * N / (ms_st * 1e-3) / 1e9
+            hbm_stages[name] = dict(ms=ms_st, bytes_per_particle=bpp, achieved_gbs=gbs, frac_of_hbm=gbs / hbm_peak)
     kern = [dict(kernel="k_force_units", ms=stage_ms["force_units"], flops_per_launch=float(flops_units)),
             dict(kernel="k_force", ms=stage_ms["force"], flops_per_launch=float(flops_groups))]
     for kd in kern:
@@ -455,7 +466,7 @@ def main():
     if rank == 0:
         out = dict(
             metric="long-range interactions/sec", value=value, unit="interactions/s", n_gpus=world, steps=K, warmup=W,
-            ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+            ms_per_step=ms_step, ms_per_step_mean=ms_mean, ms_per_step_min=step_ms[0], ms_per_step_max=step_ms[-1], higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
             config={"workload": f"BASELINE.json configs[{cfg - 1}]: N={N} Plummer (Henon units), "
                                 f"{w.meta['masses']} masses, {2 * w.meta['n_pairs']} stars in binaries, r_out_ref={w.r_out_ref}, "
                                 f"theta={w.theta}, multipole={params.multipole}, leaf<=8, group<=64",
@@ -473,8 +484,10 @@ def main():
             gpu_launches=int(launches),
             clocks=clocks,
             roofline=dict(bound="alu", kernel=dom["kernel"], achieved=dom["achieved"], peak=nominal_fp32, unit="TFLOP/s",
-                          frac=dom["frac"], traffic=TRAFFIC_NCU.get(dom["kernel"]),
-                          peak_kind=f"nominal CUDA-core FP32: 2 x 128 lanes x 148 SMs x {sm_max:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {pk_kind})",
+                          frac=dom["frac"],
+                          traffic=TRAFFIC_NCU.get(dom["kernel"]) if (cfg == TRAFFIC_NCU["config"] and args.N is None) else None,
+                          traffic_source=TRAFFIC_NCU["capture"],
+                          peak_kind=f"nominal CUDA-core FP32: 2 x 128 lanes x {n_sm} SMs x {sm_max:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {pk_kind})",
                           peak_measured_ffma_probe=probe_tflops, frac_of_probe=dom["achieved"] / probe_tflops,
                           probes_tflops=probes,
                           frac_of_cell_term_probe=dom["achieved"] / probes["quadrupole_cell_term_loop"],

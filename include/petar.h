@@ -20,7 +20,9 @@
  *     has passed the last call that uses the tree.  The tree handle is a small host object that
  *     points into the workspace; it dies with petar_tree_destroy or with the workspace.
  *   - cuda_stream is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is
- *     enqueued on it; calls return without synchronising unless a HOST output is requested.
+ *     enqueued on it; calls return without synchronising unless a HOST output is requested.  No call on
+ *     the path allocates or frees pinned memory; petar_tree_build creates the small host handle (and, with
+ *     profiling on, its CUDA events) once, petar_tree_rebuild reuses it.
  *   - Return value: 0 = PETAR_OK, negative = error (below).  No exceptions, no exit(), no stdout.
  *     Data-dependent failures found on the device (non-finite input, node/list/neighbour capacity
  *     exceeded) are recorded in a device status word, see petar_tree_status.
@@ -61,6 +63,10 @@ typedef struct {
     int32_t flags;          /* reserved, must be 0                                                  */
     double list_entries_per_particle; /* sizing of the interaction-list arena in 4-byte entries per
                                particle; <= 0 selects the default (see petar_workspace_bytes)       */
+    double nodes_per_particle; /* sizing of the node table: capacity = nodes_per_particle * N + 4096; <= 0
+                               selects the default (1 for n_leaf_limit >= 4, else 3).  The octree keeps
+                               single-child chains (rule O5), so deep tight binaries with small leaves can
+                               need more: PETAR_ST_NODE_CAP reports it, this field raises the capacity     */
 } petar_params;
 
 /* Interaction counters (HOST struct).  Self pairs are counted in n_epep, as in rule O7.            */
@@ -74,11 +80,13 @@ typedef struct {
     int64_t list_entries_used; /* 4-byte arena entries used                                         */
     int64_t n_epsp_common;  /* part of n_epsp evaluated super-group-wide (cells every i-group of a
                                super-group accepts; force phase A)             */
+    int64_t n_refined;      /* particles whose force nearly cancels (|a| < 2e-3 of the summed magnitudes) and
+                               was therefore re-evaluated in fp64                */
 } petar_counts;
 
 /* HOST-only query: bytes of device workspace petar_tree_build needs for N particles.
  * Returns 0 if N < 0 or the parameters are invalid.  Sized for: sorted copies of the inputs, keys,
- * the node table (capacity N + 4096 nodes for n_leaf_limit >= 4, else 3N + 4096), group table and
+ * the node table (capacity nodes_per_particle * N + 4096 nodes), group table and
  * the list arena (default 1024 entries per particle, at least 16 Mi entries).                        */
 size_t petar_workspace_bytes(int64_t N, const petar_params* p /* HOST */);
 
@@ -96,6 +104,13 @@ int petar_tree_build(const double* x, const double* y, const double* z, const do
                      const petar_params* p /* HOST */, void* workspace, size_t workspace_bytes,
                      void* cuda_stream, petar_tree** tree_out /* HOST */);
 
+/* The same steps into an EXISTING handle: same N, parameters and workspace as the petar_tree_build that
+ * created it, new (or moved) particle arrays.  Nothing is allocated, created or synchronised; lists and
+ * results of the previous tree are invalidated.  This is the call of a time-stepping loop.
+ * Errors: PETAR_ENOTBUILT (bad handle), PETAR_EINVAL (NULL array), PETAR_ECUDA.                     */
+int petar_tree_rebuild(petar_tree* t, const double* x, const double* y, const double* z, const double* m,
+                       const double* r_out, const double* r_search, void* cuda_stream);
+
 /* Steps S7-S8: per-group interaction-list walk (cell forced open when its box comes within
  * max(rmax_group, rmax_cell) of the group's box, else accepted iff edge < theta * distance, rule O7)
  * and the fp32 pairwise force + potential kernel (rule O8) with the changeover weights (Eq. 15-17).
@@ -103,6 +118,8 @@ int petar_tree_build(const double* x, const double* y, const double* z, const do
  *                              long-range potential phi_L,i (negative).  Any may be NULL (skipped).
  *   counts_host_or_null      : HOST; if non-NULL the call synchronises the stream and fills it, and
  *                              returns PETAR_ESTATUS if the device status word is non-zero.
+ * When the status word is non-zero (capacity exceeded, non-finite input) the force kernels write NOTHING:
+ * the outputs keep their previous contents; check petar_tree_status (or pass counts) before using them.
  * Errors: PETAR_ENOTBUILT, PETAR_ECUDA, PETAR_ESTATUS.                                              */
 int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_y, double* acc_z, double* pot,
                            petar_counts* counts_host_or_null, void* cuda_stream);

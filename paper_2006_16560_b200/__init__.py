@@ -9,7 +9,7 @@ calls raise.
 from .binding import (  # noqa: F401
     PetarParams, PetarCounts, PetarError, Tree,
     lib, library_path, exported_symbols,
-    petar_workspace_bytes, petar_tree_build, petar_long_range_force, petar_neighbor_list,
+    petar_workspace_bytes, petar_tree_build, petar_tree_rebuild, petar_long_range_force, petar_neighbor_list,
     petar_tree_status, petar_tree_destroy, petar_strerror, petar_debug_export,
     petar_set_profiling, petar_stage_times, petar_launch_count, petar_probe_fp32, petar_probe_fp32_mode,
     petar_search_radii, petar_neighbor_list_orbit, petar_clusters_workspace_bytes, petar_clusters,

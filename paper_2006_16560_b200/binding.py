@@ -5,11 +5,11 @@ import ctypes as C
 import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.environ.get("PETAR_B200_LIB", os.path.join(HERE, "libpetar_b200.so"))   # override: tuning experiments only
+_LIB_PATH = os.path.join(HERE, "libpetar_b200.so")
 _LIB = None
 
 EXPORTS = [
-    "petar_workspace_bytes", "petar_tree_build", "petar_long_range_force", "petar_neighbor_list",
+    "petar_workspace_bytes", "petar_tree_build", "petar_tree_rebuild", "petar_long_range_force", "petar_neighbor_list",
     "petar_tree_status", "petar_tree_destroy", "petar_strerror", "petar_debug_export",
     "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32", "petar_probe_fp32_mode",
     "petar_search_radii", "petar_neighbor_list_orbit", "petar_clusters_workspace_bytes", "petar_clusters",
@@ -30,12 +30,12 @@ class PetarError(RuntimeError):
 class PetarParams(C.Structure):
     _fields_ = [("G", C.c_double), ("theta", C.c_double), ("r_in_over_r_out", C.c_double),
                 ("multipole", C.c_int32), ("n_leaf_limit", C.c_int32), ("n_group_limit", C.c_int32),
-                ("flags", C.c_int32), ("list_entries_per_particle", C.c_double)]
+                ("flags", C.c_int32), ("list_entries_per_particle", C.c_double), ("nodes_per_particle", C.c_double)]
 
     @classmethod
-    def make(cls, theta, multipole, G=1.0, rho=0.1, n_leaf=8, n_group=64, list_entries_per_particle=0.0):
+    def make(cls, theta, multipole, G=1.0, rho=0.1, n_leaf=8, n_group=64, list_entries_per_particle=0.0, nodes_per_particle=0.0):
         return cls(float(G), float(theta), float(rho), int(multipole), int(n_leaf), int(n_group), 0,
-                   float(list_entries_per_particle))
+                   float(list_entries_per_particle), float(nodes_per_particle))
 
     @classmethod
     def from_workload(cls, w, theta=None, multipole=None, **kw):
@@ -45,7 +45,7 @@ class PetarParams(C.Structure):
 
 class PetarCounts(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("n_groups", "n_nodes", "n_epep", "n_epsp", "n_epep_near", "n_ep_list",
-                                         "n_sp_list", "list_entries_used", "n_epsp_common")]
+                                         "n_sp_list", "list_entries_used", "n_epsp_common", "n_refined")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -68,6 +68,8 @@ def lib():
         L.petar_tree_build.restype = C.c_int
         L.petar_tree_build.argtypes = [C.c_void_p] * 6 + [C.c_int64, C.POINTER(PetarParams), C.c_void_p, C.c_size_t,
                                                           C.c_void_p, C.POINTER(C.c_void_p)]
+        L.petar_tree_rebuild.restype = C.c_int
+        L.petar_tree_rebuild.argtypes = [C.c_void_p] * 7 + [C.c_void_p]
         L.petar_long_range_force.restype = C.c_int
         L.petar_long_range_force.argtypes = [C.c_void_p] * 5 + [C.POINTER(PetarCounts), C.c_void_p]
         L.petar_neighbor_list.restype = C.c_int
@@ -149,6 +151,13 @@ def petar_tree_build(x, y, z, m, r_out, r_search, N, params, workspace, stream=N
     if rc:
         raise PetarError(rc, "petar_tree_build")
     return h
+
+
+def petar_tree_rebuild(tree, x, y, z, m, r_out, r_search, stream=None) -> None:
+    """Steps S0-S6 into an existing handle (same N, parameters and workspace)."""
+    rc = lib().petar_tree_rebuild(tree, _ptr(x), _ptr(y), _ptr(z), _ptr(m), _ptr(r_out), _ptr(r_search), _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_tree_rebuild")
 
 
 def petar_long_range_force(tree, acc_x, acc_y, acc_z, pot, want_counts=False, stream=None):
@@ -322,10 +331,10 @@ class Tree:
         return self.inputs
 
     def build(self, stream=None):
-        if self.handle is not None:
-            petar_tree_destroy(self.handle)
-            self.handle = None
-        self.handle = petar_tree_build(*self.inputs, self.N, self.params, self.workspace, stream)
+        if self.handle is None:
+            self.handle = petar_tree_build(*self.inputs, self.N, self.params, self.workspace, stream)
+        else:
+            petar_tree_rebuild(self.handle, *self.inputs, stream)
         return self.handle
 
     def force(self, want_counts=False, stream=None):

@@ -35,6 +35,8 @@ void stage_end(petar_tree* t, int stage, cudaStream_t s) {
     t->stage_rec[stage] = 1;
 }
 
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_last_cuda = e_; return PETAR_ECUDA; } } while (0)
+
 static inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 static bool params_ok(const petar_params* p) {
@@ -44,10 +46,19 @@ static bool params_ok(const petar_params* p) {
     if (p->n_leaf_limit < 1 || p->n_leaf_limit > 64) return false;
     if (p->n_group_limit < p->n_leaf_limit || p->n_group_limit > 64) return false;
     if (p->flags != 0) return false;
+    if (!(p->list_entries_per_particle == p->list_entries_per_particle) || !(p->nodes_per_particle == p->nodes_per_particle)) return false;
     return true;
 }
 
-static int node_capacity(int64_t N, const petar_params* p) { return (int)((p->n_leaf_limit >= 4 ? N : 3 * N) + 4096); }
+// default: N + 4096 nodes for n_leaf_limit >= 4, else 3N + 4096 (measured: 0.35 N at config 3 with leaves of 8).  Rule O5 keeps
+// single-child chains, so no multiple of N is a hard bound (a tight binary deep in the tree adds a node per level):
+// nodes_per_particle raises the capacity, PETAR_ST_NODE_CAP reports an overflow.
+static int node_capacity(int64_t N, const petar_params* p) {
+    double per = p->nodes_per_particle > 0.0 ? p->nodes_per_particle : (p->n_leaf_limit >= 4 ? 1.0 : 3.0);
+    double cap = per * (double)N + 4096.0;
+    if (cap > 2.0e9) cap = 2.0e9;
+    return (int)cap;
+}
 static long long arena_chunks_for(int64_t N, const petar_params* p) {
     double per = p->list_entries_per_particle > 0.0 ? p->list_entries_per_particle : 1024.0;
     double entries = per * (double)N;
@@ -77,7 +88,7 @@ static size_t carve(Workspace* w, char* base, int64_t N, const petar_params* p) 
     W->D = (signed char*)take(n + 1); W->depth = (signed char*)take(n); W->glevel = (signed char*)take(n);
     W->gflag = (int*)take((2 * (n + 1)) * 4);
     W->tile_cnt = (int*)take((size_t)PETAR_NLEVELS * ntile * 4);
-    W->scan_tmp = (int*)take((size_t)(n / 4096 + 8) * 8);
+    W->scan_tmp = (int*)take((size_t)(3 * (n + 1) / 4096 + 8) * 8);     // partials of the longest scan (3 entries per group, list export)
     W->node_cap = node_capacity(N, p);
     W->nint = (NodeInt*)take((size_t)W->node_cap * sizeof(NodeInt));
     W->nmac = (NodeMac*)take((size_t)W->node_cap * sizeof(NodeMac));
@@ -91,6 +102,8 @@ static size_t carve(Workspace* w, char* base, int64_t N, const petar_params* p) 
     W->unit_cap = (int)(PETAR_NSUP * (N + 64));             // every unit holds at least one particle
     W->units = (ForceUnit*)take((size_t)W->unit_cap * sizeof(ForceUnit));
     W->part = (double*)take((size_t)PETAR_NSUP * n * 4 * 8);
+    W->part_s = (double*)take((size_t)PETAR_NSUP * n * 8);
+    W->refine_q = (int*)take(n * 2 * 4);
     W->nb_cnt = (int*)take(n * 4);
     W->nb_queue = (int*)take(((size_t)W->group_cap + 1) * 4);
     W->exp_scratch = (int*)take((10 * (n + 1) + 8) * 4);
@@ -105,7 +118,31 @@ extern "C" size_t petar_workspace_bytes(int64_t N, const petar_params* p) {
     return carve(nullptr, nullptr, N, p) + 256;
 }
 
-#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_last_cuda = e_; return PETAR_ECUDA; } } while (0)
+static void free_handle(petar_tree* t) {
+    if (t->ev) { for (int k = 0; k < 2 * PETAR_N_STAGES + 1; ++k) if (t->ev[k]) cudaEventDestroy(t->ev[k]); delete[] t->ev; }
+    t->magic = 0;
+    delete t;
+}
+
+// S0-S6 into the handle's workspace (shared by petar_tree_build and petar_tree_rebuild)
+static int build_into(petar_tree* t, const double* x, const double* y, const double* z, const double* m, const double* r_out,
+                      const double* r_search, cudaStream_t s) {
+    t->x = x; t->y = y; t->z = z; t->m = m; t->r_out = r_out; t->r_search = r_search;
+    t->built = false; t->walked = false;
+    for (int k = 0; k < PETAR_N_STAGES; ++k) t->stage_rec[k] = 0;
+    if (g_profiling && !t->ev) {            // events are created once per handle, never on a rebuild
+        t->ev = new (std::nothrow) cudaEvent_t[2 * PETAR_N_STAGES + 1];
+        if (!t->ev) return PETAR_EINVAL;
+        for (int k = 0; k < 2 * PETAR_N_STAGES + 1; ++k) t->ev[k] = nullptr;
+        for (int k = 0; k < 2 * PETAR_N_STAGES + 1; ++k) CK(cudaEventCreate(&t->ev[k]));
+    }
+    if (t->N > 0) {
+        CK(launch_keys_sort_gather(t, s));
+        CK(launch_tree(t, s));
+    }
+    t->built = true;
+    return PETAR_OK;
+}
 
 extern "C" int petar_tree_build(const double* x, const double* y, const double* z, const double* m, const double* r_out,
                                 const double* r_search, int64_t N, const petar_params* p, void* workspace,
@@ -120,26 +157,23 @@ extern "C" int petar_tree_build(const double* x, const double* y, const double* 
     if (!t) return PETAR_EINVAL;
     memset(t, 0, sizeof(*t));
     t->magic = PETAR_MAGIC; t->N = N; t->p = *p;
-    t->x = x; t->y = y; t->z = z; t->m = m; t->r_out = r_out; t->r_search = r_search;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
+    t->workspace = workspace; t->workspace_bytes = workspace_bytes;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&t->pinned, 64 * sizeof(long long));
-    if (e == cudaSuccess && g_profiling) {
-        t->ev = new (std::nothrow) cudaEvent_t[2 * PETAR_N_STAGES + 1];
-        for (int k = 0; t->ev && k < 2 * PETAR_N_STAGES + 1 && e == cudaSuccess; ++k) e = cudaEventCreate(&t->ev[k]);
-    }
-    if (e != cudaSuccess) { g_last_cuda = e; delete t; return PETAR_ECUDA; }
-    if (N > 0) {
-        carve(&t->w, (char*)workspace, N, p);
-        e = launch_keys_sort_gather(t, s);
-        if (e == cudaSuccess) e = launch_tree(t, s);
-        if (e != cudaSuccess) { g_last_cuda = e; cudaFreeHost(t->pinned); delete t; return PETAR_ECUDA; }
-    }
-    t->built = true; t->walked = false;
+    if (e != cudaSuccess) { g_last_cuda = e; free_handle(t); return PETAR_ECUDA; }
+    if (N > 0) carve(&t->w, (char*)workspace, N, p);
+    int rc = build_into(t, x, y, z, m, r_out, r_search, (cudaStream_t)cuda_stream);
+    if (rc) { free_handle(t); return rc; }
     *tree_out = t;
     return PETAR_OK;
+}
+
+extern "C" int petar_tree_rebuild(petar_tree* t, const double* x, const double* y, const double* z, const double* m,
+                                  const double* r_out, const double* r_search, void* cuda_stream) {
+    if (!t || t->magic != PETAR_MAGIC) return PETAR_ENOTBUILT;
+    if (t->N > 0 && (!x || !y || !z || !m || !r_out)) return PETAR_EINVAL;
+    return build_into(t, x, y, z, m, r_out, r_search, (cudaStream_t)cuda_stream);
 }
 
 static int check_tree(petar_tree* t) { return (t && t->magic == PETAR_MAGIC && t->built) ? PETAR_OK : PETAR_ENOTBUILT; }
@@ -151,7 +185,7 @@ static int ensure_walk(petar_tree* t, cudaStream_t s) {
     return PETAR_OK;
 }
 
-// reads the device header into t->pinned (as DevHeader) and synchronises
+// reads the device header into *out (HOST) and synchronises
 static int read_header(petar_tree* t, cudaStream_t s, DevHeader* out) {
     CK(cudaMemcpyAsync(out, t->w.hdr, sizeof(DevHeader), cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
@@ -176,6 +210,7 @@ extern "C" int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_
         counts->n_ep_list = (int64_t)hh.n_ep_list; counts->n_sp_list = (int64_t)hh.n_sp_list;
         counts->list_entries_used = (int64_t)hh.arena_top * PETAR_CHUNK;
         counts->n_epsp_common = (int64_t)hh.n_epsp_common;
+        counts->n_refined = (int64_t)hh.n_refine;
         if (hh.status) return PETAR_ESTATUS;
     }
     return PETAR_OK;
@@ -258,10 +293,7 @@ extern "C" int petar_tree_status(petar_tree* t, int32_t* status_host, void* cuda
 extern "C" int petar_tree_destroy(petar_tree* t) {
     if (!t) return PETAR_OK;
     if (t->magic != PETAR_MAGIC) return PETAR_ENOTBUILT;
-    t->magic = 0; t->built = false;
-    if (t->pinned) cudaFreeHost(t->pinned);
-    if (t->ev) { for (int k = 0; k < 2 * PETAR_N_STAGES + 1; ++k) cudaEventDestroy(t->ev[k]); delete[] t->ev; }
-    delete t;
+    free_handle(t);
     return PETAR_OK;
 }
 
@@ -286,7 +318,7 @@ extern "C" int petar_debug_export(petar_tree* t, int what, void* dst, size_t dst
     DevHeader hh;
     rc = read_header(t, s, &hh);
     if (rc) return rc;
-    t->pinned[0] = hh.n_nodes; t->pinned[1] = hh.n_groups;
+    t->h_nodes = hh.n_nodes; t->h_groups = hh.n_groups;
     const size_t n = (size_t)t->N;
     const Workspace& w = t->w;
     auto copy = [&](const void* src, size_t bytes) -> int {

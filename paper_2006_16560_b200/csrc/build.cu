@@ -519,7 +519,10 @@ __global__ void __launch_bounds__(256) k_moments(const DevHeader* __restrict__ h
                 NodeW wr;
                 const float l0 = (float)(lo0 - cx), l1 = (float)(lo1 - cy), l2 = (float)(lo2 - cz);
                 const float h0 = (float)(hi0 - cx), h1 = (float)(hi1 - cy), h2 = (float)(hi2 - cz);
-                const float amax = fmaxf(fmaxf(fmaxf(fabsf(l0), fabsf(h0)), fmaxf(fabsf(l1), fabsf(h1))), fmaxf(fabsf(l2), fabsf(h2)));
+                // largest |coordinate| of anything the walk's fp32 tests read from this record: the tight box and the centre of
+                // mass (for a massless cell, or with negative masses, the latter can lie outside the box)
+                const float amax = fmaxf(fmaxf(fmaxf(fmaxf(fabsf(l0), fabsf(h0)), fmaxf(fabsf(l1), fabsf(h1))), fmaxf(fabsf(l2), fabsf(h2))),
+                                         fmaxf(fmaxf(fabsf(xh), fabsf(yh)), fabsf(zh)));
                 wr.a = make_float4(l0, l1, l2, h0);
                 wr.b = make_float4(h1, h2, xh, yh);
                 wr.c = make_float4(zh, (float)rmax, amax * 4.8e-7f, 0.f);
@@ -573,7 +576,7 @@ __global__ void __launch_bounds__(256) k_groups_finish(GroupRec* __restrict__ gr
             r->end = e; r->head_sp = r->head_epn = r->head_epf = -1;
             r->n_sp = r->n_epn = r->n_epf = 0; r->n_ep_part = r->n_epn_part = 0; r->head_spp = -1; r->n_spp = 0;
             for (int k = 0; k < 3; ++k) { r->lo[k] = lo[k]; r->hi[k] = hi[k]; }
-            r->rmax = rmax; r->sid[0] = 0; r->sid[1] = 0;
+            r->rmax = rmax; for (int l = 0; l < PETAR_NSUP; ++l) r->sid[l] = 0;
         }
     }
 }

@@ -6,6 +6,13 @@
 // Member lists: stable radix sort of (label, particle index), cluster starts by a flag scan.
 #include "internal.cuh"
 
+// multiprocessors of the current device (queried once)
+static int sm_count() {
+    static int n = 0;
+    if (n == 0) { int dev = 0; if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148; }
+    return n;
+}
+
 __device__ __forceinline__ int cc_find(int* __restrict__ parent, int a) {
     int p = ((volatile int*)parent)[a];
     while (p != a) {
@@ -90,7 +97,7 @@ cudaError_t launch_clusters(const long long* offsets, const int* indices, long l
     const int nb = cdiv(n, 256);
     k_cc_init<<<nb, 256, 0, s>>>(label, n, n_clusters_dev);
     KCHECK(s, "k_cc_init");
-    k_cc_union<<<148 * 16, 256, 0, s>>>(offsets, indices, n, label);
+    k_cc_union<<<sm_count() * 16, 256, 0, s>>>(offsets, indices, n, label);
     KCHECK(s, "k_cc_union");
     k_cc_flatten<<<nb, 256, 0, s>>>(label, n, n_clusters_dev);
     KCHECK(s, "k_cc_flatten");

@@ -44,6 +44,8 @@
 #define PRAGMA_(x) PRAGMA_STR_(x)
 #define UNROLL_J PRAGMA_(unroll FORCE_UNROLL)
 #define EP_TILE 512            // particles per staged tile
+// a particle with |a| < REFINE_KAPPA * s (s: see Acc64) is re-evaluated in fp64 by k_force_refine
+#define REFINE_KAPPA 2.0e-3
 
 struct ForceConst {
     float c1, c0;              // x = r * inv_R * c1 - c0,  c1 = 1/(1-rho), c0 = rho/(1-rho)
@@ -55,9 +57,14 @@ struct ForceConst {
 __device__ __forceinline__ float rsqrt_ftz(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 struct Acc32 { float ax, ay, az, pot; };      // pot accumulates +sum m (1-W)/r; sign applied at the end
-struct Acc64 { double ax, ay, az, pot; };
+// fp64 sums of one particle.  s = sum over the flushed fp32 partial sums of |ax| + |ay| + |az|: the size of what was added
+// up before cancellation (partial sums run over <= ~64 spatially coherent terms).  |a| << s marks a particle whose
+// long-range force nearly cancels (the cluster centre): its fp32 terms carry an absolute error ~1e-7 s / sqrt(terms),
+// which the refinement kernel below removes.
+struct Acc64 { double ax, ay, az, pot, s; };
 __device__ __forceinline__ void flush(Acc32& p, Acc64& a) {
     a.ax += (double)p.ax; a.ay += (double)p.ay; a.az += (double)p.az; a.pot += (double)p.pot;
+    a.s += (double)(fabsf(p.ax) + fabsf(p.ay) + fabsf(p.az));
     p.ax = p.ay = p.az = p.pot = 0.0f;
 }
 
@@ -107,6 +114,8 @@ struct Acc2 { f2 ax, ay, az, pot; };            // .x = first particle of the pa
 __device__ __forceinline__ void flush(Acc2& p, Acc64& a0, Acc64& a1) {
     a0.ax += (double)p.ax.x; a0.ay += (double)p.ay.x; a0.az += (double)p.az.x; a0.pot += (double)p.pot.x;
     a1.ax += (double)p.ax.y; a1.ay += (double)p.ay.y; a1.az += (double)p.az.y; a1.pot += (double)p.pot.y;
+    a0.s += (double)(fabsf(p.ax.x) + fabsf(p.ay.x) + fabsf(p.az.x));
+    a1.s += (double)(fabsf(p.ax.y) + fabsf(p.ay.y) + fabsf(p.az.y));
     p.ax = p.ay = p.az = p.pot = make_float2(0.f, 0.f);
 }
 // cell_term for a pair of i-particles (same algebra, see above)
@@ -189,7 +198,7 @@ struct SpBuf { float4 q0[SP_TILE], q1[SP_TILE], q2[SP_TILE]; float q3[SP_TILE]; 
 union __align__(16) ForceSmem {
     SpBuf sp[2];                                                       // 26 KB
     struct { float4 a[EP_TILE], b[EP_TILE]; int j[EP_TILE]; } ep;      // 18 KB
-    double red[FT * 8];                                                // 8 KB
+    double red[FT * 10];                                               // 10 KB
 };
 
 // uniform cursor over the tiles (<= SP_TILE entries, never straddling a chunk) of TWO chunked lists in a
@@ -318,14 +327,17 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
 template <bool QUAD>
 __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
                                                  const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
-                                                 const unsigned* __restrict__ perm, const double* __restrict__ part, const long long n_part,
+                                                 const unsigned* __restrict__ perm, const double* __restrict__ part, const double* __restrict__ part_s,
+                                                 const long long n_part, int* __restrict__ refine_q,
                                                  double* __restrict__ oax, double* __restrict__ oay, double* __restrict__ oaz, double* __restrict__ opot,
                                                  ForceConst fc, double G) {
     __shared__ ForceSmem sm;
+    __shared__ double s_fin[64][5];
     __shared__ int s_g;
     __shared__ int s_scan[FT / 32];
     const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
     const int ng = h->n_groups;
+    if (h->status != 0) return;            // capacity exceeded / non-finite input: lists are unusable, write nothing (petar.h)
     const double rcx = h->c[0], rcy = h->c[1], rcz = h->c[2];
     for (;;) {
         __syncthreads();
@@ -349,7 +361,7 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
             gh = make_float3((float)cx, (float)cy, (float)cz);
             gl = make_float3((float)(cx - (double)gh.x), (float)(cy - (double)gh.y), (float)(cz - (double)gh.z));
         }
-        Acc64 acc0 = {0, 0, 0, 0}, acc1 = {0, 0, 0, 0};
+        Acc64 acc0 = {0, 0, 0, 0, 0}, acc1 = {0, 0, 0, 0, 0};
 
         // the group's own cells (the cells common to its super-groups were summed by k_force_units into `part`)
         sp_phase<QUAD, false>(sm, arena, nsp, -1, 0, gr->head_sp, gr->n_sp, t, slice, S, active, ia0, ib0, ia1, ib1, gh, gl, acc0, acc1);
@@ -422,27 +434,156 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
         // ---- ordered reduction over slices, then scatter to the caller's order --------------------
         __syncthreads();
         if (active) {
-            double* r = &sm.red[(size_t)(slice * (2 * P) + 2 * pslot) * 4];
-            r[0] = acc0.ax; r[1] = acc0.ay; r[2] = acc0.az; r[3] = acc0.pot;
-            r[4] = acc1.ax; r[5] = acc1.ay; r[6] = acc1.az; r[7] = acc1.pot;
+            double* r = &sm.red[(size_t)(slice * (2 * P) + 2 * pslot) * 5];
+            r[0] = acc0.ax; r[1] = acc0.ay; r[2] = acc0.az; r[3] = acc0.pot; r[4] = acc0.s;
+            r[5] = acc1.ax; r[6] = acc1.ay; r[7] = acc1.az; r[8] = acc1.pot; r[9] = acc1.s;
         }
         __syncthreads();
-        for (int k = t; k < n_i * 4; k += FT) {
-            const int i = k >> 2, comp = k & 3;
-            double s = 0.0;
+        for (int k = t; k < n_i * 5; k += FT) {
+            const int i = k / 5, comp = k - 5 * i;
+            double q = 0.0;
 #pragma unroll
-            for (int l = 0; l < PETAR_NSUP; ++l) s += part[((size_t)l * n_part + gb + i) * 4 + comp];
-            for (int sl = 0; sl < S; ++sl) s += sm.red[(size_t)(sl * (2 * P) + i) * 4 + comp];
-            const unsigned o = perm[gb + i];
-            if (comp == 3) { if (opot) opot[o] = -G * s; }
-            else {
-                double* dst = comp == 0 ? oax : comp == 1 ? oay : oaz;
-                if (dst) dst[o] = G * s;
+            for (int l = 0; l < PETAR_NSUP; ++l)
+                q += comp < 4 ? part[((size_t)l * n_part + gb + i) * 4 + comp] : part_s[(size_t)l * n_part + gb + i];
+            for (int sl = 0; sl < S; ++sl) q += sm.red[(size_t)(sl * (2 * P) + i) * 5 + comp];
+            s_fin[i][comp] = q;
+        }
+        __syncthreads();
+        if (t < n_i) {
+            const double v0 = s_fin[t][0], v1 = s_fin[t][1], v2 = s_fin[t][2], v3 = s_fin[t][3], v4 = s_fin[t][4];
+            const unsigned o = perm[gb + t];
+            if (oax) oax[o] = G * v0;
+            if (oay) oay[o] = G * v1;
+            if (oaz) oaz[o] = G * v2;
+            if (opot) opot[o] = -G * v3;
+            // near-cancelling force: queue the particle for the fp64 re-evaluation (k_force_refine)
+            if (v0 * v0 + v1 * v1 + v2 * v2 < (REFINE_KAPPA * REFINE_KAPPA) * v4 * v4) {
+                const int at = atomicAdd(&h->n_refine, 1);
+                refine_q[2 * (size_t)at] = g; refine_q[2 * (size_t)at + 1] = gb + t;
             }
         }
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// fp64 re-evaluation of the particles whose long-range force nearly cancels (queued by k_force: |a| < REFINE_KAPPA * s).
+// One warp per particle; the lanes run over the entries of every list the particle's force is made of -- the common
+// cells of its super-groups (every level), its group's own cells, the near and the far leaf ranges -- with rule O8 in
+// fp64 from the fp64 node and particle tables (Eq. 11, 15-17, 30-31; the same formulas as the fp32 kernels).  The
+// results replace the fp32 ones.  A few hundred particles of a million (the cluster centre); the cost is negligible.
+// ------------------------------------------------------------------------------------------------
+struct RefineArgs {
+    const GroupRec* grp; const SuperRec* srec; int group_cap;
+    const int* arena; const NodeMac* nmac; const NodeMom* nmom;
+    const double *xs, *ys, *zs, *ms, *routs;
+    const unsigned* perm; const int* queue;
+    double *oax, *oay, *oaz, *opot;
+    double G, rho; int quad;
+};
+struct Acc4d { double ax, ay, az, pot; };
+__device__ __forceinline__ void refine_cell(Acc4d& a, const NodeMac& c, const NodeMom& q, const bool quad, const double xi, const double yi, const double zi) {
+    const double dx = c.com[0] - xi, dy = c.com[1] - yi, dz = c.com[2] - zi;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double rinv = 1.0 / sqrt(r2), rinv2 = rinv * rinv, rinv3 = rinv * rinv2;
+    double f = q.M * rinv3, pot = q.M * rinv;
+    double qx = 0.0, qy = 0.0, qz = 0.0;
+    if (quad) {
+        const double tr = q.Q[0] + q.Q[1] + q.Q[2];
+        const double axx = 1.5 * q.Q[0] - 0.5 * tr, ayy = 1.5 * q.Q[1] - 0.5 * tr, azz = 1.5 * q.Q[2] - 0.5 * tr;
+        const double axy = 1.5 * q.Q[3], axz = 1.5 * q.Q[4], ayz = 1.5 * q.Q[5];
+        const double adx = axx * dx + axy * dy + axz * dz, ady = axy * dx + ayy * dy + ayz * dz, adz = axz * dx + ayz * dy + azz * dz;
+        const double dad = dx * adx + dy * ady + dz * adz;
+        const double rinv5 = rinv3 * rinv2;
+        pot += dad * rinv5;                                 // phi = -G [M/r + d A' d / r^5]
+        f += 5.0 * dad * rinv5 * rinv2;                     // a = M d/r^3 - 2 A' d/r^5 + 5 (d A' d) d/r^7,  d = com - x_i
+        qx = -2.0 * adx * rinv5; qy = -2.0 * ady * rinv5; qz = -2.0 * adz * rinv5;
+    }
+    a.ax += f * dx + qx; a.ay += f * dy + qy; a.az += f * dz + qz; a.pot += pot;
+}
+// pair term; near = the changeover weights 1-K (Eq. 17) and 1-W (Eq. 15) apply
+__device__ __forceinline__ void refine_pair(Acc4d& a, const bool near, const double dx, const double dy, const double dz, const double m, const double R,
+                                            const double rho) {
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double lam = (1.0 - rho) / (1.0 + rho);
+    if (!(r2 > 0.0)) { a.pot += m * (1.0 + lam) / R; return; }         // coincident j != i: no force, the constant potential (reading P4)
+    const double r = sqrt(r2), rinv = 1.0 / r;
+    double wk = 1.0, pw = rinv;
+    if (near && r < R) {
+        const double rin = rho * R;
+        double x = (r - rin) / (R - rin);
+        x = x < 0.0 ? 0.0 : x;
+        const double y = 1.0 - x, y4 = (y * y) * (y * y);
+        wk = 1.0 - y4 * (1.0 + 4.0 * x + 10.0 * x * x + 20.0 * x * x * x + 35.0 * lam * x * x * x * x);      // 1 - K
+        const double x5 = x * x * x * x * x;
+        pw = (1.0 + lam) / R - lam * x5 * (14.0 - 28.0 * x + 20.0 * x * x - 5.0 * x * x * x) * rinv;         // (1 - W)/r
+    }
+    const double f = m * wk * rinv * rinv * rinv;
+    a.ax += f * dx; a.ay += f * dy; a.az += f * dz; a.pot += m * pw;
+}
+__global__ void __launch_bounds__(256) k_force_refine(const DevHeader* __restrict__ h, const RefineArgs A) {
+    __shared__ double s_red[8][4];
+    const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
+    const int nq = h->n_refine;
+    if (h->status != 0) return;
+    for (int q = blockIdx.x; q < nq; q += gridDim.x) {          // one CTA per particle
+        const int g = A.queue[2 * (size_t)q], pos = A.queue[2 * (size_t)q + 1];
+        const GroupRec* gr = &A.grp[g];
+        const double xi = A.xs[pos], yi = A.ys[pos], zi = A.zs[pos], roi = A.routs[pos];
+        Acc4d a = {0.0, 0.0, 0.0, 0.0};
+        // cell lists: per level the common plain and precise lists, then the group's own two
+        for (int l = 0; l <= PETAR_NSUP; ++l) {
+            for (int which = 0; which < 2; ++which) {
+                int chunk, remaining;
+                if (l < PETAR_NSUP) { const SuperRec* sr = &A.srec[(size_t)l * A.group_cap + gr->sid[l]]; chunk = which ? sr->head_spp : sr->head_sp; remaining = which ? sr->n_spp : sr->n_sp; }
+                else { chunk = which ? gr->head_spp : gr->head_sp; remaining = which ? gr->n_spp : gr->n_sp; }
+                while (chunk >= 0 && remaining > 0) {
+                    const int* cp = A.arena + (size_t)chunk * PETAR_CHUNK;
+                    const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+                    for (int e = t; e < ne; e += 256) {
+                        const int id = cp[PETAR_CHUNK_HDR + e];
+                        refine_cell(a, A.nmac[id], A.nmom[id], A.quad != 0, xi, yi, zi);
+                    }
+                    remaining -= ne; chunk = cp[0];
+                }
+            }
+        }
+        // leaf ranges: near (changeover), far (Newtonian)
+        for (int pass = 0; pass < 2; ++pass) {
+            int chunk = pass == 0 ? gr->head_epn : gr->head_epf;
+            int remaining = 2 * (pass == 0 ? gr->n_epn : gr->n_epf);
+            while (chunk >= 0 && remaining > 0) {
+                const int* cp = A.arena + (size_t)chunk * PETAR_CHUNK;
+                const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+                for (int e = 2 * t; e < ne; e += 512) {
+                    const int jb = cp[PETAR_CHUNK_HDR + e], je = cp[PETAR_CHUNK_HDR + e + 1];
+                    for (int j = jb; j < je; ++j) {
+                        if (j == pos) continue;                 // the list holds the particle itself
+                        refine_pair(a, pass == 0, A.xs[j] - xi, A.ys[j] - yi, A.zs[j] - zi, A.ms[j], fmax(roi, A.routs[j]), A.rho);
+                    }
+                }
+                remaining -= ne; chunk = cp[0];
+            }
+        }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) {
+            a.ax += __shfl_xor_sync(0xffffffffu, a.ax, o); a.ay += __shfl_xor_sync(0xffffffffu, a.ay, o);
+            a.az += __shfl_xor_sync(0xffffffffu, a.az, o); a.pot += __shfl_xor_sync(0xffffffffu, a.pot, o);
+        }
+        __syncthreads();                                        // s_red of the previous particle consumed
+        if (lane == 0) { s_red[wrp][0] = a.ax; s_red[wrp][1] = a.ay; s_red[wrp][2] = a.az; s_red[wrp][3] = a.pot; }
+        __syncthreads();
+        if (t == 0) {
+            double v[4] = {0.0, 0.0, 0.0, 0.0};
+            for (int ww = 0; ww < 8; ++ww) for (int c = 0; c < 4; ++c) v[c] += s_red[ww][c];
+            const unsigned o = A.perm[pos];
+            if (A.oax) A.oax[o] = A.G * v[0];
+            if (A.oay) A.oay[o] = A.G * v[1];
+            if (A.oaz) A.oaz[o] = A.G * v[2];
+            if (A.opot) A.opot[o] = -A.G * v[3];
+        }
+    }
+}
 
 // ------------------------------------------------------------------------------------------------
 // Phase A: the cells COMMON to a super-group (accepted once for all of its i-groups by k_walk_super)
@@ -491,11 +632,13 @@ struct WarpTileCursor {
     }
 };
 
-// fp64 accumulators of phase A live in shared memory (s_acc[component][thread], conflict-free): 16 per lane
-// (a: the accumulators of the pair's first particle; the second particle's follow 4 components later)
+// fp64 accumulators of phase A live in shared memory (s_acc[component][thread], conflict-free): 20 per lane
+// (a: the accumulators of the pair's first particle, ax ay az pot s; the second particle's follow 5 components later)
 __device__ __forceinline__ void flush_smem(Acc2& p, double* __restrict__ a) {
     a[0] += (double)p.ax.x; a[UW * 32] += (double)p.ay.x; a[2 * UW * 32] += (double)p.az.x; a[3 * UW * 32] += (double)p.pot.x;
-    a[4 * UW * 32] += (double)p.ax.y; a[5 * UW * 32] += (double)p.ay.y; a[6 * UW * 32] += (double)p.az.y; a[7 * UW * 32] += (double)p.pot.y;
+    a[4 * UW * 32] += (double)(fabsf(p.ax.x) + fabsf(p.ay.x) + fabsf(p.az.x));
+    a[5 * UW * 32] += (double)p.ax.y; a[6 * UW * 32] += (double)p.ay.y; a[7 * UW * 32] += (double)p.az.y; a[8 * UW * 32] += (double)p.pot.y;
+    a[9 * UW * 32] += (double)(fabsf(p.ax.y) + fabsf(p.ay.y) + fabsf(p.az.y));
     p.ax = p.ay = p.az = p.pot = make_float2(0.f, 0.f);
 }
 
@@ -596,7 +739,7 @@ __device__ __forceinline__ void unit_phase(UBuf* __restrict__ bufs, const int* _
             if (++fl >= fl_every) {
                 fl = 0;
 #pragma unroll
-                for (int k = 0; k < NIv / 2; ++k) flush_smem(p[k], sacc + 8 * k * (UW * 32));
+                for (int k = 0; k < NIv / 2; ++k) flush_smem(p[k], sacc + 10 * k * (UW * 32));
             }
         }
         store_recs(bufs[cb ^ 1]); tn0 = tn1;
@@ -607,7 +750,7 @@ __device__ __forceinline__ void unit_phase(UBuf* __restrict__ bufs, const int* _
     }
     if (active) {
 #pragma unroll
-        for (int k = 0; k < NIv / 2; ++k) flush_smem(p[k], sacc + 8 * k * (UW * 32));
+        for (int k = 0; k < NIv / 2; ++k) flush_smem(p[k], sacc + 10 * k * (UW * 32));
     }
 }
 
@@ -622,7 +765,7 @@ __device__ __forceinline__ void unit_run(UBuf* __restrict__ bufs, const int* __r
     const bool active = slice < S;
     const int i0 = ibeg + NIv * slot, ilast = ibeg + cnt - 1;
 #pragma unroll
-    for (int c = 0; c < 4 * NIv; ++c) sacc[c * (UW * 32)] = 0.0;
+    for (int c = 0; c < 5 * NIv; ++c) sacc[c * (UW * 32)] = 0.0;
     unit_phase<QUAD, false, NIv>(bufs, arena, nsp, head_sp, n_sp, w, lane, slice, S, active, pa, pb, i0, ilast, gh, sacc);
     unit_phase<QUAD, true, NIv>(bufs, arena, nsp, head_spp, n_spp, w, lane, slice, S, active, pa, pb, i0, ilast, gh, sacc);
 }
@@ -640,13 +783,14 @@ __global__ void __launch_bounds__(UW * 32, UNITS_MIN_CTAS) k_force_units(DevHead
                                                             const int group_cap, const NodeW* __restrict__ nw,
                                                             const int* __restrict__ arena, const NodeSp* __restrict__ nsp,
                                                             const float4* __restrict__ pa, const float4* __restrict__ pb,
-                                                            double* __restrict__ part, const long long n_part) {
+                                                            double* __restrict__ part, double* __restrict__ part_s, const long long n_part) {
     __shared__ __align__(16) UBuf s_buf[UW][2];
-    __shared__ double s_acc[4 * NI][UW * 32];
+    __shared__ double s_acc[5 * NI][UW * 32];
     __shared__ int s_u;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     double* sacc = &s_acc[0][threadIdx.x];
     const int nu = h->unit_off[PETAR_UNIT_CLASSES];
+    if (h->status != 0) return;            // see k_force
     for (;;) {
         __syncthreads();                    // s_u and s_acc of the previous unit consumed
         if (threadIdx.x == 0) s_u = atomicAdd(&h->unit_ticket, 1);
@@ -667,12 +811,13 @@ __global__ void __launch_bounds__(UW * 32, UNITS_MIN_CTAS) k_force_units(DevHead
         __syncthreads();
         const int P = (cnt + ni - 1) / ni, S = 32 / P;
         double* out = part + ((size_t)fu.level * n_part + fu.ibeg) * 4;
-        for (int e = threadIdx.x; e < cnt * 4; e += UW * 32) {
-            const int i = e >> 2, comp = e & 3;
+        double* out_s = part_s + (size_t)fu.level * n_part + fu.ibeg;
+        for (int e = threadIdx.x; e < cnt * 5; e += UW * 32) {
+            const int i = e / 5, comp = e - 5 * i;
             double sum = 0.0;
             for (int ww = 0; ww < UW; ++ww)
-                for (int sl = 0; sl < S; ++sl) sum += s_acc[(i % ni) * 4 + comp][ww * 32 + sl * P + (i / ni)];
-            out[e] = sum;
+                for (int sl = 0; sl < S; ++sl) sum += s_acc[(i % ni) * 5 + comp][ww * 32 + sl * P + (i / ni)];
+            if (comp < 4) out[4 * i + comp] = sum; else out_s[i] = sum;
         }
     }
 }
@@ -739,7 +884,7 @@ __global__ void __launch_bounds__(256) k_units_fill(DevHeader* __restrict__ h, c
 }
 
 __global__ void k_reset_ticket2(DevHeader* h) {
-    if (threadIdx.x == 0) { h->group_ticket2 = 0; h->unit_ticket = 0; for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) h->unit_cnt[k] = 0; }
+    if (threadIdx.x == 0) { h->group_ticket2 = 0; h->unit_ticket = 0; h->n_refine = 0; for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) h->unit_cnt[k] = 0; }
 }
 
 // phase A: unit table, then the super-groups' common cells.  ctas_per_sm > 0 limits the grid (tuning
@@ -764,8 +909,8 @@ cudaError_t launch_force_units(petar_tree* t, cudaStream_t s, int ctas_per_sm) {
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     if (ctas_per_sm > 0 && ctas_per_sm < per_sm) per_sm = ctas_per_sm;
-    if (quad) k_force_units<true><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, (long long)t->N);
-    else k_force_units<false><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, (long long)t->N);
+    if (quad) k_force_units<true><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N);
+    else k_force_units<false><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N);
     KCHECK(s, "k_force_units");
     petar_count_launch(5);
     stage_end(t, PETAR_STAGE_FORCE_UNITS, s);
@@ -796,11 +941,18 @@ cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* a
     if (per_sm < 1) per_sm = 1;
     const int grid = t->sm_count * per_sm;
     if (quad)
-        k_force<true><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.part, (long long)t->N, ax, ay, az, pot, fc, t->p.G);
+        k_force<true><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.part, w.part_s, (long long)t->N, w.refine_q, ax, ay, az, pot, fc, t->p.G);
     else
-        k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.part, (long long)t->N, ax, ay, az, pot, fc, t->p.G);
+        k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.part, w.part_s, (long long)t->N, w.refine_q, ax, ay, az, pot, fc, t->p.G);
     KCHECK(s, "k_force");
-    petar_count_launch(1);
+    {
+        const double* rs = w.routs;
+        RefineArgs A = {w.grp, w.srec, w.group_cap, w.arena, w.nmac, w.nmom, w.xs, w.ys, w.zs, w.ms, rs, w.idx, w.refine_q,
+                        ax, ay, az, pot, t->p.G, t->p.r_in_over_r_out, quad ? 1 : 0};
+        k_force_refine<<<t->sm_count * 8, 256, 0, s>>>(w.hdr, A);
+        KCHECK(s, "k_force_refine");
+    }
+    petar_count_launch(2);
     stage_end(t, PETAR_STAGE_FORCE, s);
     return cudaGetLastError();
 }

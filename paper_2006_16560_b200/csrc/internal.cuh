@@ -20,7 +20,10 @@
 #ifndef PETAR_SUP_T1
 #define PETAR_SUP_T1 512
 #endif
-#define PETAR_SUP_LIMIT(l) ((l) == 0 ? PETAR_SUP_T0 : PETAR_SUP_T1)
+#ifndef PETAR_SUP_T2
+#define PETAR_SUP_T2 128
+#endif
+#define PETAR_SUP_LIMIT(l) ((l) == 0 ? PETAR_SUP_T0 : (l) == 1 ? PETAR_SUP_T1 : PETAR_SUP_T2)
 #define PETAR_UNIT_CLASSES 4       // phase-A force units of 128, 64, 32 and < 32 particles
 
 // ---- device-resident header (one per tree, lives at the start of the workspace) -----------------
@@ -45,7 +48,8 @@ struct DevHeader {
     int unit_off[PETAR_UNIT_CLASSES + 1];
     int unit_fill[PETAR_UNIT_CLASSES];
     int unit_ticket;
-    int pad_[2];
+    int n_refine;                  // particles queued for the fp64 re-evaluation (k_force_refine)
+    int pad_[1];
     unsigned long long n_epep, n_epsp, n_epep_near, n_ep_list, n_sp_list, n_epsp_common;
     unsigned long long nb_total;
 };
@@ -72,7 +76,7 @@ struct __align__(16) GroupRec {
     int n_ep_part, n_epn_part;         // particles in all EP ranges / in near ranges
     int head_spp, n_spp;               // cells closer than the group's own size: float-float ("precise") path
     double lo[3], hi[3], rmax;
-    int sid[2];                        // super-group (see SuperRec) of each level this group lies in
+    int sid[PETAR_NSUP];               // super-group (see SuperRec) of each level this group lies in
 };
 
 // super-group of level l: tree cell with <= PETAR_SUP_LIMIT(l) members (parent has more).  Its walk decides,
@@ -117,6 +121,8 @@ struct Workspace {
     int* smap;                     // [PETAR_NSUP][N] sorted position -> super-group id
     struct ForceUnit* units; int unit_cap;   // phase-A force units (force.cu)
     double* part;                  // [PETAR_NSUP][N][4] phase-A partial sums (sorted order): ax, ay, az, pot
+    double* part_s;                // [PETAR_NSUP][N] phase-A cancellation scale (Acc64::s)
+    int* refine_q;                 // [N][2] (group, sorted position) of the particles to re-evaluate in fp64
     // list arena
     int* arena; int arena_chunks;
     // neighbour temporaries
@@ -132,10 +138,11 @@ struct petar_tree {
     Workspace w;
     const double *x, *y, *z, *m, *r_out, *r_search;
     bool built, walked;
-    cudaEvent_t* ev;               // [2*PETAR_N_STAGES + 1] stage begin/end events (profiling only)
+    cudaEvent_t* ev;               // [2*PETAR_N_STAGES + 1] stage begin/end events (profiling only; created once per handle)
     int stage_rec[PETAR_N_STAGES];
     int sm_count;
-    int* pinned;                   // small pinned host buffer for header read-back
+    int h_nodes, h_groups;         // host copies of the header counters (filled by petar_debug_export)
+    void* workspace; size_t workspace_bytes;
 };
 
 #define PETAR_MAGIC 0x50335431u

@@ -11,6 +11,13 @@
 // 64-byte record gathered per list entry.
 #include "internal.cuh"
 
+// multiprocessors of the current device (queried once)
+static int sm_count() {
+    static int n = 0;
+    if (n == 0) { int dev = 0; if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148; }
+    return n;
+}
+
 #define SHORT_ROW 32
 
 // packed copy of the inputs: one 64-byte record per particle, so a gathered neighbour costs two sectors, not eight
@@ -133,7 +140,7 @@ extern "C" int petar_short_range_force(const double* x, const double* y, const d
     KCHECK(s, "k_short_pack");
     k_short_rows<<<cdiv(N, 256), 256, 0, s>>>(A, queue);
     KCHECK(s, "k_short_rows");
-    k_short_long_rows<<<148 * 4, 256, 0, s>>>(A, queue);
+    k_short_long_rows<<<sm_count() * 4, 256, 0, s>>>(A, queue);
     KCHECK(s, "k_short_long_rows");
     petar_count_launch(3);
     return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;

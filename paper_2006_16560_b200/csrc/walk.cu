@@ -289,9 +289,14 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
         const SuperRec* sr = &srec[(size_t)(PETAR_NSUP - 1) * group_cap + sid[PETAR_NSUP - 1]];
         int dchunk = sr->head_def, dremaining = sr->n_def, doff = 0;
         int top = 0;
-        while (top > 0 || dremaining > 0) {
+        // The loop is software-pipelined: the records of the NEXT batch of nodes are requested right after the
+        // current batch's children are pushed, so their latency is covered by the list output of the current batch.
+        int p = 0, node = -1;
+        NodeW c;
+        auto pop = [&]() {
+            p = 0; node = -1;
             if (top == 0) {                    // frontier empty: take the next (up to 256) deferred cells
-                if (dchunk < 0) break;         // truncated list (arena exhausted, PETAR_ST_LIST_CAP is set)
+                if (dremaining <= 0 || dchunk < 0) return;      // done (or truncated list: arena exhausted, PETAR_ST_LIST_CAP is set)
                 const int* cp = arena + (size_t)dchunk * PETAR_CHUNK;
                 const int k = min(256, min(dremaining, PETAR_CHUNK_PAYLOAD - doff));
                 for (int e = lane; e < k; e += 32) stack[e] = cp[PETAR_CHUNK_HDR + doff + e];
@@ -301,15 +306,19 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
             }
             // pop up to 32 nodes; throttle towards depth-first order when the frontier nears its capacity
             // (a pure depth-first descent adds at most 7 entries per level, < WALK_RESERVE in total)
-            int p = min(32, top);
+            p = min(32, top);
             if (top + 7 * p > WALK_STACK - WALK_RESERVE) p = max(1, min(p, (WALK_STACK - WALK_RESERVE - top) / 7));
-            const int node = (lane < p) ? stack[top - p + lane] : -1;
+            if (lane < p) node = stack[top - p + lane];
             top -= p;
             __syncwarp();
+            if (node >= 0) c = nw[node];
+        };
+        pop();
+        while (p > 0) {
             int act = -1;                      // 0 SP, 1 EP near, 2 EP far, 3 open, 4 SP (precise list)
             int nb = 0, ne = 0, fc = 0, nch = 0;
+            const int node_cur = node;
             if (node >= 0) {
-                const NodeW c = nw[node];
                 const int meta = c.d.w;
                 const int level = meta & 255;
                 const bool leaf = (meta >> 16) & 1;
@@ -339,17 +348,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
                 else act = mac_exact(&nmac[node], level, leaf, gr, theta, twoh);
                 if (act == 0 && d2b < gedge2) act = 4;
             }
-            // outputs
-            list_append(lsp, act == 0, 1, node, 0, arena, arena_chunks, h, lane);
-            list_append(lspp, act == 4, 1, node, 0, arena, arena_chunks, h, lane);
-            list_append(lepn, act == 1, 2, nb, ne, arena, arena_chunks, h, lane);
-            list_append(lepf, act == 2, 2, nb, ne, arena, arena_chunks, h, lane);
-            n_sp += __popc(__ballot_sync(0xffffffffu, act == 0));
-            n_spp += __popc(__ballot_sync(0xffffffffu, act == 4));
-            n_epn += __popc(__ballot_sync(0xffffffffu, act == 1));
-            n_epf += __popc(__ballot_sync(0xffffffffu, act == 2));
-            const int cn = __reduce_add_sync(0xffffffffu, (act == 1) ? (ne - nb) : 0);
-            const int cf = __reduce_add_sync(0xffffffffu, (act == 2) ? (ne - nb) : 0);
+            // children of the opened cells go to the frontier
             const int push = (act == 3) ? nch : 0;
             int pref = push;
 #pragma unroll
@@ -357,7 +356,6 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
                 int a = __shfl_up_sync(0xffffffffu, pref, o);
                 if (lane >= o) pref += a;
             }
-            n_epn_part += cn; n_ep_part += cn + cf;
             const int total_push = __shfl_sync(0xffffffffu, pref, 31);
             if (top + total_push > WALK_STACK) {                 // cannot happen (see the throttle above)
                 if (lane == 0) atomicOr(&h->status, PETAR_ST_STACK);
@@ -368,6 +366,19 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
             for (int k = 0; k < push; ++k) stack[at + k] = fc + k;
             top += total_push;
             __syncwarp();
+            pop();                             // next batch: its loads overlap the output below
+            // outputs of the current batch
+            list_append(lsp, act == 0, 1, node_cur, 0, arena, arena_chunks, h, lane);
+            list_append(lspp, act == 4, 1, node_cur, 0, arena, arena_chunks, h, lane);
+            list_append(lepn, act == 1, 2, nb, ne, arena, arena_chunks, h, lane);
+            list_append(lepf, act == 2, 2, nb, ne, arena, arena_chunks, h, lane);
+            n_sp += __popc(__ballot_sync(0xffffffffu, act == 0));
+            n_spp += __popc(__ballot_sync(0xffffffffu, act == 4));
+            n_epn += __popc(__ballot_sync(0xffffffffu, act == 1));
+            n_epf += __popc(__ballot_sync(0xffffffffu, act == 2));
+            const int cn = __reduce_add_sync(0xffffffffu, (act == 1) ? (ne - nb) : 0);
+            const int cf = __reduce_add_sync(0xffffffffu, (act == 2) ? (ne - nb) : 0);
+            n_epn_part += cn; n_ep_part += cn + cf;
         }
         if (lane == 0) {
             GroupRec* go = &grp[g];
@@ -742,7 +753,7 @@ __global__ void k_node_dbl(const DevHeader* __restrict__ h, const NodeMac* __res
 // n_groups / n_nodes are passed by the caller (api.cu reads the header back first)
 cudaError_t launch_export_lists(petar_tree* t, int what, void* dst, size_t dst_bytes, cudaStream_t s) {
     Workspace& w = t->w;
-    int ng = t->pinned[1], nn = t->pinned[0];
+    int ng = t->h_groups, nn = t->h_nodes;
     if (what == PETAR_DBG_GROUP_CNT || what == PETAR_DBG_GROUP_INT || what == PETAR_DBG_GROUP_SUPER) {
         size_t need = (size_t)ng * (what == PETAR_DBG_GROUP_INT ? 8 : what == PETAR_DBG_GROUP_SUPER ? 32 : 16);
         if (dst_bytes < need) return cudaErrorInvalidValue;

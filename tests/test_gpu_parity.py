@@ -176,6 +176,34 @@ def test_parameter_variants(mult, theta, n_leaf, n_group):
     t.close()
 
 
+def test_node_capacity_small_leaves_all_binaries():
+    """n_leaf_limit = 1 on an all-binary workload: rule O5 keeps single-child chains, so every tight binary adds a
+    node per level down to the level that separates its members and the default node table (3N + 4096) overflows.
+    The overflow is reported (PETAR_ST_NODE_CAP), the force kernels then write nothing, and nodes_per_particle
+    sizes a table that holds the tree: the result is then bit-exact / within tolerance as usual."""
+    P = _P()
+    w = make_workload(3, N=20000, seed=5)
+    w.n_leaf_limit, w.n_group_limit = 1, 8
+    T = _ora_tree(w, n_leaf=1, n_group=8)
+    assert T.n_nodes > 3 * w.N + 4096                      # the case the default cannot hold
+    t = _gpu_tree(w, list_entries_per_particle=4096.0)
+    assert P.petar_tree_status(t.handle) & 2               # PETAR_ST_NODE_CAP
+    t.acc_x.fill_(123.0)
+    with pytest.raises(P.PetarError):
+        t.force(want_counts=True)                          # PETAR_ESTATUS
+    assert float(t.acc_x.min()) == 123.0 and float(t.acc_x.max()) == 123.0      # untouched
+    t.close()
+    t = _gpu_tree(w, list_entries_per_particle=4096.0, nodes_per_particle=float(T.n_nodes) / w.N + 0.5)
+    check_structures(t, T, w)
+    counts = t.force(want_counts=True)
+    check_counts_and_lists(t, T, counts, sample=10)
+    g = [_np(v) for v in (t.acc_x, t.acc_y, t.acc_z, t.pot)]
+    ea, ep = _rel_err(g, T.force())
+    assert ea.max() < TOL and ep.max() < TOL
+    check_neighbors(t, T, w.N)
+    t.close()
+
+
 def test_search_radius_hook():
     """r_search (Eq. 24 hook): neighbours and the forced-open rule use it; forces still use r_out."""
     w = make_workload(2, N=8000, seed=3)
@@ -305,24 +333,36 @@ def test_rebuild_is_deterministic():
 # ---- BASELINE.json full sizes, in the launch configuration bench.py times -------------------------------
 @pytest.mark.parametrize("cfg", [3, 4])
 def test_full_size(cfg):
-    """N = 2^20 (configs 3 and 4): structures and counts bit-exact over the whole system, forces on sampled
-    i-groups the oracle can compute one by one, neighbour lists in full."""
+    """N = 2^20 (configs 3 and 4): structures, counts and neighbour lists bit-exact over the whole system (the per-group
+    counts pin every list's size; list MEMBERSHIP is compared as sets on sampled groups, the flattened lists of all
+    56 000 groups being ~1 GB).  Forces: config 3, the headline, on ALL i-groups (every particle; the criterion is a
+    max, and the particles where fp32 hurts most -- near-cancelling forces at the centre -- must not be missed by a
+    sample); config 4 on sampled groups plus the central mass's group."""
     w = make_workload(cfg)
     t, T = _gpu_tree(w), _ora_tree(w)
     check_structures(t, T, w)
     counts = t.force(want_counts=True)
     check_counts_and_lists(t, T, counts, sample=12)
-    rng = np.random.default_rng(cfg)
-    sel = rng.choice(T.n_groups, size=160, replace=False)
-    if cfg == 4:    # include the group of the central point mass (longest neighbour row)
+    if cfg == 3:
+        sel = None                                      # every group
+    else:
+        rng = np.random.default_rng(cfg)
+        sel = rng.choice(T.n_groups, size=160, replace=False)
+        # include the group of the central point mass (longest neighbour row)
         key, perm = T.keys()
         gb, ge, *_ = T.groups()
         pos0 = int(np.where(perm == 0)[0][0])
         sel = np.concatenate([sel, [int(np.searchsorted(ge, pos0, side="right"))]])
-    a = T.force(sel)
+    a = T.force(sel) if sel is not None else T.force()
     g = [_np(v) for v in (t.acc_x, t.acc_y, t.acc_z, t.pot)]
     ea, ep = _rel_err(g, a)
-    assert ea.size > 1000 and ea.max() < TOL and ep.max() < TOL, (ea.max(), ep.max())
+    idx_all = np.where(~np.isnan(a[0]))[0]
+    worst = int(idx_all[np.argmax(ea)])
+    print(f"config {cfg}: {ea.size} particles compared; acceleration error max {ea.max():.3e} (particle {worst}), "
+          f"99.9th percentile {np.quantile(ea, 0.999):.3e}, median {np.median(ea):.3e}; "
+          f"potential error max {ep.max():.3e}, 99.9th percentile {np.quantile(ep, 0.999):.3e}, median {np.median(ep):.3e}")
+    assert ea.size == (w.N if cfg == 3 else ea.size) and ea.size > 1000
+    assert ea.max() < TOL and ep.max() < TOL, (ea.max(), ep.max(), worst)
     off, idx = check_neighbors(t, T, w.N)
     if cfg == 4:
         assert np.diff(off)[0] > 500            # the central mass has r_out ~ 0.066 and a long row
@@ -375,22 +415,25 @@ def test_config5_capacity():
 
 def test_rms_error_vs_direct_sum_config4():
     """Reported separately (north_star): RMS relative force error against the DEFINITION (direct long-range sum
-    over all N sources) on a 4096-target subsample, theta sweep of config 4.  PARITY UNPINNED: the paper prints
-    no such number; only monotonicity and a loose ceiling are asserted."""
+    over all N sources) on the 4096-target subsample, theta sweep 0.2 / 0.3 / 0.5 / 0.7 of config 4 (the same targets
+    as bench.py --theta-sweep).  PARITY UNPINNED: the paper prints no such number; only monotonicity in theta and
+    loose ceilings are asserted."""
     w = make_workload(4)
     rng = np.random.default_rng(44)
-    tg = np.sort(rng.choice(w.N, size=1024, replace=False)).astype(np.int64)
+    tg = np.sort(rng.choice(w.N, size=4096, replace=False)).astype(np.int64)
     d = oracle.direct(w.x, w.y, w.z, w.m, w.r_out, oracle.OracleParams.from_workload(w), "long", targets=tg)
-    errs = []
-    for theta in (0.3, 0.7):
-        t = _gpu_tree(w, theta=theta)
-        t.force()
+    errs, inter = [], []
+    for theta in (0.2, 0.3, 0.5, 0.7):
+        t = _gpu_tree(w, theta=theta, list_entries_per_particle=2048.0 if theta < 0.3 else 0.0)
+        c = t.force(want_counts=True)
         g = [_np(v)[tg] for v in (t.acc_x, t.acc_y, t.acc_z, t.pot)]
         rel = np.sqrt(sum((g[k] - d[k]) ** 2 for k in range(3))) / np.sqrt(sum(d[k] ** 2 for k in range(3)))
         errs.append(float(np.sqrt(np.mean(rel ** 2))))
+        inter.append(c.n_epep + c.n_epsp)
         t.close()
-    print("RMS relative force error vs direct sum, theta 0.3 / 0.7:", errs)
-    assert errs[0] < errs[1] < 5e-3 and errs[0] < 5e-4
+    print("RMS relative force error vs direct sum, theta 0.2 / 0.3 / 0.5 / 0.7:", errs, "interactions:", inter)
+    assert errs[0] < errs[1] < errs[2] < errs[3] < 5e-3 and errs[1] < 5e-4 and errs[0] < 5e-5
+    assert inter[0] > inter[1] > inter[2] > inter[3]
 
 
 def test_scale_and_translation():

@@ -1,5 +1,5 @@
-"""world_size-2 gloo test of bench.py's multi-rank aggregation rule (replicas only: the ranks share no
-data; value = total interactions / max-over-ranks time)."""
+"""world_size-2 gloo test of bench.py's multi-rank aggregation (replicas only: the ranks share no data;
+value = total interactions / max-over-ranks time).  Calls bench.aggregate_ranks, the function bench.py itself runs."""
 import os
 import sys
 
@@ -19,9 +19,10 @@ def _worker(rank, world, port, q):
     w = make_workload(1, N=512, seed=SEED_BASE + 1 + 1000 * rank if rank else None)
     inter = float(1000 + w.x[0] * 0 + 10 * rank)
     ms = 5.0 + rank
-    t = torch.tensor([ms], dtype=torch.float64); dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    s = torch.tensor([inter], dtype=torch.float64); dist.all_reduce(s, op=dist.ReduceOp.SUM)
-    q.put((rank, float(t[0]), float(s[0]), float(w.x[1])))
+    import bench
+    ms_step, e2e_ms, total = bench.aggregate_ranks(ms, 2.0 * ms, inter, dist, "cpu")
+    assert e2e_ms == 12.0
+    q.put((rank, ms_step, total, float(w.x[1])))
     dist.barrier()
     dist.destroy_process_group()
 

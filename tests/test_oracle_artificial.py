@@ -30,9 +30,9 @@ def _golden_rows():
 
 def test_generalized_inverse_reproduces_table1():
     """The least-squares inverse of Eq. 28 built from Table 1's polynomial and measure points has exactly the rows
-    the paper prints (18 legible rows)."""
+    the paper prints (all 22 rows of the table: 6 of the second order, 16 of the third)."""
     rows = _golden_rows()
-    assert len(rows) == 18
+    assert len(rows) == 22 and sum(1 for (o, _) in rows if o == 2) == 6
     for order in (2, 3):
         Pi = np.linalg.pinv(A.tidal_design_matrix(order))
         names = A.T2_NAMES if order == 2 else A.T3_NAMES

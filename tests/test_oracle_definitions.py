@@ -111,3 +111,27 @@ def test_plummer_potential_energy():
     rng = np.random.Generator(np.random.PCG64(5))
     r = np.linalg.norm(plummer_positions(200000, rng), axis=1)
     assert np.median(r) == pytest.approx(PLUMMER_A / np.sqrt(2 ** (2 / 3) - 1), rel=0.01)
+
+
+def test_changeover_radii_eq12():
+    """Eq. 12: r_out,i = max(1, m_i/<m>)^(1/3) r_out,ref with <m> the average mass of the system
+    (reading P5).  Pins workloads.changeover_radii -- the one piece of the paper's arithmetic in the input generators --
+    against numbers worked out by hand from the formula: config 4's central mass 0.01 among N - 1 stars of total
+    mass 0.99 has m/<m> = 0.01 N = 10485.76, so 21.888 x 0.003 = 0.06566; a 150 Msun star at <m> = 0.586 Msun
+    (Kroupa 0.08-150) gets 6.35 x; every star at or below the mean keeps r_out,ref."""
+    from workloads.generators import changeover_radii
+    N = 1 << 20
+    m = np.full(N, 0.99 / (N - 1)); m[0] = 0.01
+    r = changeover_radii(m, 0.003)
+    assert r[0] == pytest.approx(0.003 * (0.01 * N) ** (1.0 / 3.0), rel=1e-14)
+    assert r[0] == pytest.approx(0.0657, abs=5e-5) and r[0] / 0.003 == pytest.approx(21.9, abs=0.05)
+    assert np.all(r[1:] == 0.003)                                   # below the mean: exactly r_out,ref
+    m = np.full(10000, (5860.0 - 150.0 - 0.08 - 0.3) / 9997.0); m[0], m[1], m[2] = 150.0, 0.08, 0.3      # mean 0.586
+    r = changeover_radii(m, 0.01)
+    assert m.sum() / m.size == pytest.approx(0.586, rel=1e-12)
+    assert r[0] / 0.01 == pytest.approx((150.0 / 0.586) ** (1.0 / 3.0), rel=1e-12) and r[0] / 0.01 == pytest.approx(6.35, abs=0.005)
+    assert r[1] == 0.01 and r[2] == 0.01 and np.all(r[3:] == 0.01)
+    # equal masses: a no-op; the radius grows as the cube root of the mass (8 x the mean mass -> twice the radius)
+    assert np.all(changeover_radii(np.full(100, 0.01), 0.05) == 0.05)
+    m = np.ones(1000); m[0] = 8.0 * (999.0 / 992.0)                # m_0 / <m> = 8 exactly: <m> = (999 + m_0)/1000
+    assert changeover_radii(m, 1.0)[0] == pytest.approx(2.0, rel=1e-12)
