@@ -335,6 +335,7 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
     __shared__ double s_fin[64][5];
     __shared__ int s_g;
     __shared__ int s_scan[FT / 32];
+    __shared__ int s_off[FT + 1], s_jb[FT];
     const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
     const int ng = h->n_groups;
     if (h->status != 0) return;            // capacity exceeded / non-finite input: lists are unusable, write nothing (petar.h)
@@ -395,12 +396,19 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
                         int woff = 0, total = 0;
 #pragma unroll
                         for (int ww = 0; ww < FT / 32; ++ww) { int vv = s_scan[ww]; if (ww < wrp) woff += vv; total += vv; }
-                        const int my0 = woff + incl - cnt;     // exclusive offset of my range
+                        s_off[t] = woff + incl - cnt;          // exclusive offset of my range
+                        s_jb[t] = jb;
+                        if (t == 0) s_off[FT] = total;
+                        __syncthreads();
                         for (int w0 = 0; w0 < total; w0 += EP_TILE) {
                             if (w0) __syncthreads();
-                            const int lo = max(my0, w0), hi = min(my0 + cnt, w0 + EP_TILE);
-                            for (int q = lo; q < hi; ++q) {
-                                const int j = jb + (q - my0);
+                            // staging is shared out by OUTPUT slot (ranges differ in length: 1 .. 64 particles once contiguous leaves
+                            // are joined): slot q belongs to the last range whose offset is <= q
+                            for (int q = w0 + t; q < min(total, w0 + EP_TILE); q += FT) {
+                                int r = 0;
+#pragma unroll
+                                for (int step = FT / 2; step > 0; step >>= 1) if (s_off[r + step] <= q) r += step;
+                                const int j = s_jb[r] + (q - s_off[r]);
                                 sm.ep.a[q - w0] = pa[j]; sm.ep.b[q - w0] = pb[j];
                                 if (pass == 0) sm.ep.j[q - w0] = j;
                             }
