@@ -101,8 +101,8 @@ static size_t carve(Workspace* w, char* base, int64_t N, const petar_params* p) 
     W->smap = (int*)take((size_t)PETAR_NSUP * n * 4);
     W->unit_cap = (int)(PETAR_NSUP * (N + 64));             // every unit holds at least one particle
     W->units = (ForceUnit*)take((size_t)W->unit_cap * sizeof(ForceUnit));
-    W->part = (double*)take((size_t)PETAR_NSUP * n * 4 * 8);
-    W->part_s = (double*)take((size_t)PETAR_NSUP * n * 8);
+    W->part = (double*)take((size_t)(PETAR_NSUP + 1) * n * 4 * 8);
+    W->part_s = (double*)take((size_t)(PETAR_NSUP + 1) * n * 8);
     W->refine_q = (int*)take(n * 2 * 4);
     W->nb_cnt = (int*)take(n * 4);
     W->nb_queue = (int*)take(((size_t)W->group_cap + 1) * 4);

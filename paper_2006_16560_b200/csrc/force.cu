@@ -216,7 +216,7 @@ struct TileCursorT {
         if (n1 > 0) { head_b = head2; n_b = n2; start(arena, head1, n1); }
         else { head_b = -1; n_b = 0; start(arena, head2, n2); }
     }
-    __device__ __forceinline__ int count() const { return (chunk >= 0 && remaining > 0) ? min(TILE, min(remaining, PETAR_CHUNK_PAYLOAD - off)) : 0; }
+    __device__ __forceinline__ int count(const int tile) const { return (chunk >= 0 && remaining > 0) ? min(tile, min(remaining, PETAR_CHUNK_PAYLOAD - off)) : 0; }
     __device__ __forceinline__ void advance(const int* arena, int n) {
         remaining -= n; off += n;
         if (remaining > 0 && off >= PETAR_CHUNK_PAYLOAD) {
@@ -253,13 +253,14 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
     }
     Acc2 p = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
     TileCursor cur; cur.init(arena, head, n, head2, n2);
+    const int tile_s = (SP_TILE / S) * S;       // cells per staged tile: a multiple of the slice count, so every slice sees the same number
     int tn0 = 0, tn1 = 0, tn2 = 0;
     int id2[SP_REC];
     float4 q0[SP_REC], q1[SP_REC], q2[SP_REC];
 #pragma unroll
     for (int r = 0; r < SP_REC; ++r) id2[r] = 0;
     auto load_ids = [&]() {
-        tn2 = cur.count();
+        tn2 = cur.count(tile_s);
 #pragma unroll
         for (int r = 0; r < SP_REC; ++r) if (t + r * FT < tn2) id2[r] = cur.cp[PETAR_CHUNK_HDR + cur.off + t + r * FT];
         cur.advance(arena, tn2);
@@ -324,6 +325,78 @@ __device__ __forceinline__ void sp_phase(ForceSmem& sm, const int* __restrict__ 
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Changeover pairs (k_force_near): the particles of a group's NEAR leaf ranges (within r_out of the group; ~30 per group,
+// 0.5 % of all interactions) against the group's particles, with the weights 1-K (Eq. 17) and 1-W (Eq. 15).  One warp
+// per group, lanes own i-particles, the ranges are flattened by a warp scan and staged 32 particles at a time; no CTA
+// barrier.  (Inside k_force the same work cost four block barriers and two dependent global loads per group, 0.5 ms
+// per step.)  Sums go to part[PETAR_NSUP] / part_s[PETAR_NSUP] (sorted order), k_force adds them.
+// ------------------------------------------------------------------------------------------------
+#define NEAR_WARPS 8
+struct NearTile { float4 a[32], b[32]; int j[32]; };
+__global__ void __launch_bounds__(NEAR_WARPS * 32) k_force_near(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
+                                                                const float4* __restrict__ pa, const float4* __restrict__ pb,
+                                                                double* __restrict__ part_near, double* __restrict__ part_s_near, ForceConst fc) {
+    __shared__ NearTile s_tile[NEAR_WARPS];
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    NearTile& tl = s_tile[wp];
+    const int ng = h->n_groups;
+    if (h->status != 0) return;
+    for (;;) {
+        int g = 0;
+        if (lane == 0) g = atomicAdd(&h->group_ticket4, 1);
+        g = __shfl_sync(0xffffffffu, g, 0);
+        if (g >= ng) break;
+        const GroupRec* gr = &grp[g];
+        const int gb = gr->begin, ge = gr->end;
+        for (int ib = gb; ib < ge; ib += 32) {          // blocks of 32 i-particles (groups hold <= 64)
+            const int i = ib + lane;
+            const bool vi = i < ge;
+            const float4 ia = pa[vi ? i : gb], ib4 = pb[vi ? i : gb];
+            const IFF i1 = {-ia.x, -ia.y, -ia.z, -ib4.x, -ib4.y, -ib4.z, ib4.w};
+            double ax = 0.0, ay = 0.0, az = 0.0, pot = 0.0, sc = 0.0;
+            int chunk = gr->head_epn;
+            int remaining = gr->n_epn * 2;
+            while (chunk >= 0 && remaining > 0) {
+                const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
+                const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+                for (int e0 = 0; e0 < ne; e0 += 64) {
+                    int jb_l = 0, cnt_l = 0;
+                    if (e0 + 2 * lane < ne) { const int2 be = *reinterpret_cast<const int2*>(cp + PETAR_CHUNK_HDR + e0 + 2 * lane); jb_l = be.x; cnt_l = be.y - be.x; }
+                    int incl = cnt_l;
+#pragma unroll
+                    for (int o2 = 1; o2 < 32; o2 <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o2); if (lane >= o2) incl += v; }
+                    const int total = __shfl_sync(0xffffffffu, incl, 31);
+                    const int excl = incl - cnt_l;
+                    for (int p0 = 0; p0 < total; p0 += 32) {
+                        const int p = p0 + lane;
+                        int lo = 0;                               // smallest range whose inclusive count exceeds p
+#pragma unroll
+                        for (int step = 16; step > 0; step >>= 1) { const int v = __shfl_sync(0xffffffffu, incl, lo + step - 1); if (v <= p) lo += step; }
+                        lo = min(lo, 31);
+                        const int rjb = __shfl_sync(0xffffffffu, jb_l, lo), rex = __shfl_sync(0xffffffffu, excl, lo);
+                        __syncwarp();
+                        if (p < total) { const int j = rjb + (p - rex); tl.a[lane] = pa[j]; tl.b[lane] = pb[j]; tl.j[lane] = j; }
+                        __syncwarp();
+                        const int nb = min(32, total - p0);
+                        Acc32 q = {0.f, 0.f, 0.f, 0.f};
+                        for (int k = 0; k < nb; ++k) ep_near_one(q, i1, tl.a[k], tl.b[k], fc, tl.j[k] == i);
+                        ax += (double)q.ax; ay += (double)q.ay; az += (double)q.az; pot += (double)q.pot;
+                        sc += (double)(fabsf(q.ax) + fabsf(q.ay) + fabsf(q.az));
+                    }
+                }
+                remaining -= ne;
+                chunk = cp[0];
+            }
+            if (vi) {
+                double* o = part_near + (size_t)i * 4;
+                o[0] = ax; o[1] = ay; o[2] = az; o[3] = pot;
+                part_s_near[i] = sc;
+            }
+        }
+    }
+}
+
 template <bool QUAD>
 __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restrict__ h, const GroupRec* __restrict__ grp, const int* __restrict__ arena,
                                                  const NodeSp* __restrict__ nsp, const float4* __restrict__ pa, const float4* __restrict__ pb,
@@ -376,8 +449,9 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
                              make_float2(i0.nxl, i1.nxl), make_float2(i0.nyl, i1.nyl), make_float2(i0.nzl, i1.nzl)};
             Acc32 p0 = {0.f, 0.f, 0.f, 0.f}, p1 = {0.f, 0.f, 0.f, 0.f};
             Acc2 pf = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+            // (the near ranges -- changeover pairs -- were summed by k_force_near into part[PETAR_NSUP])
 #pragma unroll 1
-            for (int pass = 0; pass < 2; ++pass) {
+            for (int pass = 1; pass < 2; ++pass) {
                 int chunk = pass == 0 ? gr->head_epn : gr->head_epf;
                 int remaining = 2 * (pass == 0 ? gr->n_epn : gr->n_epf);
                 while (chunk >= 0 && remaining > 0) {
@@ -451,7 +525,7 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
             const int i = k / 5, comp = k - 5 * i;
             double q = 0.0;
 #pragma unroll
-            for (int l = 0; l < PETAR_NSUP; ++l)
+            for (int l = 0; l <= PETAR_NSUP; ++l)
                 q += comp < 4 ? part[((size_t)l * n_part + gb + i) * 4 + comp] : part_s[(size_t)l * n_part + gb + i];
             for (int sl = 0; sl < S; ++sl) q += sm.red[(size_t)(sl * (2 * P) + i) * 5 + comp];
             s_fin[i][comp] = q;
@@ -529,8 +603,9 @@ __device__ __forceinline__ void refine_pair(Acc4d& a, const bool near, const dou
     const double f = m * wk * rinv * rinv * rinv;
     a.ax += f * dx; a.ay += f * dy; a.az += f * dz; a.pot += m * pw;
 }
-__global__ void __launch_bounds__(256) k_force_refine(const DevHeader* __restrict__ h, const RefineArgs A) {
-    __shared__ double s_red[8][4];
+#define REFINE_THREADS 1024   // one CTA per particle: the lists (~10^4 entries) are walked by all its threads
+__global__ void __launch_bounds__(REFINE_THREADS) k_force_refine(const DevHeader* __restrict__ h, const RefineArgs A) {
+    __shared__ double s_red[REFINE_THREADS / 32][4];
     const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
     const int nq = h->n_refine;
     if (h->status != 0) return;
@@ -548,7 +623,7 @@ __global__ void __launch_bounds__(256) k_force_refine(const DevHeader* __restric
                 while (chunk >= 0 && remaining > 0) {
                     const int* cp = A.arena + (size_t)chunk * PETAR_CHUNK;
                     const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
-                    for (int e = t; e < ne; e += 256) {
+                    for (int e = t; e < ne; e += REFINE_THREADS) {
                         const int id = cp[PETAR_CHUNK_HDR + e];
                         refine_cell(a, A.nmac[id], A.nmom[id], A.quad != 0, xi, yi, zi);
                     }
@@ -563,7 +638,7 @@ __global__ void __launch_bounds__(256) k_force_refine(const DevHeader* __restric
             while (chunk >= 0 && remaining > 0) {
                 const int* cp = A.arena + (size_t)chunk * PETAR_CHUNK;
                 const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
-                for (int e = 2 * t; e < ne; e += 512) {
+                for (int e = 2 * t; e < ne; e += 2 * REFINE_THREADS) {
                     const int jb = cp[PETAR_CHUNK_HDR + e], je = cp[PETAR_CHUNK_HDR + e + 1];
                     for (int j = jb; j < je; ++j) {
                         if (j == pos) continue;                 // the list holds the particle itself
@@ -583,7 +658,7 @@ __global__ void __launch_bounds__(256) k_force_refine(const DevHeader* __restric
         __syncthreads();
         if (t == 0) {
             double v[4] = {0.0, 0.0, 0.0, 0.0};
-            for (int ww = 0; ww < 8; ++ww) for (int c = 0; c < 4; ++c) v[c] += s_red[ww][c];
+            for (int ww = 0; ww < REFINE_THREADS / 32; ++ww) for (int c = 0; c < 4; ++c) v[c] += s_red[ww][c];
             const unsigned o = A.perm[pos];
             if (A.oax) A.oax[o] = A.G * v[0];
             if (A.oay) A.oay[o] = A.G * v[1];
@@ -892,7 +967,7 @@ __global__ void __launch_bounds__(256) k_units_fill(DevHeader* __restrict__ h, c
 }
 
 __global__ void k_reset_ticket2(DevHeader* h) {
-    if (threadIdx.x == 0) { h->group_ticket2 = 0; h->unit_ticket = 0; h->n_refine = 0; for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) h->unit_cnt[k] = 0; }
+    if (threadIdx.x == 0) { h->group_ticket2 = 0; h->group_ticket4 = 0; h->unit_ticket = 0; h->n_refine = 0; for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) h->unit_cnt[k] = 0; }
 }
 
 // phase A: unit table, then the super-groups' common cells.  ctas_per_sm > 0 limits the grid (tuning
@@ -941,6 +1016,9 @@ cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* a
     fc.a4 = (float)(35.0 * lam);
     const bool quad = t->p.multipole >= 2;
     stage_begin(t, s);
+    k_force_near<<<t->sm_count * 8, NEAR_WARPS * 32, 0, s>>>(w.hdr, w.grp, w.arena, w.pa, w.pb, w.part + (size_t)PETAR_NSUP * t->N * 4,
+                                                               w.part_s + (size_t)PETAR_NSUP * t->N, fc);
+    KCHECK(s, "k_force_near");
     int per_sm = 0;
     cudaError_t e;
     if (quad) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<true>, FT, 0);
@@ -957,10 +1035,10 @@ cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* a
         const double* rs = w.routs;
         RefineArgs A = {w.grp, w.srec, w.group_cap, w.arena, w.nmac, w.nmom, w.xs, w.ys, w.zs, w.ms, rs, w.idx, w.refine_q,
                         ax, ay, az, pot, t->p.G, t->p.r_in_over_r_out, quad ? 1 : 0};
-        k_force_refine<<<t->sm_count * 8, 256, 0, s>>>(w.hdr, A);
+        k_force_refine<<<t->sm_count, REFINE_THREADS, 0, s>>>(w.hdr, A);
         KCHECK(s, "k_force_refine");
     }
-    petar_count_launch(2);
+    petar_count_launch(3);
     stage_end(t, PETAR_STAGE_FORCE, s);
     return cudaGetLastError();
 }

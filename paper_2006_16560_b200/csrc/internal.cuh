@@ -49,7 +49,7 @@ struct DevHeader {
     int unit_fill[PETAR_UNIT_CLASSES];
     int unit_ticket;
     int n_refine;                  // particles queued for the fp64 re-evaluation (k_force_refine)
-    int pad_[1];
+    int group_ticket4;             // k_force_near
     unsigned long long n_epep, n_epsp, n_epep_near, n_ep_list, n_sp_list, n_epsp_common;
     unsigned long long nb_total;
 };
@@ -120,8 +120,8 @@ struct Workspace {
     SuperRec* srec;                // [PETAR_NSUP][group_cap] super-groups
     int* smap;                     // [PETAR_NSUP][N] sorted position -> super-group id
     struct ForceUnit* units; int unit_cap;   // phase-A force units (force.cu)
-    double* part;                  // [PETAR_NSUP][N][4] phase-A partial sums (sorted order): ax, ay, az, pot
-    double* part_s;                // [PETAR_NSUP][N] phase-A cancellation scale (Acc64::s)
+    double* part;                  // [PETAR_NSUP + 1][N][4] partial sums (sorted order) ax, ay, az, pot: phase A per super-group level, then the changeover pairs
+    double* part_s;                // [PETAR_NSUP + 1][N] cancellation scale (Acc64::s) of the same
     int* refine_q;                 // [N][2] (group, sorted position) of the particles to re-evaluate in fp64
     // list arena
     int* arena; int arena_chunks;
