@@ -22,15 +22,12 @@ void petar_debug_check(cudaStream_t s, const char* name) {
 // Stage timing: events are only RECORDED here (asynchronously, on the caller's stream);
 // petar_stage_times synchronises on them later.  No effect unless petar_set_profiling(1)
 // was called before petar_tree_build.
-void stage_begin(petar_tree* t, cudaStream_t s) {
+void stage_begin(petar_tree* t, int stage, cudaStream_t s) {
     if (!t->ev) return;
-    cudaEventRecord(t->ev[2 * PETAR_N_STAGES], s);      // scratch slot
+    cudaEventRecord(t->ev[2 * stage], s);
 }
 void stage_end(petar_tree* t, int stage, cudaStream_t s) {
     if (!t->ev) return;
-    cudaEvent_t b = t->ev[2 * PETAR_N_STAGES];          // swap the begin event into the stage's slot
-    t->ev[2 * PETAR_N_STAGES] = t->ev[2 * stage];
-    t->ev[2 * stage] = b;
     cudaEventRecord(t->ev[2 * stage + 1], s);
     t->stage_rec[stage] = 1;
 }
@@ -119,7 +116,10 @@ extern "C" size_t petar_workspace_bytes(int64_t N, const petar_params* p) {
 }
 
 static void free_handle(petar_tree* t) {
-    if (t->ev) { for (int k = 0; k < 2 * PETAR_N_STAGES + 1; ++k) if (t->ev[k]) cudaEventDestroy(t->ev[k]); delete[] t->ev; }
+    if (t->ev) { for (int k = 0; k < 2 * PETAR_N_STAGES; ++k) if (t->ev[k]) cudaEventDestroy(t->ev[k]); delete[] t->ev; }
+    if (t->ev_fork) cudaEventDestroy(t->ev_fork);
+    if (t->ev_join) cudaEventDestroy(t->ev_join);
+    if (t->side) cudaStreamDestroy(t->side);
     t->magic = 0;
     delete t;
 }
@@ -131,10 +131,15 @@ static int build_into(petar_tree* t, const double* x, const double* y, const dou
     t->built = false; t->walked = false;
     for (int k = 0; k < PETAR_N_STAGES; ++k) t->stage_rec[k] = 0;
     if (g_profiling && !t->ev) {            // events are created once per handle, never on a rebuild
-        t->ev = new (std::nothrow) cudaEvent_t[2 * PETAR_N_STAGES + 1];
+        t->ev = new (std::nothrow) cudaEvent_t[2 * PETAR_N_STAGES];
         if (!t->ev) return PETAR_EINVAL;
-        for (int k = 0; k < 2 * PETAR_N_STAGES + 1; ++k) t->ev[k] = nullptr;
-        for (int k = 0; k < 2 * PETAR_N_STAGES + 1; ++k) CK(cudaEventCreate(&t->ev[k]));
+        for (int k = 0; k < 2 * PETAR_N_STAGES; ++k) t->ev[k] = nullptr;
+        for (int k = 0; k < 2 * PETAR_N_STAGES; ++k) CK(cudaEventCreate(&t->ev[k]));
+    }
+    if (!t->side) {                         // once per handle
+        CK(cudaStreamCreateWithFlags(&t->side, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&t->ev_fork, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&t->ev_join, cudaEventDisableTiming));
     }
     if (t->N > 0) {
         CK(launch_keys_sort_gather(t, s));
@@ -176,6 +181,12 @@ extern "C" int petar_tree_rebuild(petar_tree* t, const double* x, const double* 
     return build_into(t, x, y, z, m, r_out, r_search, (cudaStream_t)cuda_stream);
 }
 
+#ifndef OVERLAP_WALK_CTAS
+#define OVERLAP_WALK_CTAS 1      // CTAs per SM of k_walk / k_force_units while the two run side by side
+#endif
+#ifndef OVERLAP_UNITS_CTAS
+#define OVERLAP_UNITS_CTAS 0      // 0 = no limit: the walk CTA is resident first, two unit CTAs fit beside it, the third follows when it leaves
+#endif
 static int check_tree(petar_tree* t) { return (t && t->magic == PETAR_MAGIC && t->built) ? PETAR_OK : PETAR_ENOTBUILT; }
 
 static int ensure_walk(petar_tree* t, cudaStream_t s) {
@@ -198,9 +209,21 @@ extern "C" int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_
     if (rc) return rc;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (t->N == 0) { if (counts) memset(counts, 0, sizeof(*counts)); return PETAR_OK; }
-    rc = ensure_walk(t, s);
-    if (rc) return rc;
-    CK(launch_force(t, acc_x, acc_y, acc_z, pot, s));
+    if (!t->walked) {
+        // Force phase A needs the super-group walks only.  The per-group walk (latency- and integer-bound) runs beside it on
+        // the handle's second stream: phase A is bound by the FMA pipe and leaves half of the issue slots free.
+        CK(launch_walk_supers(t, s));
+        CK(cudaEventRecord(t->ev_fork, s));
+        CK(cudaStreamWaitEvent(t->side, t->ev_fork, 0));
+        CK(launch_walk_groups(t, t->side, OVERLAP_WALK_CTAS));
+        CK(cudaEventRecord(t->ev_join, t->side));
+        CK(launch_force_units(t, s, OVERLAP_UNITS_CTAS));
+        CK(cudaStreamWaitEvent(s, t->ev_join, 0));
+        t->walked = true;
+        CK(launch_force_groups(t, acc_x, acc_y, acc_z, pot, s));
+    } else {
+        CK(launch_force(t, acc_x, acc_y, acc_z, pot, s));
+    }
     if (counts) {
         DevHeader hh;
         rc = read_header(t, s, &hh);

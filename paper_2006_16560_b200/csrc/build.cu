@@ -744,7 +744,7 @@ cudaError_t launch_search_radii(const double* vx, const double* vy, const double
 cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s) {
     Workspace& w = t->w;
     const long long n = t->N;
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_BBOX_KEYS, s);
     k_reset_header<<<1, 32, 0, s>>>(w.hdr);
     KCHECK(s, "k_reset_header");
     int g = min(cdiv(n, 256), t->sm_count * 8);
@@ -757,7 +757,7 @@ cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s) {
     petar_count_launch(4);
     stage_end(t, PETAR_STAGE_BBOX_KEYS, s);
 
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_SORT, s);
     {
         cudaError_t e = launch_radix_sort(w.key, w.key_alt, w.idx, w.idx_alt, w.sort_hist, w.sort_blk, n, 8, s);
         if (e != cudaSuccess) return e;
@@ -765,7 +765,7 @@ cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s) {
     // 8 passes: the sorted data is back in (key, idx)
     stage_end(t, PETAR_STAGE_SORT, s);
 
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_GATHER, s);
     k_gather<<<cdiv(n, 256), 256, 0, s>>>(w.idx, n, w.hdr, t->x, t->y, t->z, t->m, t->r_out, t->r_search,
                                           w.xs, w.ys, w.zs, w.ms, w.routs, t->r_search ? w.rss : nullptr, w.pa, w.pb);
     KCHECK(s, "k_gather");
@@ -778,7 +778,7 @@ cudaError_t launch_tree(petar_tree* t, cudaStream_t s) {
     Workspace& w = t->w;
     const long long n = t->N;
     const int ntile = cdiv(n, RANK_THREADS);
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_TREE, s);
     k_diverge<<<cdiv(n + 1, 256), 256, 0, s>>>(w.key, n, w.D);
     KCHECK(s, "k_diverge");
     size_t sh = DEPTH_THREADS + 2 * t->p.n_group_limit + 1;
@@ -793,7 +793,7 @@ cudaError_t launch_tree(petar_tree* t, cudaStream_t s) {
     petar_count_launch(5);
     stage_end(t, PETAR_STAGE_TREE, s);
 
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_MOMENTS, s);
     {
         int per_sm = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moments, 256, 0);
@@ -813,7 +813,7 @@ cudaError_t launch_tree(petar_tree* t, cudaStream_t s) {
     }
     stage_end(t, PETAR_STAGE_MOMENTS, s);
 
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_GROUPS, s);
     cudaError_t e = launch_scan_i32(w.gflag, w.gflag + (n + 1), (int)n, w.scan_tmp, s);
     if (e != cudaSuccess) return e;
     k_groups_begin<<<cdiv(n, 256), 256, 0, s>>>(w.gflag, w.gflag + (n + 1), n, w.grp, w.hdr);

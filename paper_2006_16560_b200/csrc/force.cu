@@ -974,7 +974,7 @@ __global__ void k_reset_ticket2(DevHeader* h) {
 // experiments).  Needs the super-group walks only.
 cudaError_t launch_force_units(petar_tree* t, cudaStream_t s, int ctas_per_sm) {
     Workspace& w = t->w;
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_FORCE_UNITS, s);
     k_reset_ticket2<<<1, 32, 0, s>>>(w.hdr);
     KCHECK(s, "k_reset_ticket2");
     const bool quad = t->p.multipole >= 2;
@@ -1015,7 +1015,7 @@ cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* a
     fc.b4 = (float)(-35.0 * lam);
     fc.a4 = (float)(35.0 * lam);
     const bool quad = t->p.multipole >= 2;
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_FORCE, s);
     k_force_near<<<t->sm_count * 8, NEAR_WARPS * 32, 0, s>>>(w.hdr, w.grp, w.arena, w.pa, w.pb, w.part + (size_t)PETAR_NSUP * t->N * 4,
                                                                w.part_s + (size_t)PETAR_NSUP * t->N, fc);
     KCHECK(s, "k_force_near");

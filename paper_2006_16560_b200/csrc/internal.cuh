@@ -138,10 +138,12 @@ struct petar_tree {
     Workspace w;
     const double *x, *y, *z, *m, *r_out, *r_search;
     bool built, walked;
-    cudaEvent_t* ev;               // [2*PETAR_N_STAGES + 1] stage begin/end events (profiling only; created once per handle)
+    cudaEvent_t* ev;               // [2*PETAR_N_STAGES] stage begin/end events (profiling only; created once per handle)
     int stage_rec[PETAR_N_STAGES];
     int sm_count;
     int h_nodes, h_groups;         // host copies of the header counters (filled by petar_debug_export)
+    cudaStream_t side;             // second stream: the per-group walk runs beside force phase A (created once per handle)
+    cudaEvent_t ev_fork, ev_join;
     void* workspace; size_t workspace_bytes;
 };
 
@@ -178,7 +180,7 @@ void petar_count_launch(int n);
 // PETAR_DEBUG_SYNC=1 in the environment: synchronise after every kernel and report the first failing one
 void petar_debug_check(cudaStream_t s, const char* name);
 #define KCHECK(s, name) petar_debug_check(s, name)
-void stage_begin(petar_tree* t, cudaStream_t s);
+void stage_begin(petar_tree* t, int stage, cudaStream_t s);
 void stage_end(petar_tree* t, int stage, cudaStream_t s);
 
 static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }

@@ -422,7 +422,7 @@ __global__ void k_reset_ticket(DevHeader* h, int which) {
 // the super-group levels (everything the force phase A needs)
 cudaError_t launch_walk_supers(petar_tree* t, cudaStream_t s) {
     Workspace& w = t->w;
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_WALK_SUPER, s);
     k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 0);
     KCHECK(s, "k_reset_ticket");
     int per_sm = 0;
@@ -448,7 +448,7 @@ cudaError_t launch_walk_supers(petar_tree* t, cudaStream_t s) {
 // the per-group walks; ctas_per_sm > 0 limits the grid (tuning experiments)
 cudaError_t launch_walk_groups(petar_tree* t, cudaStream_t s, int ctas_per_sm) {
     Workspace& w = t->w;
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_WALK, s);
     int per_sm = 0;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_walk, WALK_WARPS * 32, 0);
     if (e != cudaSuccess) return e;
@@ -660,7 +660,7 @@ cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, 
     const double* rss = t->r_search ? w.rss : w.routs;
     const bool orbit = vx != nullptr;
     NbArgs A = {w.arena, w.idx, w.xs, w.ys, w.zs, rss, w.nb_cnt, nullptr, nullptr, 0, {w.vxs, w.vys, w.vzs, w.ms, w.routs, t->p.G, Cv}};
-    stage_begin(t, s);
+    stage_begin(t, PETAR_STAGE_NEIGHBOR, s);
     const int grid = t->sm_count * 8, grid_big = t->sm_count;
     if (orbit) {
         k_gather_vel<<<cdiv(n, 256), 256, 0, s>>>(w.idx, n, vx, vy, vz, w.vxs, w.vys, w.vzs);
