@@ -419,14 +419,17 @@ def main():
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(stream); fl = P.petar_probe_fp32(400000, scratch, stream); b.record(stream); b.synchronize()
     probe_tflops = fl / (a.elapsed_time(b) * 1e-3) / 1e12
-    # the same with three distinct register operands per FFMA, and the kernel's own cell term on register operands
+    # the other instruction streams of petar_probe_fp32_mode (include/petar.h): the scalar and the packed cell term on register
+    # operands, and the FFMA operand patterns of the register-bank issue model (profiles/fp32_issue_model_r02.md)
     probes = {}
-    for mode, name, iters in ((1, "ffma_3_distinct_registers", 400000), (2, "quadrupole_cell_term_loop", 2000)):
+    for mode, name, iters in ((1, "ffma_3_distinct_registers", 400000), (2, "quadrupole_cell_term_loop_scalar", 2000),
+                              (3, "quadrupole_cell_term_loop_packed", 2000), (4, "pattern_ffma_3_registers_independent", 200000),
+                              (5, "pattern_ffma_2_registers", 200000), (6, "pattern_ffma_shared_operand", 200000),
+                              (7, "pattern_ffma3_plus_fadd", 200000)):
         P.petar_probe_fp32_mode(mode, max(1, iters // 50), scratch, stream)
         torch.cuda.synchronize()
         a.record(stream); fl = P.petar_probe_fp32_mode(mode, iters, scratch, stream); b.record(stream); b.synchronize()
         probes[name] = fl / (a.elapsed_time(b) * 1e-3) / 1e12
-
     pk, pk_kind = peaks()
     sm_max = float(pk.get("sm_max_mhz", 1965.0))
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
@@ -476,6 +479,8 @@ def main():
                     "n_epep_changeover": int(counts.n_epep_near), "neighbours": nb_total, "n_groups": int(counts.n_groups),
                     "n_nodes": int(counts.n_nodes), "status": status, "multi_gpu": "replicas only (no data-path collective)"},
             stage_ms=stage_ms,
+            stage_note="the per-group walk (stage walk) runs on the library's side stream BESIDE force phase A (stage force_units): the two "
+                       "stage times overlap and each is longer than when run alone",
             hbm_stages=dict(peak_gbs=hbm_peak, note="keys / sort / tree stages: algorithmic bytes over stage time; at N = 2^20 the working "
                             "set (12-116 MB) sits in the 126 MB L2 and the stages are launch- and latency-bound, the fraction of HBM "
                             "bandwidth only means something at --config 5 (N = 10^7)", stages=hbm_stages),
@@ -490,7 +495,9 @@ def main():
                           peak_kind=f"nominal CUDA-core FP32: 2 x 128 lanes x {n_sm} SMs x {sm_max:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {pk_kind})",
                           peak_measured_ffma_probe=probe_tflops, frac_of_probe=dom["achieved"] / probe_tflops,
                           probes_tflops=probes,
-                          frac_of_cell_term_probe=dom["achieved"] / probes["quadrupole_cell_term_loop"],
+                          probes_note="cell-term probes: TFLOP/s at 53 flops per interaction; pattern probes: 2 x thread instructions per "
+                                      "second, i.e. value / peak = warp instructions per clock and sub-partition",
+                          frac_of_cell_term_probe=dom["achieved"] / probes["quadrupole_cell_term_loop_packed"],
                           flops_convention=f"{FLOP_NEWTON}/{FLOP_CUT}/{FLOP_QUAD} flops per Newtonian / changeover / quadrupole interaction",
                           flops_per_launch=dom["flops_per_launch"], kernel_ms=dom["ms"], kernel_share_of_step=dom["share_of_step"],
                           force_kernels=kern, both_force_kernels=dict(ms=force_ms, achieved=achieved_both, frac=achieved_both / nominal_fp32,

@@ -305,10 +305,15 @@ int petar_probe_fp32(int64_t iters, double* flops_out_host, float* scratch_dev, 
 /* The same with a choice of instruction stream ("operand bandwidth"):
  *   mode 0: FFMA whose two other operands are the same for every chain (as petar_probe_fp32);
  *   mode 1: FFMA with three distinct register operands per instruction;
- *   mode 2: the force kernel's own quadrupole cell term (rule O8) on register operands, 4 i-particles
+ *   mode 2: the quadrupole cell term (rule O8) with SCALAR fp32 instructions on register operands, 4 i-particles
  *           per thread, cells broadcast from shared memory -- *flops_out_host then counts 53 flops per
- *           interaction (the convention of bench.py), so the result is the rate attainable by this
- *           instruction mix with no list, staging or tail cost.
+ *           interaction (the convention of bench.py): the rate of the round-1 instruction mix;
+ *   mode 3: the same term with the PACKED fp32x2 instructions the force kernels use (two packed pairs per thread):
+ *           the rate attainable by the kernels' instruction mix with no list, staging or tail cost;
+ *   modes 4-7: FFMA operand patterns behind profiles/fp32_issue_model_r02.md -- 4: a = b*c + a (three distinct
+ *           registers), 5: a = b*b + a (two), 6: a = b*e + a; c = d*e + c (one operand shared by all), 7: a = b*c + d;
+ *           d = a + e.  *flops_out_host = 2 x thread-level instructions, so value / time / (nominal FP32 peak) is
+ *           warp instructions per clock and sub-partition.
  * Errors: PETAR_EINVAL (mode), PETAR_ECUDA.                                                          */
 int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream);
 

@@ -13,7 +13,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.environ.get("PETAR_B200_LIB_OUT", os.path.join(HERE, "libpetar_b200.so"))
+LIB = os.path.join(HERE, "libpetar_b200.so")
 SOURCES = [("build.cu", ["-fmad=false"]), ("walk.cu", ["-fmad=false"]), ("force.cu", []), ("cluster.cu", []), ("short.cu", []), ("artificial.cu", []), ("api.cu", [])]
 COMMON = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
@@ -36,8 +36,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     procs = []
     for src, extra in SOURCES:
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
-        more = os.environ.get("PETAR_NVCC_EXTRA", "").split()          # tuning experiments (-DSP_REC=1 ...)
-        cmd = [nvcc] + COMMON + extra + more + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc] + COMMON + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)
     for cmd, p in procs:

@@ -27,19 +27,11 @@
 // fp32 partial sums live only across one tile slice and are flushed into fp64 accumulators.
 #include "internal.cuh"
 
-#ifndef FT
 #define FT 128                 // threads per CTA
-#endif
-#ifndef SP_REC
 #define SP_REC 2               // staged cells per thread per tile
-#endif
 #define SP_TILE (SP_REC * FT)  // cells per staged tile
-#ifndef FORCE_MIN_CTAS
 #define FORCE_MIN_CTAS 4
-#endif
-#ifndef FORCE_UNROLL
 #define FORCE_UNROLL 2
-#endif
 #define PRAGMA_STR_(x) _Pragma(#x)
 #define PRAGMA_(x) PRAGMA_STR_(x)
 #define UNROLL_J PRAGMA_(unroll FORCE_UNROLL)
@@ -681,16 +673,10 @@ __global__ void __launch_bounds__(REFINE_THREADS) k_force_refine(const DevHeader
 // (unscaled by G), in a fixed summation order; k_force adds these to the group's own sums.
 // ------------------------------------------------------------------------------------------------
 #define UW 4                   // warps per CTA
-#ifndef UNITS_MIN_CTAS
 #define UNITS_MIN_CTAS 3
-#endif
-#ifndef NI
 #define NI 4                   // i-particles per lane
-#endif
 #define UNIT_MAX (32 * NI)     // particles per unit
-#ifndef UT
 #define UT 32                  // cells per staged warp tile
-#endif
 #define UREC (UT / 32)
 struct UBuf { float4 q0[UT], q1[UT], q2[UT]; float q3[UT]; };          // 3328 B
 
@@ -1110,20 +1096,89 @@ __global__ void __launch_bounds__(128, 4) k_probe_cell(float* __restrict__ out, 
     if (s == 123.456f) out[0] = s;
 }
 
+// mode 3: the PACKED quadrupole cell term of the force kernels (two packed pairs = 4 i-particles per thread, cells broadcast
+// from shared memory as scalars): the rate attainable by the kernels' own instruction mix
+__global__ void __launch_bounds__(128, 4) k_probe_cell2(float* __restrict__ out, long long iters) {
+    __shared__ float4 q0[64], q1[64];
+    __shared__ float2 q2[64];
+    const int t = threadIdx.x;
+    if (t < 64) {
+        q0[t] = make_float4(10.f + t, 20.f - t, 30.f + 0.5f * t, 1.f + 0.01f * t);
+        q1[t] = make_float4(1e-3f * t, -2e-3f * t, 1e-3f * t, 3e-4f * t);
+        q2[t] = make_float2(-1e-4f * t, 2e-4f * t);
+    }
+    __syncthreads();
+    f2 nx[2], ny[2], nz[2];
+    Acc2 p[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        nx[k] = make_float2(-(t * 0.01f + 2 * k + out[0]), -(t * 0.01f + 2 * k + 1 + out[0]));
+        ny[k] = make_float2(-(t * 0.02f - 2 * k), -(t * 0.02f - 2 * k - 1));
+        nz[k] = make_float2(-(0.5f * k + out[0]), -(0.5f * k + 0.25f + out[0]));
+        p[k].ax = p[k].ay = p[k].az = p[k].pot = make_float2(0.f, 0.f);
+    }
+    for (long long it = 0; it < iters; ++it) {
+#pragma unroll 1
+        for (int j = 0; j < 64; ++j) {
+            const float4 a = q0[j], b = q1[j]; const float2 c = q2[j];
+#pragma unroll
+            for (int k = 0; k < 2; ++k) cell_term2<true>(p[k], add2(bc(a.x), nx[k]), add2(bc(a.y), ny[k]), add2(bc(a.z), nz[k]), a.w, b.x, b.y, b.z, b.w, c.x, c.y);
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) s += p[k].ax.x + p[k].ay.x + p[k].az.x + p[k].pot.x + p[k].ax.y + p[k].ay.y + p[k].az.y + p[k].pot.y;
+    if (s == 123.456f) out[0] = s;
+}
+// modes 4-7: operand patterns that separate the register-bank model from a plain "operands per clock" model
+// (profiles/fp32_issue_model_r02.md).  8 chains per thread, 4 warps per sub-partition.
+template <int PAT>
+__global__ void __launch_bounds__(128) k_probe_pattern(float* __restrict__ out, long long iters, float s0, float s1) {
+    float a[8], b[8], c[8], d[8];
+#pragma unroll
+    // every operand depends on the thread index: a warp-uniform value would be kept in a uniform register, which costs no register-file read
+    for (int i = 0; i < 8; ++i) { a[i] = threadIdx.x * 1e-3f + i; b[i] = 1.0f + 1e-6f * (threadIdx.x + i); c[i] = 1e-3f * (i + 1) + s1 * threadIdx.x; d[i] = 0.5f * i + s0 * threadIdx.x; }
+    const float e = s0 * threadIdx.x + 0.25f;
+    for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if (PAT == 4) a[i] = fmaf(b[i], c[i], a[i]);                                    // three distinct registers, independent chains
+            if (PAT == 5) a[i] = fmaf(b[i], b[i], a[i]);                                    // two distinct registers
+            if (PAT == 6) { a[i] = fmaf(b[i], e, a[i]); c[i] = fmaf(d[i], e, c[i]); }       // one operand shared by every instruction
+            if (PAT == 7) { a[i] = fmaf(b[i], c[i], d[i]); d[i] = a[i] + e; }               // FFMA (3 registers) + FADD (2 registers)
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i] + b[i] + c[i] + d[i];
+    if (s == 123.456f) out[0] = s;
+}
+
 extern "C" int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream) {
     if (mode == 0) return petar_probe_fp32(iters, flops_out_host, scratch_dev, cuda_stream);
-    if (mode != 1 && mode != 2) return PETAR_EINVAL;
+    if (mode < 1 || mode > 7) return PETAR_EINVAL;
     int dev = 0, sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return PETAR_ECUDA;
     if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PETAR_ECUDA;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
     if (mode == 1) {
         const int grid = sm * 8;
-        k_probe_ffma3<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(scratch_dev, (long long)iters);
+        k_probe_ffma3<<<grid, 256, 0, s>>>(scratch_dev, (long long)iters);
         if (flops_out_host) *flops_out_host = 2.0 * 16.0 * (double)iters * 256.0 * (double)grid;
-    } else {
+    } else if (mode == 2 || mode == 3) {
         const int grid = sm * 4;
-        k_probe_cell<<<grid, 128, 0, (cudaStream_t)cuda_stream>>>(scratch_dev, (long long)iters);
+        if (mode == 2) k_probe_cell<<<grid, 128, 0, s>>>(scratch_dev, (long long)iters);
+        else k_probe_cell2<<<grid, 128, 0, s>>>(scratch_dev, (long long)iters);
         if (flops_out_host) *flops_out_host = 53.0 * 4.0 * 64.0 * (double)iters * 128.0 * (double)grid;
+    } else {
+        const int grid = sm * 4;        // 4 CTAs x 4 warps per SM: 4 warps per sub-partition
+        const double per = (mode == 6 || mode == 7) ? 2.0 : 1.0;       // instructions per chain and iteration
+        if (mode == 4) k_probe_pattern<4><<<grid, 128, 0, s>>>(scratch_dev, (long long)iters, 0.999f, 1e-3f);
+        if (mode == 5) k_probe_pattern<5><<<grid, 128, 0, s>>>(scratch_dev, (long long)iters, 0.999f, 1e-3f);
+        if (mode == 6) k_probe_pattern<6><<<grid, 128, 0, s>>>(scratch_dev, (long long)iters, 0.999f, 1e-3f);
+        if (mode == 7) k_probe_pattern<7><<<grid, 128, 0, s>>>(scratch_dev, (long long)iters, 0.999f, 1e-3f);
+        // *flops_out_host = thread-level INSTRUCTIONS x 2 (so that value / time / nominal peak = warp instructions per clock and sub-partition)
+        if (flops_out_host) *flops_out_host = 2.0 * 8.0 * per * (double)iters * 128.0 * (double)grid;
     }
     petar_count_launch(1);
     return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;

@@ -11,19 +11,10 @@
 #define PETAR_CHUNK_HDR 2
 #define PETAR_CHUNK_PAYLOAD (PETAR_CHUNK - PETAR_CHUNK_HDR)   // 1022 entries (even: EP ranges are pairs)
 // super-group levels (see SuperRec): level l holds the tree cells with <= PETAR_SUP_LIMIT(l) members
-#ifndef PETAR_NSUP
 #define PETAR_NSUP 2
-#endif
-#ifndef PETAR_SUP_T0
 #define PETAR_SUP_T0 4096
-#endif
-#ifndef PETAR_SUP_T1
 #define PETAR_SUP_T1 512
-#endif
-#ifndef PETAR_SUP_T2
-#define PETAR_SUP_T2 128
-#endif
-#define PETAR_SUP_LIMIT(l) ((l) == 0 ? PETAR_SUP_T0 : (l) == 1 ? PETAR_SUP_T1 : PETAR_SUP_T2)
+#define PETAR_SUP_LIMIT(l) ((l) == 0 ? PETAR_SUP_T0 : PETAR_SUP_T1)
 #define PETAR_UNIT_CLASSES 4       // phase-A force units of 128, 64, 32 and < 32 particles
 
 // ---- device-resident header (one per tree, lives at the start of the workspace) -----------------

@@ -4,9 +4,7 @@
 #include "internal.cuh"
 
 #define WALK_WARPS 8
-#ifndef WALK_STACK
 #define WALK_STACK 1504          // frontier entries per warp (shared memory)
-#endif
 
 // warp-uniform cursor of one chunked list
 struct ListCursor {
@@ -245,9 +243,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk_super(DevHeader* __res
 }
 
          // > 7 * 21: room for a pure depth-first descent from any state
-#ifndef WALK_MIN_CTAS
 #define WALK_MIN_CTAS 3
-#endif
 __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
                                                           const NodeMac* __restrict__ nmac, GroupRec* __restrict__ grp,
                                                           const SuperRec* __restrict__ srec, const int* __restrict__ smap,
