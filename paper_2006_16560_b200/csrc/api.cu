@@ -78,6 +78,7 @@ static size_t carve(Workspace* w, char* base, int64_t N, const petar_params* p) 
     W->idx = (unsigned*)take(n * 4); W->idx_alt = (unsigned*)take(n * 4);
     W->sort_hist = (unsigned*)take(8 * 256 * 4);
     W->sort_blk = (unsigned*)take((size_t)256 * nblk * 4);
+    W->rec = (double2*)take(n * 64);
     W->xs = (double*)take(n * 8); W->ys = (double*)take(n * 8); W->zs = (double*)take(n * 8);
     W->ms = (double*)take(n * 8); W->routs = (double*)take(n * 8); W->rss = (double*)take(n * 8);
     W->vxs = (double*)take(n * 8); W->vys = (double*)take(n * 8); W->vzs = (double*)take(n * 8);

@@ -122,21 +122,35 @@ __device__ __forceinline__ unsigned long long morton_key(const double vx, const 
     }
     return (spread21(q[0]) << 2) | (spread21(q[1]) << 1) | spread21(q[2]);
 }
+// Also packs the particle's inputs into one 64-byte record (x, y, z, m, r_out, r_search, -, -) in the caller's order: the
+// gather by the sorted permutation then fetches ONE aligned 64-byte record per particle instead of five or six scattered
+// 8-byte values, each of which costs a 64-128-byte DRAM fetch (profiles/hbm_r02_config5.md: 604 -> ~140 bytes moved per particle).
 __global__ void __launch_bounds__(256) k_keys(const double* __restrict__ x, const double* __restrict__ y,
-                                              const double* __restrict__ z, long long n, const DevHeader* __restrict__ h,
-                                              unsigned long long* __restrict__ key, unsigned* __restrict__ idx) {
+                                              const double* __restrict__ z, const double* __restrict__ m, const double* __restrict__ ro,
+                                              const double* __restrict__ rs, long long n, const DevHeader* __restrict__ h,
+                                              unsigned long long* __restrict__ key, unsigned* __restrict__ idx, double2* __restrict__ rec) {
     const long long i = 2 * (blockIdx.x * (long long)blockDim.x + threadIdx.x);
     if (i >= n) return;
     const double inv_s = h->inv_s, o0 = h->o[0], o1 = h->o[1], o2 = h->o[2];
-    const bool vec = ((((uintptr_t)x) | ((uintptr_t)y) | ((uintptr_t)z)) & 15u) == 0;
+    const bool vec = ((((uintptr_t)x) | ((uintptr_t)y) | ((uintptr_t)z) | ((uintptr_t)m) | ((uintptr_t)ro) | ((uintptr_t)rs)) & 15u) == 0;
     if (vec && i + 1 < n) {
         const double2 vx = *reinterpret_cast<const double2*>(x + i), vy = *reinterpret_cast<const double2*>(y + i), vz = *reinterpret_cast<const double2*>(z + i);
+        const double2 vm = *reinterpret_cast<const double2*>(m + i), vr = *reinterpret_cast<const double2*>(ro + i);
+        const double2 vs = rs ? *reinterpret_cast<const double2*>(rs + i) : vr;
         ulonglong2 k2;
         k2.x = morton_key(vx.x, vy.x, vz.x, o0, o1, o2, inv_s); k2.y = morton_key(vx.y, vy.y, vz.y, o0, o1, o2, inv_s);
         *reinterpret_cast<ulonglong2*>(key + i) = k2;
         *reinterpret_cast<uint2*>(idx + i) = make_uint2((unsigned)i, (unsigned)i + 1u);
+        double2* r = rec + 4 * i;
+        r[0] = make_double2(vx.x, vy.x); r[1] = make_double2(vz.x, vm.x); r[2] = make_double2(vr.x, vs.x); r[3] = make_double2(0.0, 0.0);
+        r[4] = make_double2(vx.y, vy.y); r[5] = make_double2(vz.y, vm.y); r[6] = make_double2(vr.y, vs.y); r[7] = make_double2(0.0, 0.0);
     } else {
-        for (long long j = i; j < min(i + 2, n); ++j) { key[j] = morton_key(x[j], y[j], z[j], o0, o1, o2, inv_s); idx[j] = (unsigned)j; }
+        for (long long j = i; j < min(i + 2, n); ++j) {
+            key[j] = morton_key(x[j], y[j], z[j], o0, o1, o2, inv_s); idx[j] = (unsigned)j;
+            double2* r = rec + 4 * j;
+            const double vr = ro[j];
+            r[0] = make_double2(x[j], y[j]); r[1] = make_double2(z[j], m[j]); r[2] = make_double2(vr, rs ? rs[j] : vr); r[3] = make_double2(0.0, 0.0);
+        }
     }
 }
 
@@ -246,23 +260,22 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort_scatter(const unsigned lo
 // ------------------------------------------------------------------------------------------------
 // S3: gather into sorted order + fp32 float-float records relative to the root centre
 // ------------------------------------------------------------------------------------------------
-// One sorted position per thread (the permuted 8-byte loads are what bounds this kernel: one 32-byte sector per value; four
-// positions per thread with 32-byte stores measured slower, 1.23 vs 1.03 ms at N = 10^7).  Also the finiteness / sign checks
-// of m, r_out, r_search (the positions were checked by k_bbox).
+// One sorted position per thread: its 64-byte input record (packed by k_keys) is fetched with four 16-byte loads.  Also the
+// finiteness / sign checks of m, r_out, r_search (the positions were checked by k_bbox).
 __global__ void __launch_bounds__(256) k_gather(const unsigned* __restrict__ idx, long long n, DevHeader* __restrict__ h,
-                                                const double* __restrict__ x, const double* __restrict__ y, const double* __restrict__ z,
-                                                const double* __restrict__ m, const double* __restrict__ ro, const double* __restrict__ rs,
+                                                const double2* __restrict__ rec, const bool have_rs,
                                                 double* __restrict__ xs, double* __restrict__ ys, double* __restrict__ zs,
                                                 double* __restrict__ ms, double* __restrict__ ros, double* __restrict__ rss,
                                                 float4* __restrict__ pa, float4* __restrict__ pb) {
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     bool bad = false;
     if (i < n) {
-        const unsigned o = idx[i];
-        const double vx = x[o], vy = y[o], vz = z[o], vm = m[o], vr = ro[o];
+        const double2* r = rec + 4 * (size_t)idx[i];
+        const double2 r0 = r[0], r1 = r[1], r2 = r[2];
+        const double vx = r0.x, vy = r0.y, vz = r1.x, vm = r1.y, vr = r2.x, vq = r2.y;
         bad = !(isfinite(vm) && isfinite(vr) && vr > 0.0);
         xs[i] = vx; ys[i] = vy; zs[i] = vz; ms[i] = vm; ros[i] = vr;
-        if (rs) { const double q = rs[o]; rss[i] = q; bad |= !(isfinite(q) && q >= vr); }
+        if (have_rs) { rss[i] = vq; bad |= !(isfinite(vq) && vq >= vr); }
         const double dx = vx - h->c[0], dy = vy - h->c[1], dz = vz - h->c[2];
         const float xh = (float)dx, yh = (float)dy, zh = (float)dz;
         const float xl = (float)(dx - (double)xh), yl = (float)(dy - (double)yh), zl = (float)(dz - (double)zh);
@@ -752,7 +765,7 @@ cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s) {
     KCHECK(s, "k_bbox");
     k_root<<<1, 32, 0, s>>>(w.hdr);
     KCHECK(s, "k_root");
-    k_keys<<<cdiv(n, 512), 256, 0, s>>>(t->x, t->y, t->z, n, w.hdr, w.key, w.idx);
+    k_keys<<<cdiv(n, 512), 256, 0, s>>>(t->x, t->y, t->z, t->m, t->r_out, t->r_search, n, w.hdr, w.key, w.idx, w.rec);
     KCHECK(s, "k_keys");
     petar_count_launch(4);
     stage_end(t, PETAR_STAGE_BBOX_KEYS, s);
@@ -766,7 +779,7 @@ cudaError_t launch_keys_sort_gather(petar_tree* t, cudaStream_t s) {
     stage_end(t, PETAR_STAGE_SORT, s);
 
     stage_begin(t, PETAR_STAGE_GATHER, s);
-    k_gather<<<cdiv(n, 256), 256, 0, s>>>(w.idx, n, w.hdr, t->x, t->y, t->z, t->m, t->r_out, t->r_search,
+    k_gather<<<cdiv(n, 256), 256, 0, s>>>(w.idx, n, w.hdr, w.rec, t->r_search != nullptr,
                                           w.xs, w.ys, w.zs, w.ms, w.routs, t->r_search ? w.rss : nullptr, w.pa, w.pb);
     KCHECK(s, "k_gather");
     petar_count_launch(1);

@@ -93,6 +93,7 @@ struct Workspace {
     unsigned int *idx, *idx_alt;
     unsigned int *sort_hist;       // [8][256] global digit totals, then per-pass block counts
     unsigned int *sort_blk;        // [256][nblk]
+    double2* rec;                  // [N][4] packed inputs in the caller's order: (x, y), (z, m), (r_out, r_search), -
     // sorted particle data
     double *xs, *ys, *zs, *ms, *routs, *rss;
     double *vxs, *vys, *vzs;       // sorted velocities (petar_neighbor_list_orbit only)
