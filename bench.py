@@ -34,7 +34,7 @@ sys.path.insert(0, ROOT)
 FLOP_NEWTON, FLOP_CUT, FLOP_QUAD = 20, 49, 53      # fixed flops-per-interaction convention
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the force kernels, from the committed `ncu --set full` capture of
 # THIS round's build at config 3 (profiles/ncu_r02_force.md).  Emitted only for that configuration; any other run reports null.
-TRAFFIC_NCU = {"capture": "profiles/ncu_r02_force.md", "config": 3, "k_force_units": 187.2e6, "k_force": 1237.5e6}
+TRAFFIC_NCU = {"capture": "profiles/ncu_r02_force.md", "config": 3, "k_force_units": 207.0e6, "k_force": 1230.7e6}
 
 
 def parse():
@@ -253,6 +253,23 @@ def main():
     ms_total = sum(a.elapsed_time(b) for a, b in ev)
     status = P.petar_tree_status(tree.handle)
 
+    # ---- the same work with the calls in the other order (neighbour count first): the per-group walk then runs ALONE before the
+    #      force kernels instead of beside force phase A, which gives every kernel's duration without the overlap (not part of `value`)
+    stage_seq = {k: 0.0 for k in P.STAGE_NAMES}
+    seq_ms = 0.0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for rep in range(3):
+        flush.fill_(rep)
+        e0.record(stream)
+        tree.build(stream)
+        P.petar_neighbor_list(tree.handle, tree.offsets, None, 0, None, stream)
+        P.petar_long_range_force(tree.handle, tree.acc_x, tree.acc_y, tree.acc_z, tree.pot, False, stream)
+        P.petar_neighbor_list(tree.handle, tree.offsets, cap[0], cap[0].numel(), tree.nb_status, stream)
+        e1.record(stream); e1.synchronize()
+        seq_ms += e0.elapsed_time(e1) / 3
+        for name, v in P.petar_stage_times(tree.handle).items():
+            stage_seq[name] += v / 3
+
     # ---- e2e: HOST buffers through the C-ABI, copies inside the timed region ---------------------------
     host_out = [torch.empty(N, dtype=torch.float64).pin_memory() for _ in range(4)]
     host_off = torch.empty(N + 1, dtype=torch.int64).pin_memory()
@@ -458,7 +475,9 @@ def main():
             hbm_stages[name] = dict(ms=ms_st, bytes_per_particle=bpp, achieved_gbs=gbs, frac_of_hbm=gbs / hbm_peak)
     kern = [dict(kernel="k_force_units", ms=stage_ms["force_units"], flops_per_launch=float(flops_units)),
             dict(kernel="k_force", ms=stage_ms["force"], flops_per_launch=float(flops_groups))]
+    kern[0]["ms_alone"], kern[1]["ms_alone"] = stage_seq["force_units"], stage_seq["force"]
     for kd in kern:
+        kd["frac_alone"] = kd["flops_per_launch"] / (kd["ms_alone"] * 1e-3) / 1e12 / nominal_fp32 if kd["ms_alone"] > 0 else 0.0
         kd["achieved"] = kd["flops_per_launch"] / (kd["ms"] * 1e-3) / 1e12 if kd["ms"] > 0 else 0.0
         kd["frac"] = kd["achieved"] / nominal_fp32
         kd["share_of_step"] = kd["ms"] / ms_step
@@ -479,6 +498,9 @@ def main():
                     "n_epep_changeover": int(counts.n_epep_near), "neighbours": nb_total, "n_groups": int(counts.n_groups),
                     "n_nodes": int(counts.n_nodes), "status": status, "multi_gpu": "replicas only (no data-path collective)"},
             stage_ms=stage_ms,
+            stage_ms_sequential=dict(stage_seq, step=seq_ms,
+                                     note="calls in the order build, neighbour count, force, neighbour fill: the per-group walk runs alone; "
+                                          "kernel durations without the overlap (3 repetitions after the timed region)"),
             stage_note="the per-group walk (stage walk) runs on the library's side stream BESIDE force phase A (stage force_units): the two "
                        "stage times overlap and each is longer than when run alone",
             hbm_stages=dict(peak_gbs=hbm_peak, note="keys / sort / tree stages: algorithmic bytes over stage time; at N = 2^20 the working "
