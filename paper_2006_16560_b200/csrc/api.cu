@@ -182,7 +182,7 @@ extern "C" int petar_tree_rebuild(petar_tree* t, const double* x, const double* 
     return build_into(t, x, y, z, m, r_out, r_search, (cudaStream_t)cuda_stream);
 }
 
-#define OVERLAP_WALK_CTAS 1      // CTAs per SM of k_walk / k_force_units while the two run side by side
+#define OVERLAP_WALK_CTAS 2      // CTAs per SM of k_walk / k_force_units while the two run side by side
 #define OVERLAP_UNITS_CTAS 0      // 0 = no limit: the walk CTA is resident first, two unit CTAs fit beside it, the third follows when it leaves
 static int check_tree(petar_tree* t) { return (t && t->magic == PETAR_MAGIC && t->built) ? PETAR_OK : PETAR_ENOTBUILT; }
 

@@ -25,6 +25,8 @@
 // 48-byte records one tile ahead in registers, current tile in double-buffered shared memory), so
 // the dependent id -> record loads overlap the arithmetic.
 // fp32 partial sums live only across one tile slice and are flushed into fp64 accumulators.
+#include <stdio.h>
+#include <stdlib.h>
 #include "internal.cuh"
 
 #define FT 128                 // threads per CTA
@@ -852,17 +854,18 @@ __global__ void __launch_bounds__(UW * 32, UNITS_MIN_CTAS) k_force_units(DevHead
                                                             const int group_cap, const NodeW* __restrict__ nw,
                                                             const int* __restrict__ arena, const NodeSp* __restrict__ nsp,
                                                             const float4* __restrict__ pa, const float4* __restrict__ pb,
-                                                            double* __restrict__ part, double* __restrict__ part_s, const long long n_part) {
+                                                            double* __restrict__ part, double* __restrict__ part_s, const long long n_part, const int first_class) {
     __shared__ __align__(16) UBuf s_buf[UW][2];
     __shared__ double s_acc[5 * NI][UW * 32];
     __shared__ int s_u;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     double* sacc = &s_acc[0][threadIdx.x];
     const int nu = h->unit_off[PETAR_UNIT_CLASSES];
+    const int u0 = h->unit_off[first_class];       // units of the classes before first_class belong to k_force_units_tc
     if (h->status != 0) return;            // see k_force
     for (;;) {
         __syncthreads();                    // s_u and s_acc of the previous unit consumed
-        if (threadIdx.x == 0) s_u = atomicAdd(&h->unit_ticket, 1);
+        if (threadIdx.x == 0) s_u = u0 + atomicAdd(&h->unit_ticket, 1);
         __syncthreads();
         const int u = s_u;
         if (u >= nu) break;
@@ -891,12 +894,360 @@ __global__ void __launch_bounds__(UW * 32, UNITS_MIN_CTAS) k_force_units(DevHead
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Phase A on the tensor cores (k_force_units_tc): units of 80..128 particles against the PLAIN common cells of their
+// super-group.  The quadrupole part of a cell term is bilinear in particle and cell data: with d = c - x (both relative
+// to the unit's origin gh) and phi(x) = [x, y, z, 1, x^2, y^2, z^2, xy, xz, yz],
+//     d.B.d   = phi(x) . [-2(Bc)x, -2(Bc)y, -2(Bc)z, c.B.c, Bxx, Byy, Bzz, 2Bxy, 2Bxz, 2Byz]
+//     (B d)_x = phi(x) . [-Bxx, -Bxy, -Bxz, (Bc)x, 0, ...]          (likewise y, z)
+// so the four numbers that cost 12 of the 33 FP32 instructions of cell_term2 are one GEMM per tile:
+//     D[128 particles x (4 outputs x 16 cells)] = A[128 x 32] * B[32 x 64]        (tcgen05.mma kind::tf32, fp32 accumulate in TMEM)
+// Precision: tf32 keeps 11 significant bits, so every operand is split v = hi + lo (hi = v with the low 13 mantissa bits
+// cleared, lo = v - hi exactly) and the K dimension holds three blocks, A = [phi_hi | phi_lo | phi_hi], B = [psi_hi | psi_hi | psi_lo]:
+// hi*hi + lo*hi + hi*lo carries ~2^-21 relative error per product, on terms (the quadrupole correction) that are at most a
+// few per cent of the monopole.  The monopole, r^2 and 1/r stay in fp32 on the CUDA cores.
+// Roles: warp 4 = producer (gathers the 48-byte cell records of a tile, builds the B operand and the (c, M) pairs in
+// shared memory, issues the MMAs); warps 0-3 = consumers, thread t owns particle t = TMEM lane t, reads its four
+// numbers per cell with tcgen05.ld and evaluates TWO cells per packed fp32x2 instruction (21 FP32 + 2 MUFU per pair).
+// Tiles are double-buffered in shared memory and TMEM: full[b] (MMA done -> consumers), empty[b] (consumers -> producer).
+// The short PRECISE lists (cells closer to the box than its edge) follow on the CUDA cores with float-float coordinates.
+// ------------------------------------------------------------------------------------------------
+#define TC_CELLS 32                   // cells per tile (one per producer lane)
+#define TC_N (4 * TC_CELLS)           // MMA N = TMEM columns per tile buffer
+#define TC_K 32                       // 3 x 10 split features + 2 zero columns = 4 MMAs of K = 8
+#define TC_PRODUCERS 2                // producer warps: producer p stages the tiles whose running number is p mod 2 (and owns TMEM buffer p)
+#define TC_SETS 1                     // consumer warp sets: set h (warps 4h .. 4h+3) evaluates cell pairs h, h + TC_SETS, ... of every tile
+#define TC_CONSUMERS (128 * TC_SETS)
+#define TC_THREADS (TC_CONSUMERS + 32 * TC_PRODUCERS)
+#define TC_MIN_CTAS 2                 // CTAs per SM (2 x TC_BUFS x TC_N = 512 TMEM columns)
+#define TC_REG_CTAS 3                 // register cap (112): two CTAs leave room for one k_walk CTA, which runs beside this kernel
+#define TC_BUFS 2                     // tile buffers in tensor memory per CTA
+#define TC_UNIT_MIN 80                // smaller units go to k_force_units
+#define TC_LBO 128u                   // bytes between core matrices adjacent in K (no-swizzle K-major canonical layout)
+#define TC_SBO (128u * (TC_K / 4))    // bytes between 8-row groups of A
+#define TC_SBO_B (TC_SBO + 32u)       // ... of B: padded so that the producer's 16-byte stores of 8 lanes fall into 8 different bank groups
+#define TC_STAGES 4                   // shared-memory stages of B and C (tensor memory holds TC_BUFS tiles)
+#define TC_STAGE_BYTES ((TC_N / 8) * TC_SBO_B)
+#define TC_FLUSH 4                    // tiles between flushes of the fp32 partial sums into the fp64 accumulators
+#define TC_TPC ((PETAR_CHUNK_PAYLOAD + TC_CELLS - 1) / TC_CELLS)      // tiles per full chunk (a tile never straddles a chunk)
+struct __align__(128) TcSmem {
+    union {
+        float A[128 * TC_K];                        // particles: row t at (t/8) SBO + (t%8) 16 B, k-chunk kc at kc LBO
+        float4 P[4 * TC_SETS][3][32];               // per consumer warp: staged records of the precise list (after the unit's last MMA)
+        double R[128][5];                           // sums of the consumer sets > 0, added by set 0 (after the precise list)
+    };
+    float B[TC_STAGES][TC_STAGE_BYTES / 4];         // cells: row n = 8 (cell/2) + 2 output + (cell&1)
+    float4 C[TC_STAGES][TC_CELLS / 2][2];           // (cx0, cx1, cy0, cy1), (cz0, cz1, M0, M1) of a cell pair
+    unsigned long long full[TC_BUFS], empty[TC_BUFS];       // TC_PRODUCERS == TC_BUFS: a producer is never more than one phase ahead of its buffer
+    uint32_t tmem_base;
+    int unit;
+};
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_wait(const uint32_t bar, const uint32_t parity) {
+    uint32_t done = 0;
+    while (!done) asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ uint64_t tc_desc(const uint32_t saddr, const uint32_t sbo) {
+    return (uint64_t)((saddr >> 4) & 0x3fffu) | ((uint64_t)(TC_LBO >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) | (1ull << 46);
+}
+__device__ __forceinline__ void split_tf32(const float v, float& hi, float& lo) { hi = __uint_as_float(__float_as_uint(v) & 0xffffe000u); lo = v - hi; }
+__device__ __forceinline__ int tc_tiles(const int n) {
+    const int full = n / PETAR_CHUNK_PAYLOAD, rem = n - full * PETAR_CHUNK_PAYLOAD;
+    return full * TC_TPC + (rem + TC_CELLS - 1) / TC_CELLS;
+}
+
+// 16 TMEM columns of this thread's lane: (dbd, bdx, bdy, bdz) x (cell j, j+1) for two cell pairs
+__device__ __forceinline__ void tc_ld16(uint32_t (&v)[16], const uint32_t taddr) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr));
+}
+// two cell pairs against one particle: the halves of every float2 are the cells j and j + 1; the particle's negated coordinates are
+// broadcast scalars.  Same algebra as cell_term2, with d.B.d and B d read from tensor memory.
+__device__ __forceinline__ void tc_pairs(Acc2& p, const uint32_t (&v)[16], const float4 (&cpair)[4], const float nx, const float ny, const float nz) {
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const float4 c0 = cpair[2 * q], c1 = cpair[2 * q + 1];
+        const f2 dx = add2(make_float2(c0.x, c0.y), bc(nx)), dy = add2(make_float2(c0.z, c0.w), bc(ny)), dz = add2(make_float2(c1.x, c1.y), bc(nz));
+        const f2 Mp = make_float2(c1.z, c1.w);
+        const f2 dbd = make_float2(__uint_as_float(v[8 * q + 0]), __uint_as_float(v[8 * q + 1]));
+        const f2 bdx = make_float2(__uint_as_float(v[8 * q + 2]), __uint_as_float(v[8 * q + 3]));
+        const f2 bdy = make_float2(__uint_as_float(v[8 * q + 4]), __uint_as_float(v[8 * q + 5]));
+        const f2 bdz = make_float2(__uint_as_float(v[8 * q + 6]), __uint_as_float(v[8 * q + 7]));
+        const f2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+        f2 rinv; rinv.x = rsqrt_ftz(r2.x); rinv.y = rsqrt_ftz(r2.y);
+        const f2 rinv2 = mul2(rinv, rinv);
+        const f2 mr = mul2(Mp, rinv);
+        const f2 rinv4 = mul2(rinv2, rinv2);
+        const f2 rinv5 = mul2(rinv4, rinv);
+        const f2 uu = mul2(dbd, rinv5);
+        p.pot = fma2(uu, bc(-0.5f), add2(p.pot, mr));
+        const f2 ff = mul2(fma2(uu, bc(-2.5f), mr), rinv2);
+        p.ax = fma2(ff, dx, fma2(rinv5, bdx, p.ax));
+        p.ay = fma2(ff, dy, fma2(rinv5, bdy, p.ay));
+        p.az = fma2(ff, dz, fma2(rinv5, bdz, p.az));
+    }
+}
+
+__global__ void __launch_bounds__(TC_THREADS, TC_REG_CTAS) k_force_units_tc(DevHeader* __restrict__ h, const ForceUnit* __restrict__ units, const SuperRec* __restrict__ srec,
+                                                                    const int group_cap, const NodeW* __restrict__ nw,
+                                                                    const int* __restrict__ arena, const NodeSp* __restrict__ nsp,
+                                                                    const float4* __restrict__ pa, const float4* __restrict__ pb,
+                                                                    double* __restrict__ part, double* __restrict__ part_s, const long long n_part) {
+    extern __shared__ __align__(128) unsigned char tc_smem_raw[];
+    TcSmem& sm = *reinterpret_cast<TcSmem*>(tc_smem_raw);
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const int nu = h->unit_off[1];                 // class 0
+    if (h->status != 0) return;
+    if (t == 0) {
+        for (int q = 0; q < TC_BUFS; ++q) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&sm.full[q])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&sm.empty[q])), "n"(4 * TC_SETS));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    if (w == TC_CONSUMERS / 32) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&sm.tmem_base)), "n"(TC_BUFS * TC_N));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    for (int e = t; e < (int)(sizeof(sm.B) / 4); e += TC_THREADS) (&sm.B[0][0])[e] = 0.f;      // the zero entries of B are never rewritten
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem = sm.tmem_base;
+    uint32_t ctr = 0;                                // tiles handled so far by this CTA (producers and consumers count alike)
+    for (;;) {
+        if (t == 0) sm.unit = atomicAdd(&h->unit_ticket_tc, 1);
+        __syncthreads();
+        const int u = sm.unit;
+        if (u >= nu) break;
+        const ForceUnit fu = units[u];
+        const int cnt = fu.cnt;
+        const SuperRec* sr = &srec[(size_t)fu.level * group_cap + fu.rec];
+        const int head_sp = sr->head_sp, n_sp = sr->n_sp;
+        const float4 ba = nw[sr->node].a, bb = nw[sr->node].b;
+        const float3 gh = make_float3(0.5f * (ba.x + ba.w), 0.5f * (ba.y + bb.x), 0.5f * (ba.z + bb.y));
+        const int nt = tc_tiles(n_sp);
+        float4 ia = make_float4(0.f, 0.f, 0.f, 0.f), ib = ia;
+        float x = 0.f, y = 0.f, z = 0.f;
+        const int ti = t & 127;                      // consumers: the thread's particle = its TMEM lane
+        if (w < TC_CONSUMERS / 32) {
+            const int i = fu.ibeg + min(ti, cnt - 1);
+            ia = pa[i]; ib = pb[i];
+            x = (ia.x - gh.x) + ib.x; y = (ia.y - gh.y) + ib.y; z = (ia.z - gh.z) + ib.z;
+        }
+        if (w < 4) {
+            const float f[10] = {x, y, z, 1.0f, x * x, y * y, z * z, x * y, x * z, y * z};
+            float fh[10], fl[10];
+#pragma unroll
+            for (int k = 0; k < 10; ++k) split_tf32(f[k], fh[k], fl[k]);
+            float4* row = reinterpret_cast<float4*>(reinterpret_cast<char*>(sm.A) + (size_t)(t >> 3) * TC_SBO + (size_t)(t & 7) * 16);
+            const int cs = TC_LBO / 16;      // float4 stride between k-chunks
+            row[0 * cs] = make_float4(fh[0], fh[1], fh[2], fh[3]);
+            row[1 * cs] = make_float4(fh[4], fh[5], fh[6], fh[7]);
+            row[2 * cs] = make_float4(fh[8], fh[9], fl[0], fl[1]);
+            row[3 * cs] = make_float4(fl[2], fl[3], fl[4], fl[5]);
+            row[4 * cs] = make_float4(fl[6], fl[7], fl[8], fl[9]);
+            row[5 * cs] = make_float4(fh[0], fh[1], fh[2], fh[3]);
+            row[6 * cs] = make_float4(fh[4], fh[5], fh[6], fh[7]);
+            row[7 * cs] = make_float4(fh[8], fh[9], 0.f, 0.f);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        }
+        __syncthreads();
+        if (w >= TC_CONSUMERS / 32) {
+            // ================= producers =================
+            const int pr = w - TC_CONSUMERS / 32;
+            const int c = lane;
+            // this warp's tiles: k = k0, k0 + TC_PRODUCERS, ... (those whose running number ctr + k is pr mod TC_PRODUCERS)
+            const int k0 = (int)((pr - ctr) & (TC_PRODUCERS - 1));
+            int qi = 0;                                    // chunk the cursor stands on
+            const int* cp = arena + (size_t)(n_sp > 0 ? head_sp : 0) * PETAR_CHUNK;
+            int tn1 = 0, tn2 = 0, id2 = 0;
+            float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f), q1 = q0, q2 = q0;
+            auto load_ids = [&](const int k) {         // ids of tile k
+                tn2 = 0;
+                if (k < nt) {
+                    const int q = k / TC_TPC, off = (k - q * TC_TPC) * TC_CELLS;
+                    while (qi < q) { cp = arena + (size_t)cp[0] * PETAR_CHUNK; ++qi; }
+                    tn2 = min(TC_CELLS, min(n_sp - q * PETAR_CHUNK_PAYLOAD, PETAR_CHUNK_PAYLOAD) - off);
+                    if (c < tn2) id2 = cp[PETAR_CHUNK_HDR + off + c];
+                }
+            };
+            auto load_recs = [&]() {
+                tn1 = tn2;
+                if (c < tn1) { const NodeSp* sp = &nsp[id2]; q0 = sp->q0; q1 = sp->q1; q2 = sp->q2; }
+            };
+            load_ids(k0); load_recs(); load_ids(k0 + TC_PRODUCERS);
+            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+            const uint64_t da0 = tc_desc(smem_u32(sm.A), TC_SBO), db0 = tc_desc(smem_u32(sm.B[0]), TC_SBO_B);
+            for (int k = k0; k < nt; k += TC_PRODUCERS) {
+                const uint32_t cc = ctr + (uint32_t)k;
+                const int b = cc & (TC_BUFS - 1), sg = cc & (TC_STAGES - 1);
+                // the tile's operands from the records in registers
+                float cx = 1.0e3f, cy = 1.0e3f, cz = 1.0e3f, M = 0.f;
+                float bxx = 0.f, byy = 0.f, bxy = 0.f, bxz = 0.f, byz = 0.f;
+                if (c < tn1) {
+                    cx = (q0.x - gh.x) + q1.x; cy = (q0.y - gh.y) + q1.y; cz = (q0.z - gh.z) + q1.z; M = q0.w;
+                    bxx = q1.w; byy = q2.x; bxy = q2.y; bxz = q2.z; byz = q2.w;
+                }
+                load_recs();                            // this warp's next tile (its ids arrived a tile ago)
+                load_ids(k + 2 * TC_PRODUCERS);         // and the one after
+                const float bzz = -(bxx + byy);
+                const float bcx = fmaf(bxx, cx, fmaf(bxy, cy, bxz * cz));
+                const float bcy = fmaf(bxy, cx, fmaf(byy, cy, byz * cz));
+                const float bcz = fmaf(bxz, cx, fmaf(byz, cy, bzz * cz));
+                const float cbc = fmaf(cx, bcx, fmaf(cy, bcy, cz * bcz));
+                // stage sg held tile cc - TC_STAGES: its MMA is complete and its (c, M) pairs are consumed, because this warp has already
+                // passed the empty barrier of its previous tile cc - 2, which the consumers signal after tile cc - 2 - TC_BUFS
+                char* rowb = reinterpret_cast<char*>(sm.B[sg]) + (size_t)(c >> 1) * TC_SBO_B + (size_t)(c & 1) * 16;
+                auto st = [&](const int o, const int kc, const float4 v) { *reinterpret_cast<float4*>(rowb + (size_t)o * 32 + (size_t)kc * TC_LBO) = v; };
+                {
+                    // output 0: d.B.d
+                    const float p0[10] = {-2.f * bcx, -2.f * bcy, -2.f * bcz, cbc, bxx, byy, bzz, 2.f * bxy, 2.f * bxz, 2.f * byz};
+                    float ph[10], pl[10];
+#pragma unroll
+                    for (int q = 0; q < 10; ++q) split_tf32(p0[q], ph[q], pl[q]);
+                    st(0, 0, make_float4(ph[0], ph[1], ph[2], ph[3]));
+                    st(0, 1, make_float4(ph[4], ph[5], ph[6], ph[7]));
+                    st(0, 2, make_float4(ph[8], ph[9], ph[0], ph[1]));
+                    st(0, 3, make_float4(ph[2], ph[3], ph[4], ph[5]));
+                    st(0, 4, make_float4(ph[6], ph[7], ph[8], ph[9]));
+                    st(0, 5, make_float4(pl[0], pl[1], pl[2], pl[3]));
+                    st(0, 6, make_float4(pl[4], pl[5], pl[6], pl[7]));
+                    st(0, 7, make_float4(pl[8], pl[9], 0.f, 0.f));
+                    float* cs = reinterpret_cast<float*>(&sm.C[sg][c >> 1][0]) + (c & 1);
+                    cs[0] = cx; cs[2] = cy; cs[4] = cz; cs[6] = M;
+                    // outputs 1..3: (B d)_x, (B d)_y, (B d)_z = phi . [-B row, (Bc)_k, 0 ...]
+                    const float r1[4] = {-bxx, -bxy, -bxz, bcx}, r2[4] = {-bxy, -byy, -byz, bcy}, r3[4] = {-bxz, -byz, -bzz, bcz};
+#pragma unroll
+                    for (int o = 1; o <= 3; ++o) {
+                        const float* r = o == 1 ? r1 : (o == 2 ? r2 : r3);
+                        float rh[4], rl[4];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) split_tf32(r[q], rh[q], rl[q]);
+                        st(o, 0, make_float4(rh[0], rh[1], rh[2], rh[3]));
+                        st(o, 2, make_float4(0.f, 0.f, rh[0], rh[1]));
+                        st(o, 3, make_float4(rh[2], rh[3], 0.f, 0.f));
+                        st(o, 5, make_float4(rl[0], rl[1], rl[2], rl[3]));
+                    }
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                mbar_wait(smem_u32(&sm.empty[b]), ((cc / TC_BUFS) & 1) ^ 1);       // consumers are done with TMEM buffer b (tile cc - TC_BUFS)
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) {
+                    const uint64_t db = db0 + (uint64_t)((uint32_t)sg * (TC_STAGE_BYTES >> 4));
+#pragma unroll
+                    for (int ks = 0; ks < TC_K / 8; ++ks) {
+                        const uint32_t accf = ks > 0;
+                        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                                     :: "r"(tmem + (uint32_t)b * TC_N), "l"(da0 + (uint64_t)(ks * ((2 * TC_LBO) >> 4))), "l"(db + (uint64_t)(ks * ((2 * TC_LBO) >> 4))), "r"(idesc), "r"(accf) : "memory");
+                    }
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&sm.full[b])) : "memory");
+                }
+                __syncwarp();
+            }
+            ctr += (uint32_t)nt;
+        } else {
+            // ================= consumers =================
+            const float nx = -x, ny = -y, nz = -z;
+            Acc64 acc = {0, 0, 0, 0, 0};
+            Acc2 p = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+            const int set = w >> 2;
+            const uint32_t tl = tmem + ((uint32_t)((w & 3) * 32) << 16);
+            for (int k = 0; k < nt; ++k, ++ctr) {
+                const int b = ctr & (TC_BUFS - 1), sg = ctr & (TC_STAGES - 1);
+                mbar_wait(smem_u32(&sm.full[b]), (ctr / TC_BUFS) & 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                // software pipeline over the tile's 8 column groups (2 cell pairs each): the next group's tcgen05.ld is in flight
+                // while the current one is evaluated
+                uint32_t va[16], vb[16];
+                float4 ca[4], cb[4];                          // the (c, M) pairs of the same two column groups
+                constexpr int NG = TC_N / 16 / TC_SETS;       // column groups per set and tile
+                const uint32_t tcol = tl + (uint32_t)b * TC_N + (uint32_t)set * (NG * 16);
+                const float4* cp2 = &sm.C[sg][set * NG * 2][0];
+                tc_ld16(va, tcol);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) ca[q] = cp2[q];
+#pragma unroll
+                for (int hh = 0; hh < NG; hh += 2) {
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    tc_ld16(vb, tcol + (hh + 1) * 16);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) cb[q] = cp2[(hh + 1) * 4 + q];
+                    tc_pairs(p, va, ca, nx, ny, nz);
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    if (hh + 2 < NG) {
+                        tc_ld16(va, tcol + (hh + 2) * 16);
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) ca[q] = cp2[(hh + 2) * 4 + q];
+                    }
+                    tc_pairs(p, vb, cb, nx, ny, nz);
+                }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(&sm.empty[b])) : "memory");
+                // fp32 partial sums of TC_FLUSH tiles (16 / TC_SETS terms per tile and half) into the fp64 accumulators
+                if ((k & (TC_FLUSH - 1)) == TC_FLUSH - 1 || k == nt - 1) {
+                    const float sx = p.ax.x + p.ax.y, sy = p.ay.x + p.ay.y, sz = p.az.x + p.az.y, sp = p.pot.x + p.pot.y;
+                    acc.ax += (double)sx; acc.ay += (double)sy; acc.az += (double)sz; acc.pot += (double)sp;
+                    acc.s += (double)(fabsf(sx) + fabsf(sy) + fabsf(sz));
+                    p.ax = p.ay = p.az = p.pot = make_float2(0.f, 0.f);
+                }
+            }
+            // ---- the precise list: float-float displacements, CUDA cores, one particle per thread ----
+            {
+                const int n_spp = sr->n_spp;
+                int chunk = n_spp > 0 ? sr->head_spp : -1, remaining = n_spp;
+                float4 (*pt)[32] = sm.P[w];          // aliases A: every MMA of this unit is complete (the last full barrier has been passed)
+                while (chunk >= 0 && remaining > 0) {
+                    const int* cp = arena + (size_t)chunk * PETAR_CHUNK;
+                    const int ne = min(remaining, PETAR_CHUNK_PAYLOAD);
+                    for (int e0 = 32 * set; e0 < ne; e0 += 32 * TC_SETS) {
+                        const int nb = min(32, ne - e0);
+                        __syncwarp();
+                        if (lane < nb) { const NodeSp* sp = &nsp[cp[PETAR_CHUNK_HDR + e0 + lane]]; pt[0][lane] = sp->q0; pt[1][lane] = sp->q1; pt[2][lane] = sp->q2; }
+                        __syncwarp();
+                        Acc32 q = {0.f, 0.f, 0.f, 0.f};
+                        for (int j = 0; j < nb; ++j) {
+                            const float4 a = pt[0][j], b4 = pt[1][j], c4 = pt[2][j];
+                            cell_term<true>(q, (a.x - ia.x) + (b4.x - ib.x), (a.y - ia.y) + (b4.y - ib.y), (a.z - ia.z) + (b4.z - ib.z), a.w,
+                                            b4.w, c4.x, -(b4.w + c4.x), c4.y, c4.z, c4.w);
+                        }
+                        flush(q, acc);
+                    }
+                    remaining -= ne;
+                    chunk = cp[0];
+                }
+            }
+            // the sets' sums of a particle meet in set 0 (fixed order); bar 1 = the consumers only
+            asm volatile("bar.sync 1, %0;" :: "n"(TC_CONSUMERS) : "memory");        // every P tile consumed (R aliases P)
+#pragma unroll 1
+            for (int hs = 1; hs < TC_SETS; ++hs) {
+                if (set == hs) { double* r = sm.R[ti]; r[0] = acc.ax; r[1] = acc.ay; r[2] = acc.az; r[3] = acc.pot; r[4] = acc.s; }
+                asm volatile("bar.sync 1, %0;" :: "n"(TC_CONSUMERS) : "memory");
+                if (set == 0) { const double* r = sm.R[ti]; acc.ax += r[0]; acc.ay += r[1]; acc.az += r[2]; acc.pot += r[3]; acc.s += r[4]; }
+                if (hs + 1 < TC_SETS) asm volatile("bar.sync 1, %0;" :: "n"(TC_CONSUMERS) : "memory");
+            }
+            if (set == 0 && ti < cnt) {
+                double* o = part + ((size_t)fu.level * n_part + fu.ibeg + ti) * 4;
+                o[0] = acc.ax; o[1] = acc.ay; o[2] = acc.az; o[3] = acc.pot;
+                part_s[(size_t)fu.level * n_part + fu.ibeg + ti] = acc.s;
+            }
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (w == TC_CONSUMERS / 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "n"(TC_BUFS * TC_N));
+}
+
 // unit table: every super-group is cut into units of 128 particles, then at most one each of 64, 32 and < 32;
 // units are stored by size class (largest first) so the ticket order ends with the small ones
 template <class F>
 __device__ __forceinline__ void for_units(const int begin, const int n, F f) {
     int b = begin, r = n;
     while (r >= UNIT_MAX) { f(0, b, UNIT_MAX); b += UNIT_MAX; r -= UNIT_MAX; }
+    if (r >= TC_UNIT_MIN) { f(0, b, r); return; }           // class 0: 80..128 particles (k_force_units_tc; k_force_units for monopole-only runs)
 #pragma unroll
     for (int c = 1; c < PETAR_UNIT_CLASSES - 1; ++c) {
         const int sz = UNIT_MAX >> c;
@@ -953,7 +1304,7 @@ __global__ void __launch_bounds__(256) k_units_fill(DevHeader* __restrict__ h, c
 }
 
 __global__ void k_reset_ticket2(DevHeader* h) {
-    if (threadIdx.x == 0) { h->group_ticket2 = 0; h->group_ticket4 = 0; h->unit_ticket = 0; h->n_refine = 0; for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) h->unit_cnt[k] = 0; }
+    if (threadIdx.x == 0) { h->group_ticket2 = 0; h->group_ticket4 = 0; h->unit_ticket = 0; h->unit_ticket_tc = 0; h->n_refine = 0; for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) h->unit_cnt[k] = 0; }
 }
 
 // phase A: unit table, then the super-groups' common cells.  ctas_per_sm > 0 limits the grid (tuning
@@ -973,13 +1324,31 @@ cudaError_t launch_force_units(petar_tree* t, cudaStream_t s, int ctas_per_sm) {
     KCHECK(s, "k_units_fill");
     int per_sm = 0;
     cudaError_t e;
+    if (quad) {
+        // units of 80..128 particles: quadrupole contraction on the tensor cores
+        // (the occupancy query reports 1 CTA per SM for a kernel that allocates tensor memory; registers, shared memory and the
+        // 512 TMEM columns allow TC_MIN_CTAS, and persistent CTAs that find no ticket left simply exit)
+        per_sm = TC_MIN_CTAS;
+        if (ctas_per_sm > 0 && ctas_per_sm < per_sm) per_sm = ctas_per_sm;
+        static bool tc_attr = false;
+        if (!tc_attr) {
+            // the same (maximal) shared-memory carve-out for every kernel that runs beside another one: an SM only changes its carve-out when idle
+            e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TcSmem)); if (e != cudaSuccess) return e;
+            e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
+            e = cudaFuncSetAttribute(k_force_units<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
+            tc_attr = true;
+        }
+        k_force_units_tc<<<t->sm_count * per_sm, TC_THREADS, sizeof(TcSmem), s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N);
+        KCHECK(s, "k_force_units_tc");
+        petar_count_launch(1);
+    }
     if (quad) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force_units<true>, UW * 32, 0);
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force_units<false>, UW * 32, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     if (ctas_per_sm > 0 && ctas_per_sm < per_sm) per_sm = ctas_per_sm;
-    if (quad) k_force_units<true><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N);
-    else k_force_units<false><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N);
+    if (quad) k_force_units<true><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N, 1);
+    else k_force_units<false><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N, 0);
     KCHECK(s, "k_force_units");
     petar_count_launch(5);
     stage_end(t, PETAR_STAGE_FORCE_UNITS, s);

@@ -15,7 +15,7 @@
 #define PETAR_SUP_T0 4096
 #define PETAR_SUP_T1 512
 #define PETAR_SUP_LIMIT(l) ((l) == 0 ? PETAR_SUP_T0 : PETAR_SUP_T1)
-#define PETAR_UNIT_CLASSES 4       // phase-A force units of 128, 64, 32 and < 32 particles
+#define PETAR_UNIT_CLASSES 4       // phase-A force units: class 0 = 80..128 particles (tensor-core kernel), then 64, 32 and < 32
 
 // ---- device-resident header (one per tree, lives at the start of the workspace) -----------------
 struct DevHeader {
@@ -39,6 +39,7 @@ struct DevHeader {
     int unit_off[PETAR_UNIT_CLASSES + 1];
     int unit_fill[PETAR_UNIT_CLASSES];
     int unit_ticket;
+    int unit_ticket_tc;            // k_force_units_tc (class-0 units)
     int n_refine;                  // particles queued for the fp64 re-evaluation (k_force_refine)
     int group_ticket4;             // k_force_near
     unsigned long long n_epep, n_epsp, n_epep_near, n_ep_list, n_sp_list, n_epsp_common;
