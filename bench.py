@@ -34,7 +34,7 @@ sys.path.insert(0, ROOT)
 FLOP_NEWTON, FLOP_CUT, FLOP_QUAD = 20, 49, 53      # fixed flops-per-interaction convention
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the force kernels, from the committed `ncu --set full` capture of
 # THIS round's build at config 3 (profiles/ncu_r02_force.md).  Emitted only for that configuration; any other run reports null.
-TRAFFIC_NCU = {"capture": "profiles/ncu_r02_force.md", "config": 3, "k_force_units": 207.0e6, "k_force": 1230.7e6}
+TRAFFIC_NCU = {"capture": "profiles/ncu_r02_force.md", "config": 3, "k_force_units_tc": 132.8e6, "k_force_units": 132.8e6, "k_force": 1231.3e6}
 
 
 def parse():
@@ -220,7 +220,7 @@ def main():
     n_inter = counts.n_epep + counts.n_epsp
     quad = params.multipole >= 2
     flop_sp = FLOP_QUAD if quad else FLOP_NEWTON
-    flops_units = flop_sp * counts.n_epsp_common                      # phase A: k_force_units (super-group-wide cells)
+    flops_units = flop_sp * counts.n_epsp_common                      # phase A: k_force_units_tc + k_force_units (super-group-wide cells)
     flops_groups = (FLOP_CUT * counts.n_epep_near + FLOP_NEWTON * (counts.n_epep - counts.n_epep_near)
                     + flop_sp * (counts.n_epsp - counts.n_epsp_common))  # phase B: k_force (the groups' own lists)
     flops_step = flops_units + flops_groups
@@ -473,7 +473,9 @@ def main():
         if ms_st > 0.0:
             gbs = bpp * N / (ms_st * 1e-3) / 1e9
             hbm_stages[name] = dict(ms=ms_st, bytes_per_particle=bpp, achieved_gbs=gbs, frac_of_hbm=gbs / hbm_peak)
-    kern = [dict(kernel="k_force_units", ms=stage_ms["force_units"], flops_per_launch=float(flops_units)),
+    # stage force_units = the unit table, k_force_units_tc (units of 80..128 particles: quadrupole contraction on the tensor cores) and
+    # k_force_units (smaller units, CUDA cores only); the 53 flops per quadrupole interaction are counted wherever they are executed
+    kern = [dict(kernel="k_force_units_tc" if quad else "k_force_units", ms=stage_ms["force_units"], flops_per_launch=float(flops_units)),
             dict(kernel="k_force", ms=stage_ms["force"], flops_per_launch=float(flops_groups))]
     kern[0]["ms_alone"], kern[1]["ms_alone"] = stage_seq["force_units"], stage_seq["force"]
     for kd in kern:
