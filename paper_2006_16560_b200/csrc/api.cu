@@ -120,6 +120,7 @@ static void free_handle(petar_tree* t) {
     if (t->ev) { for (int k = 0; k < 2 * PETAR_N_STAGES; ++k) if (t->ev[k]) cudaEventDestroy(t->ev[k]); delete[] t->ev; }
     if (t->ev_fork) cudaEventDestroy(t->ev_fork);
     if (t->ev_join) cudaEventDestroy(t->ev_join);
+    if (t->ev_tab) cudaEventDestroy(t->ev_tab);
     if (t->side) cudaStreamDestroy(t->side);
     t->magic = 0;
     delete t;
@@ -141,6 +142,7 @@ static int build_into(petar_tree* t, const double* x, const double* y, const dou
         CK(cudaStreamCreateWithFlags(&t->side, cudaStreamNonBlocking));
         CK(cudaEventCreateWithFlags(&t->ev_fork, cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&t->ev_join, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&t->ev_tab, cudaEventDisableTiming));
     }
     if (t->N > 0) {
         CK(launch_keys_sort_gather(t, s));
@@ -183,7 +185,6 @@ extern "C" int petar_tree_rebuild(petar_tree* t, const double* x, const double* 
 }
 
 #define OVERLAP_WALK_CTAS 2      // CTAs per SM of k_walk / k_force_units while the two run side by side
-#define OVERLAP_UNITS_CTAS 0      // 0 = no limit: the walk CTA is resident first, two unit CTAs fit beside it, the third follows when it leaves
 static int check_tree(petar_tree* t) { return (t && t->magic == PETAR_MAGIC && t->built) ? PETAR_OK : PETAR_ENOTBUILT; }
 
 static int ensure_walk(petar_tree* t, cudaStream_t s) {
@@ -212,10 +213,16 @@ extern "C" int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_
         CK(launch_walk_supers(t, s));
         CK(cudaEventRecord(t->ev_fork, s));
         CK(cudaStreamWaitEvent(t->side, t->ev_fork, 0));
-        CK(launch_walk_groups(t, t->side, OVERLAP_WALK_CTAS));
+        CK(launch_walk_groups(t, t->side, OVERLAP_WALK_CTAS));      // launched first: its CTAs take their place on the SMs before the unit kernels'
+        CK(launch_force_units_table(t, s));
+        CK(cudaEventRecord(t->ev_tab, s));
+        CK(launch_force_units_tc(t, s));
+        CK(cudaStreamWaitEvent(t->side, t->ev_tab, 0));
+        CK(launch_force_units_small(t, t->side));          // the small units and the changeover pairs follow the walk on the side stream,
+        CK(launch_force_near(t, t->side));                 // beside the tail of the tensor-core kernel
         CK(cudaEventRecord(t->ev_join, t->side));
-        CK(launch_force_units(t, s, OVERLAP_UNITS_CTAS));
         CK(cudaStreamWaitEvent(s, t->ev_join, 0));
+        stage_end(t, PETAR_STAGE_FORCE_UNITS, s);
         t->walked = true;
         CK(launch_force_groups(t, acc_x, acc_y, acc_z, pot, s));
     } else {

@@ -1307,14 +1307,12 @@ __global__ void k_reset_ticket2(DevHeader* h) {
     if (threadIdx.x == 0) { h->group_ticket2 = 0; h->group_ticket4 = 0; h->unit_ticket = 0; h->unit_ticket_tc = 0; h->n_refine = 0; for (int k = 0; k < PETAR_UNIT_CLASSES; ++k) h->unit_cnt[k] = 0; }
 }
 
-// phase A: unit table, then the super-groups' common cells.  ctas_per_sm > 0 limits the grid (tuning
-// experiments).  Needs the super-group walks only.
-cudaError_t launch_force_units(petar_tree* t, cudaStream_t s, int ctas_per_sm) {
+// phase A, part 1: the unit table (needs the super-group walks only)
+cudaError_t launch_force_units_table(petar_tree* t, cudaStream_t s) {
     Workspace& w = t->w;
     stage_begin(t, PETAR_STAGE_FORCE_UNITS, s);
     k_reset_ticket2<<<1, 32, 0, s>>>(w.hdr);
     KCHECK(s, "k_reset_ticket2");
-    const bool quad = t->p.multipole >= 2;
     const int nrec_blocks = cdiv(w.group_cap, 256);
     k_units_count<<<nrec_blocks, 256, 0, s>>>(w.hdr, w.srec, w.group_cap);
     KCHECK(s, "k_units_count");
@@ -1322,42 +1320,56 @@ cudaError_t launch_force_units(petar_tree* t, cudaStream_t s, int ctas_per_sm) {
     KCHECK(s, "k_units_offsets");
     k_units_fill<<<nrec_blocks, 256, 0, s>>>(w.hdr, w.srec, w.group_cap, w.units);
     KCHECK(s, "k_units_fill");
+    petar_count_launch(4);
+    return cudaGetLastError();
+}
+// phase A, part 2: units of 80..128 particles, quadrupole contraction on the tensor cores (nothing to do for monopole-only runs)
+cudaError_t launch_force_units_tc(petar_tree* t, cudaStream_t s) {
+    Workspace& w = t->w;
+    if (t->p.multipole < 2) return cudaSuccess;
+    cudaError_t e;
+    static bool tc_attr = false;
+    if (!tc_attr) {
+        // the same (maximal) shared-memory carve-out for every kernel that runs beside another one: an SM only changes its carve-out when idle
+        e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TcSmem)); if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_force_units<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
+        tc_attr = true;
+    }
+    // (the occupancy query reports 1 CTA per SM for a kernel that allocates tensor memory; registers, shared memory and the
+    // 512 TMEM columns allow TC_MIN_CTAS, and persistent CTAs that find no ticket left simply exit)
+    k_force_units_tc<<<t->sm_count * TC_MIN_CTAS, TC_THREADS, sizeof(TcSmem), s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N);
+    KCHECK(s, "k_force_units_tc");
+    petar_count_launch(1);
+    return cudaGetLastError();
+}
+// phase A, part 3: the remaining units (all of them for monopole-only runs) on the CUDA cores
+cudaError_t launch_force_units_small(petar_tree* t, cudaStream_t s) {
+    Workspace& w = t->w;
+    const bool quad = t->p.multipole >= 2;
     int per_sm = 0;
     cudaError_t e;
-    if (quad) {
-        // units of 80..128 particles: quadrupole contraction on the tensor cores
-        // (the occupancy query reports 1 CTA per SM for a kernel that allocates tensor memory; registers, shared memory and the
-        // 512 TMEM columns allow TC_MIN_CTAS, and persistent CTAs that find no ticket left simply exit)
-        per_sm = TC_MIN_CTAS;
-        if (ctas_per_sm > 0 && ctas_per_sm < per_sm) per_sm = ctas_per_sm;
-        static bool tc_attr = false;
-        if (!tc_attr) {
-            // the same (maximal) shared-memory carve-out for every kernel that runs beside another one: an SM only changes its carve-out when idle
-            e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TcSmem)); if (e != cudaSuccess) return e;
-            e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
-            e = cudaFuncSetAttribute(k_force_units<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
-            tc_attr = true;
-        }
-        k_force_units_tc<<<t->sm_count * per_sm, TC_THREADS, sizeof(TcSmem), s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N);
-        KCHECK(s, "k_force_units_tc");
-        petar_count_launch(1);
-    }
     if (quad) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force_units<true>, UW * 32, 0);
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force_units<false>, UW * 32, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
-    if (ctas_per_sm > 0 && ctas_per_sm < per_sm) per_sm = ctas_per_sm;
     if (quad) k_force_units<true><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N, 1);
     else k_force_units<false><<<t->sm_count * per_sm, UW * 32, 0, s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N, 0);
     KCHECK(s, "k_force_units");
-    petar_count_launch(5);
-    stage_end(t, PETAR_STAGE_FORCE_UNITS, s);
+    petar_count_launch(1);
     return cudaGetLastError();
+}
+// phase A on one stream
+cudaError_t launch_force_units(petar_tree* t, cudaStream_t s) {
+    cudaError_t e = launch_force_units_table(t, s);
+    if (e == cudaSuccess) e = launch_force_units_tc(t, s);
+    if (e == cudaSuccess) e = launch_force_units_small(t, s);
+    stage_end(t, PETAR_STAGE_FORCE_UNITS, s);
+    return e;
 }
 
 // phase B: the groups' own lists (needs the per-group walk and phase A)
-cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s) {
-    Workspace& w = t->w;
+static ForceConst force_const(const petar_tree* t) {
     const double rho = t->p.r_in_over_r_out;
     const double lam = (1.0 - rho) / (1.0 + rho);
     ForceConst fc;
@@ -1369,11 +1381,22 @@ cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* a
     fc.b3 = (float)(120.0 * lam - 20.0 * (1.0 - lam));
     fc.b4 = (float)(-35.0 * lam);
     fc.a4 = (float)(35.0 * lam);
+    return fc;
+}
+// the changeover pairs of every group (needs the per-group walk only; its sums are added by k_force)
+cudaError_t launch_force_near(petar_tree* t, cudaStream_t s) {
+    Workspace& w = t->w;
+    k_force_near<<<t->sm_count * 8, NEAR_WARPS * 32, 0, s>>>(w.hdr, w.grp, w.arena, w.pa, w.pb, w.part + (size_t)PETAR_NSUP * t->N * 4,
+                                                               w.part_s + (size_t)PETAR_NSUP * t->N, force_const(t));
+    KCHECK(s, "k_force_near");
+    petar_count_launch(1);
+    return cudaGetLastError();
+}
+cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s) {
+    Workspace& w = t->w;
+    const ForceConst fc = force_const(t);
     const bool quad = t->p.multipole >= 2;
     stage_begin(t, PETAR_STAGE_FORCE, s);
-    k_force_near<<<t->sm_count * 8, NEAR_WARPS * 32, 0, s>>>(w.hdr, w.grp, w.arena, w.pa, w.pb, w.part + (size_t)PETAR_NSUP * t->N * 4,
-                                                               w.part_s + (size_t)PETAR_NSUP * t->N, fc);
-    KCHECK(s, "k_force_near");
     int per_sm = 0;
     cudaError_t e;
     if (quad) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_force<true>, FT, 0);
@@ -1393,13 +1416,14 @@ cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* a
         k_force_refine<<<t->sm_count, REFINE_THREADS, 0, s>>>(w.hdr, A);
         KCHECK(s, "k_force_refine");
     }
-    petar_count_launch(3);
+    petar_count_launch(2);
     stage_end(t, PETAR_STAGE_FORCE, s);
     return cudaGetLastError();
 }
 
 cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s) {
-    cudaError_t e = launch_force_units(t, s, 0);
+    cudaError_t e = launch_force_units(t, s);
+    if (e == cudaSuccess) e = launch_force_near(t, s);
     if (e != cudaSuccess) return e;
     return launch_force_groups(t, ax, ay, az, pot, s);
 }

@@ -136,7 +136,7 @@ struct petar_tree {
     int sm_count;
     int h_nodes, h_groups;         // host copies of the header counters (filled by petar_debug_export)
     cudaStream_t side;             // second stream: the per-group walk runs beside force phase A (created once per handle)
-    cudaEvent_t ev_fork, ev_join;
+    cudaEvent_t ev_fork, ev_join, ev_tab;
     void* workspace; size_t workspace_bytes;
 };
 
@@ -149,7 +149,11 @@ cudaError_t launch_walk(petar_tree* t, cudaStream_t s);
 cudaError_t launch_walk_supers(petar_tree* t, cudaStream_t s);
 cudaError_t launch_walk_groups(petar_tree* t, cudaStream_t s, int ctas_per_sm);
 cudaError_t launch_force(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s);
-cudaError_t launch_force_units(petar_tree* t, cudaStream_t s, int ctas_per_sm);
+cudaError_t launch_force_units(petar_tree* t, cudaStream_t s);
+cudaError_t launch_force_units_table(petar_tree* t, cudaStream_t s);
+cudaError_t launch_force_units_tc(petar_tree* t, cudaStream_t s);
+cudaError_t launch_force_units_small(petar_tree* t, cudaStream_t s);
+cudaError_t launch_force_near(petar_tree* t, cudaStream_t s);
 cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* az, double* pot, cudaStream_t s);
 // vx != nullptr: the orbit-dependent two-stage criterion (rule O10) with velocities in the caller's order
 cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, int64_t capacity,
