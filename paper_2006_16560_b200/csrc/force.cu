@@ -33,7 +33,7 @@
 #define SP_REC 2               // staged cells per thread per tile
 #define SP_TILE (SP_REC * FT)  // cells per staged tile
 #define FORCE_MIN_CTAS 4
-#define FORCE_UNROLL 2
+#define FORCE_UNROLL 4
 #define PRAGMA_STR_(x) _Pragma(#x)
 #define PRAGMA_(x) PRAGMA_STR_(x)
 #define UNROLL_J PRAGMA_(unroll FORCE_UNROLL)
