@@ -442,7 +442,8 @@ def main():
     for mode, name, iters in ((1, "ffma_3_distinct_registers", 400000), (2, "quadrupole_cell_term_loop_scalar", 2000),
                               (3, "quadrupole_cell_term_loop_packed", 2000), (4, "pattern_ffma_3_registers_independent", 200000),
                               (5, "pattern_ffma_2_registers", 200000), (6, "pattern_ffma_shared_operand", 200000),
-                              (7, "pattern_ffma3_plus_fadd", 200000)):
+                              (7, "pattern_ffma3_plus_fadd", 200000), (8, "tc_consumer_loop_alone", 20000),
+                              (9, "tc_consumer_loop_beside_mma", 20000)):
         P.petar_probe_fp32_mode(mode, max(1, iters // 50), scratch, stream)
         torch.cuda.synchronize()
         a.record(stream); fl = P.petar_probe_fp32_mode(mode, iters, scratch, stream); b.record(stream); b.synchronize()

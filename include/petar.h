@@ -313,7 +313,11 @@ int petar_probe_fp32(int64_t iters, double* flops_out_host, float* scratch_dev, 
  *   modes 4-7: FFMA operand patterns behind profiles/fp32_issue_model_r02.md -- 4: a = b*c + a (three distinct
  *           registers), 5: a = b*b + a (two), 6: a = b*e + a; c = d*e + c (one operand shared by all), 7: a = b*c + d;
  *           d = a + e.  *flops_out_host = 2 x thread-level instructions, so value / time / (nominal FP32 peak) is
- *           warp instructions per clock and sub-partition.
+ *           warp instructions per clock and sub-partition;
+ *   modes 8, 9: the consumer loop of the tensor-core phase-A kernel (k_force_units_tc: tcgen05.ld of d.B.d and B d, 21 packed
+ *           FP32 + 2 MUFU per cell pair) on static operands, iters = 32-cell tiles per CTA, 53 flops per interaction --
+ *           8: alone, 9: with the kernel's MMAs (4 x 128x128x8 tf32 per tile) issued beside it through the kernel's
+ *           full / empty mbarrier handshake.  Their difference is the cost of the tensor-core work to the CUDA-core loop.
  * Errors: PETAR_EINVAL (mode), PETAR_ECUDA.                                                          */
 int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream);
 

@@ -1547,9 +1547,110 @@ __global__ void __launch_bounds__(128) k_probe_pattern(float* __restrict__ out, 
     if (s == 123.456f) out[0] = s;
 }
 
+// modes 8, 9: the consumer loop of k_force_units_tc (tcgen05.ld of the four numbers per cell, broadcast (c, M) pairs from shared
+// memory, 21 packed FP32 + 2 MUFU per cell pair) on static operands, 2 CTAs of 4 consumer warps per SM.  Mode 8: nothing else runs;
+// mode 9: a fifth warp issues the kernel's MMAs (4 x 128x128x8 tf32 per 32-cell tile) into the other TMEM buffer, with the
+// kernel's full / empty mbarrier handshake -- the difference is what the tensor-core work beside the CUDA-core loop costs.
+template <bool MMA>
+__global__ void __launch_bounds__(160, 3) k_probe_tc(float* __restrict__ out, long long iters) {
+    __shared__ __align__(128) float sA[128 * TC_K];
+    __shared__ __align__(128) float sB[TC_STAGE_BYTES / 4];
+    __shared__ __align__(16) float4 sC[2][TC_CELLS / 2][2];
+    __shared__ __align__(8) unsigned long long full[2], empty[2];
+    __shared__ uint32_t tmem_base;
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    for (int e = t; e < 128 * TC_K; e += 160) sA[e] = 1e-3f * (float)(e & 63);
+    for (int e = t; e < TC_STAGE_BYTES / 4; e += 160) sB[e] = 2e-3f * (float)(e & 31);
+    if (t < 2 * TC_CELLS) reinterpret_cast<float4*>(sC)[t] = make_float4(10.f + t, 10.5f + t, 20.f - t, 20.5f - t);
+    if (t == 0) {
+        for (int q = 0; q < 2; ++q) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&full[q])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 4;" :: "r"(smem_u32(&empty[q])));
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;");
+    }
+    if (w == 4) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base)), "n"(2 * TC_N));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem = tmem_base;
+    if (w == 4) {
+        if (MMA) {
+            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+            const uint64_t da0 = tc_desc(smem_u32(sA), TC_SBO), db0 = tc_desc(smem_u32(sB), TC_SBO_B);
+            for (long long k = 0; k < iters; ++k) {
+                const int b = (int)(k & 1);
+                mbar_wait(smem_u32(&empty[b]), (uint32_t)(((k >> 1) & 1) ^ 1));
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                if (lane == 0) {
+#pragma unroll
+                    for (int ks = 0; ks < TC_K / 8; ++ks) {
+                        const uint32_t accf = ks > 0;
+                        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                                     :: "r"(tmem + (uint32_t)b * TC_N), "l"(da0 + (uint64_t)(ks * ((2 * TC_LBO) >> 4))), "l"(db0 + (uint64_t)(ks * ((2 * TC_LBO) >> 4))), "r"(idesc), "r"(accf) : "memory");
+                    }
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&full[b])) : "memory");
+                }
+                __syncwarp();
+            }
+        }
+    } else {
+        const uint32_t tl = tmem + ((uint32_t)(w * 32) << 16);
+        if (!MMA) {         // some finite numbers in tensor memory
+            for (int c = 0; c < 2 * TC_N; c += 4) {
+                const uint32_t a = __float_as_uint(1e-3f * (float)(t + c)), b = __float_as_uint(-2e-3f * (float)(c + 1));
+                asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" :: "r"(tl + c), "r"(a), "r"(b), "r"(a), "r"(b));
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;");
+        }
+        const float nx = -(t * 0.01f + out[0]), ny = -(t * 0.02f), nz = -(0.5f + out[0]);
+        Acc2 p = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        for (long long k = 0; k < iters; ++k) {
+            const int b = (int)(k & 1);
+            if (MMA) { mbar_wait(smem_u32(&full[b]), (uint32_t)((k >> 1) & 1)); asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+            uint32_t va[16], vb[16];
+            float4 ca[4], cb[4];
+            const uint32_t tcol = tl + (uint32_t)b * TC_N;
+            const float4* cp2 = &sC[b][0][0];
+            tc_ld16(va, tcol);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) ca[q] = cp2[q];
+#pragma unroll
+            for (int hh = 0; hh < TC_N / 16; hh += 2) {
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                tc_ld16(vb, tcol + (hh + 1) * 16);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) cb[q] = cp2[(hh + 1) * 4 + q];
+                tc_pairs(p, va, ca, nx, ny, nz);
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                if (hh + 2 < TC_N / 16) {
+                    tc_ld16(va, tcol + (hh + 2) * 16);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) ca[q] = cp2[(hh + 2) * 4 + q];
+                }
+                tc_pairs(p, vb, cb, nx, ny, nz);
+            }
+            if (MMA) {
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(&empty[b])) : "memory");
+            }
+        }
+        const float s = p.ax.x + p.ay.x + p.az.x + p.pot.x + p.ax.y + p.ay.y + p.az.y + p.pot.y;
+        if (s == 123.456f) out[0] = s;
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (w == 4) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "n"(2 * TC_N));
+}
+
 extern "C" int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream) {
     if (mode == 0) return petar_probe_fp32(iters, flops_out_host, scratch_dev, cuda_stream);
-    if (mode < 1 || mode > 7) return PETAR_EINVAL;
+    if (mode < 1 || mode > 9) return PETAR_EINVAL;
     int dev = 0, sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return PETAR_ECUDA;
     if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PETAR_ECUDA;
@@ -1558,6 +1659,11 @@ extern "C" int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_
         const int grid = sm * 8;
         k_probe_ffma3<<<grid, 256, 0, s>>>(scratch_dev, (long long)iters);
         if (flops_out_host) *flops_out_host = 2.0 * 16.0 * (double)iters * 256.0 * (double)grid;
+    } else if (mode == 8 || mode == 9) {
+        const int grid = sm * 2;
+        if (mode == 8) k_probe_tc<false><<<grid, 160, 0, s>>>(scratch_dev, (long long)iters);
+        else k_probe_tc<true><<<grid, 160, 0, s>>>(scratch_dev, (long long)iters);
+        if (flops_out_host) *flops_out_host = 53.0 * (double)TC_CELLS * 128.0 * (double)iters * (double)grid;
     } else if (mode == 2 || mode == 3) {
         const int grid = sm * 4;
         if (mode == 2) k_probe_cell<<<grid, 128, 0, s>>>(scratch_dev, (long long)iters);
