@@ -4,7 +4,8 @@
 #include "internal.cuh"
 
 #define WALK_WARPS 8
-#define WALK_STACK 1504          // frontier entries per warp (shared memory)
+#define WALK_STACK 1504          // frontier entries per warp (shared memory) of the super-group walks
+#define GWALK_STACK 640          // ... of the per-group walk (it starts from short deferred lists; 20 KB per CTA let two of its CTAs share an SM with two CTAs of k_force_units_tc)
 
 // warp-uniform cursor of one chunked list
 struct ListCursor {
@@ -244,12 +245,12 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) k_walk_super(DevHeader* __res
 
          // > 7 * 21: room for a pure depth-first descent from any state
 #define WALK_MIN_CTAS 3
-__global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
+__global__ void __maxnreg__(56) k_walk(DevHeader* __restrict__ h, const NodeW* __restrict__ nw,
                                                           const NodeMac* __restrict__ nmac, GroupRec* __restrict__ grp,
                                                           const SuperRec* __restrict__ srec, const int* __restrict__ smap,
                                                           int* __restrict__ arena, int arena_chunks, double theta, int node_cap,
                                                           long long n_part, int group_cap) {
-    __shared__ int s_stack[WALK_WARPS][WALK_STACK];
+    __shared__ int s_stack[WALK_WARPS][GWALK_STACK];
     __shared__ float s_lt[PETAR_NLEVELS];          // edge(level) / theta  (inf when theta == 0: nothing is ever "far")
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     int* stack = s_stack[w];
@@ -303,7 +304,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
             // pop up to 32 nodes; throttle towards depth-first order when the frontier nears its capacity
             // (a pure depth-first descent adds at most 7 entries per level, < WALK_RESERVE in total)
             p = min(32, top);
-            if (top + 7 * p > WALK_STACK - WALK_RESERVE) p = max(1, min(p, (WALK_STACK - WALK_RESERVE - top) / 7));
+            if (top + 7 * p > GWALK_STACK - WALK_RESERVE) p = max(1, min(p, (GWALK_STACK - WALK_RESERVE - top) / 7));
             if (lane < p) node = stack[top - p + lane];
             top -= p;
             __syncwarp();
@@ -353,7 +354,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MIN_CTAS) k_walk(DevHead
                 if (lane >= o) pref += a;
             }
             const int total_push = __shfl_sync(0xffffffffu, pref, 31);
-            if (top + total_push > WALK_STACK) {                 // cannot happen (see the throttle above)
+            if (top + total_push > GWALK_STACK) {                 // cannot happen (see the throttle above)
                 if (lane == 0) atomicOr(&h->status, PETAR_ST_STACK);
                 top = 0;
                 break;
