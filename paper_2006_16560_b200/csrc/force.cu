@@ -1,23 +1,30 @@
 // force.cu -- step S8: fp32 pairwise force + potential over the walk's lists (rule O8), with the
 // changeover weights 1-K (Eq. 17) and 1-W (Eq. 15) on near EP pairs.
 //
-// Two kernels:
-//   PHASE A, k_force_units: the cells COMMON to a super-group (accepted once for all of its i-groups by
-//     k_walk_super) against all of its particles, in units of 128 / 64 / 32 / < 32 particles, four
-//     i-particles per lane, warps that stage their own tiles without CTA barriers; sums go to `part`.
-//   PHASE B, k_force: one CTA (128 threads) per i-group for the group's OWN cells and particles, groups
+// Kernels:
+//   PHASE A: the cells COMMON to a super-group (accepted once for all of its i-groups by k_walk_super) against all of its
+//     particles; sums go to `part`.
+//     k_force_units_tc: units of 80..128 particles.  The quadrupole part of the cell term (d.B.d and B d) is a GEMM per
+//       32-cell tile on the tensor cores (tcgen05.mma kind::tf32, 3xTF32 split operands, accumulators in tensor memory);
+//       producer warps build the operands, consumer warps (thread = particle = TMEM lane) do r^2, 1/r, the monopole and the
+//       accumulation with packed fp32x2 instructions, two cells per instruction.
+//     k_force_units: the smaller units (and everything for monopole-only runs), packed fp32x2 on the CUDA cores, four
+//       i-particles per lane, warps that stage their own tiles without CTA barriers.
+//   PHASE B, k_force: one CTA (128 threads) per i-group for the group's OWN cells and far particles, groups
 //     pulled from a device ticket (persistent CTAs).  Thread mapping: the group's n_i particles are taken
 //     two per thread ("pair slot" p = t % P, P = ceil(n_i/2)); S = 128 / P slices split every staged
 //     j-tile (slice s handles j = s, s+S, ...), so >= 80 % of the lanes are busy for any n_i in 1..64 and
 //     every shared-memory j-record feeds two interactions.  It adds `part`, scales by G and scatters.
+//     k_force_near: the changeover pairs (weights 1-K, 1-W), one warp per group.  k_force_refine: fp64 re-evaluation of the
+//     particles whose long-range force nearly cancels.
 //
-// The kernels are bound by FP32 instruction issue, more precisely by the register-operand bandwidth of
-// the sub-partition (an FFMA with three distinct register sources issues at 0.61 per clock, the packed
-// fp32x2 forms gain nothing), so the design minimises instructions per interaction:
+// The CUDA-core arithmetic uses the packed fp32x2 instructions (FFMA2 / FMUL2 / FADD2: one instruction = one operation for two
+// i-particles or two cells; their 64-bit operands avoid the even/odd register-bank conflicts that held the scalar stream at
+// 1.22 cycles per instruction, profiles/fp32_issue_model_r02.md).  Instructions per interaction are kept low:
 //   * cells farther from the (super-)group than its own size (the bulk) are evaluated with
 //     GROUP-RELATIVE single floats: the j-record is translated to the box centre once when its tile
-//     is staged, the displacement is then one FADD per axis (33 fp32 instructions + 1 MUFU per
-//     quadrupole interaction);
+//     is staged, the displacement is then one FADD per axis (33 fp32 operations + 1 MUFU per
+//     quadrupole interaction on the CUDA cores, 21 + 1 with the contraction on the tensor cores);
 //   * cells closer than that, and all particles, keep float-float coordinates (hi + lo, relative to
 //     the root-cube centre): displacement (xjh - xih) + (xjl - xil), exact to ~1e-7 of the
 //     separation whatever the distance from the origin (needed for tight binaries in sparse groups).
