@@ -487,3 +487,24 @@ def test_scale_and_translation():
     assert ea.max() < TOL and ep.max() < TOL, (ea.max(), ep.max())
     check_neighbors(t2, T2, wt.N)
     t2.close()
+
+
+def test_quadrupole_correction_precision():
+    """The quadrupole part of the cell term alone (quadrupole run minus monopole run, same lists: the walk does not depend on the
+    multipole order) against the oracle's.  In force phase A this part comes from the tensor cores (tf32 operands split hi + lo,
+    DESIGN.md section 5); a lost split term would show as a relative error of ~2^-11 = 5e-4 of the correction, far below the 1e-5
+    bar on the whole force (the correction is ~1e-3 of it).  Measured: median 3e-5 (the fp32 noise of the difference), p99 4.5e-4."""
+    w = make_workload(2)
+    acc = {}
+    for mult in (1, 2):
+        t = _gpu_tree(w, theta=0.5, multipole=mult)
+        c = t.force(True)
+        assert c.n_epsp_common > 0.3 * c.n_epsp          # the super-group-wide phase carries a good part of the cells
+        acc["g", mult] = np.stack([_np(t.acc_x), _np(t.acc_y), _np(t.acc_z)], 1)
+        o = _ora_tree(w, theta=0.5, multipole=mult).force()
+        acc["o", mult] = np.stack([o[0], o[1], o[2]], 1)
+    cg, co = acc["g", 2] - acc["g", 1], acc["o", 2] - acc["o", 1]
+    rel = np.linalg.norm(cg - co, axis=1) / np.linalg.norm(co, axis=1)
+    print("quadrupole correction: median rel. error %.2e, p99 %.2e" % (np.median(rel), np.percentile(rel, 99)))
+    assert np.median(rel) < 1e-4
+    assert np.percentile(rel, 99) < 2e-3
