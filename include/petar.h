@@ -128,7 +128,8 @@ int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_y, double* 
  * r2 < R_ij^2 with R_ij = max(r_search,i, r_search,j), strict).
  *   offsets    : DEVICE int64[N+1]; always written; offsets[N] = total number of neighbours.
  *   indices    : DEVICE int32[capacity] or NULL.  NULL => only offsets (count + scan) are written;
- *                the caller reads offsets[N], allocates, and calls again (two-phase output).
+ *                the caller reads offsets[N], allocates, and calls again (two-phase output).  The per-particle counts of
+ *                the first call are kept in the workspace until the next (re)build or _orbit call: the second call only scans and fills.
  *   status_dev : DEVICE int32[1] or NULL; set to 0, or 1 if offsets[N] > capacity (then rows that
  *                do not fit are not written).
  * Row order is deterministic but unspecified (compare rows as sets).

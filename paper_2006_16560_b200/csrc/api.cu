@@ -130,7 +130,7 @@ static void free_handle(petar_tree* t) {
 static int build_into(petar_tree* t, const double* x, const double* y, const double* z, const double* m, const double* r_out,
                       const double* r_search, cudaStream_t s) {
     t->x = x; t->y = y; t->z = z; t->m = m; t->r_out = r_out; t->r_search = r_search;
-    t->built = false; t->walked = false;
+    t->built = false; t->walked = false; t->nb_counted = false;
     for (int k = 0; k < PETAR_N_STAGES; ++k) t->stage_rec[k] = 0;
     if (g_profiling && !t->ev) {            // events are created once per handle, never on a rebuild
         t->ev = new (std::nothrow) cudaEvent_t[2 * PETAR_N_STAGES];

@@ -131,6 +131,7 @@ struct petar_tree {
     Workspace w;
     const double *x, *y, *z, *m, *r_out, *r_search;
     bool built, walked;
+    bool nb_counted;               // w.nb_cnt / w.nb_queue hold the count pass of petar_neighbor_list for this tree (the fill call reuses it)
     cudaEvent_t* ev;               // [2*PETAR_N_STAGES] stage begin/end events (profiling only; created once per handle)
     int stage_rec[PETAR_N_STAGES];
     int sm_count;

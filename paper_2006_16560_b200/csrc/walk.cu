@@ -666,14 +666,18 @@ cudaError_t launch_neighbors(petar_tree* t, int64_t* offsets, int32_t* indices, 
         KCHECK(s, "k_gather_vel");
         petar_count_launch(1);
     }
-    cudaError_t e = cudaMemsetAsync(w.nb_queue, 0, 4, s);
-    if (e != cudaSuccess) return e;
-    k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 1);
-    KCHECK(s, "k_reset_ticket");
-    if (orbit) { k_neighbors<false, true><<<grid, 256, 0, s>>>(w.hdr, w.grp, A, w.nb_queue); k_neighbors_big<false, true><<<grid_big, 256, 0, s>>>(w.grp, A, w.nb_queue); }
-    else { k_neighbors<false, false><<<grid, 256, 0, s>>>(w.hdr, w.grp, A, w.nb_queue); k_neighbors_big<false, false><<<grid_big, 256, 0, s>>>(w.grp, A, w.nb_queue); }
-    KCHECK(s, "k_neighbors");
-    petar_count_launch(3);
+    cudaError_t e = cudaSuccess;
+    if (orbit || !t->nb_counted) {          // the count pass (two-phase output: a count call followed by a fill call counts once)
+        e = cudaMemsetAsync(w.nb_queue, 0, 4, s);
+        if (e != cudaSuccess) return e;
+        k_reset_ticket<<<1, 32, 0, s>>>(w.hdr, 1);
+        KCHECK(s, "k_reset_ticket");
+        if (orbit) { k_neighbors<false, true><<<grid, 256, 0, s>>>(w.hdr, w.grp, A, w.nb_queue); k_neighbors_big<false, true><<<grid_big, 256, 0, s>>>(w.grp, A, w.nb_queue); }
+        else { k_neighbors<false, false><<<grid, 256, 0, s>>>(w.hdr, w.grp, A, w.nb_queue); k_neighbors_big<false, false><<<grid_big, 256, 0, s>>>(w.grp, A, w.nb_queue); }
+        KCHECK(s, "k_neighbors");
+        petar_count_launch(3);
+        t->nb_counted = !orbit;
+    }
     e = launch_scan_i32_to_i64(w.nb_cnt, (long long*)offsets, n, (long long*)w.scan_tmp, s);
     if (e != cudaSuccess) return e;
     if (indices) {
