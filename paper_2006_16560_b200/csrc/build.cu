@@ -472,6 +472,7 @@ __global__ void __launch_bounds__(256) k_moments(const DevHeader* __restrict__ h
     const double cx = h->c[0], cy = h->c[1], cz = h->c[2];
     for (int l = PETAR_MAXLEVEL; l >= 0; --l) {
         const int n0 = h->level_off[l], n1 = h->level_off[l + 1], n2 = h->level_off[l + 2];
+        if (n0 == n1) continue;                    // empty level (uniform across the grid): no phase, no grid barrier
         for (long long id = n0 + gtid; id < n1; id += gsz) {
             NodeInt r = nint[id];
             double M = 0, S0 = 0, S1 = 0, S2 = 0, rmax = 0;
