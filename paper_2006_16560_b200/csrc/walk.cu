@@ -365,9 +365,6 @@ __global__ void __maxnreg__(56) k_walk(DevHeader* __restrict__ h, const NodeW* _
             __syncwarp();
             pop();                             // next batch: its loads overlap the output below
             // outputs of the current batch
-            list_append(lsp, act == 0, 1, node_cur, 0, arena, arena_chunks, h, lane);
-            list_append(lspp, act == 4, 1, node_cur, 0, arena, arena_chunks, h, lane);
-            list_append(lepn, act == 1, 2, nb, ne, arena, arena_chunks, h, lane);
             // far leaves: the lanes hold the nodes in frontier order, i.e. siblings in ascending order, so neighbouring lanes often hold
             // leaves whose particle ranges are contiguous; such runs are written as ONE range (EP(g) is a set of particles, rule O7;
             // the force kernel's range expansion gets ~3 x fewer entries)
@@ -378,11 +375,29 @@ __global__ void __maxnreg__(56) k_walk(DevHeader* __restrict__ h, const NodeW* _
             const unsigned after = lane < 31 ? (cm >> (lane + 1)) : 0u;
             const int run = __ffs(~after) - 1;                         // lanes that continue my range
             const int ne_run = __shfl_sync(0xffffffffu, ne, min(lane + run, 31));
-            list_append(lepf, head, 2, nb, ne_run, arena, arena_chunks, h, lane);
-            n_sp += __popc(__ballot_sync(0xffffffffu, act == 0));
-            n_spp += __popc(__ballot_sync(0xffffffffu, act == 4));
-            n_epn += __popc(__ballot_sync(0xffffffffu, act == 1));
-            n_epf += __popc(__ballot_sync(0xffffffffu, head));
+            // the four lists of the batch.  Usual case: every list has room in its current chunk -- one set of ballots, no per-list
+            // branching; otherwise (a new chunk is needed somewhere, about once in 16 batches) the general append, list by list
+            const unsigned m_sp = __ballot_sync(0xffffffffu, act == 0), m_spp = __ballot_sync(0xffffffffu, act == 4);
+            const unsigned m_epn = __ballot_sync(0xffffffffu, act == 1), m_epf = __ballot_sync(0xffffffffu, head);
+            const int c_sp = __popc(m_sp), c_spp = __popc(m_spp), c_epn = __popc(m_epn), c_epf = __popc(m_epf);
+            const bool fits = (c_sp == 0 || (lsp.chunk >= 0 && !lsp.dead && lsp.pos + c_sp <= PETAR_CHUNK_PAYLOAD)) &&
+                              (c_spp == 0 || (lspp.chunk >= 0 && !lspp.dead && lspp.pos + c_spp <= PETAR_CHUNK_PAYLOAD)) &&
+                              (c_epn == 0 || (lepn.chunk >= 0 && !lepn.dead && lepn.pos + 2 * c_epn <= PETAR_CHUNK_PAYLOAD)) &&
+                              (c_epf == 0 || (lepf.chunk >= 0 && !lepf.dead && lepf.pos + 2 * c_epf <= PETAR_CHUNK_PAYLOAD));
+            if (fits) {
+                const unsigned lt = (1u << lane) - 1u;
+                if (act == 0) arena[(size_t)lsp.chunk * PETAR_CHUNK + PETAR_CHUNK_HDR + lsp.pos + __popc(m_sp & lt)] = node_cur;
+                else if (act == 4) arena[(size_t)lspp.chunk * PETAR_CHUNK + PETAR_CHUNK_HDR + lspp.pos + __popc(m_spp & lt)] = node_cur;
+                else if (act == 1) { int* q = arena + (size_t)lepn.chunk * PETAR_CHUNK + PETAR_CHUNK_HDR + lepn.pos + 2 * __popc(m_epn & lt); q[0] = nb; q[1] = ne; }
+                else if (head) { int* q = arena + (size_t)lepf.chunk * PETAR_CHUNK + PETAR_CHUNK_HDR + lepf.pos + 2 * __popc(m_epf & lt); q[0] = nb; q[1] = ne_run; }
+                lsp.pos += c_sp; lspp.pos += c_spp; lepn.pos += 2 * c_epn; lepf.pos += 2 * c_epf;
+            } else {
+                list_append(lsp, act == 0, 1, node_cur, 0, arena, arena_chunks, h, lane);
+                list_append(lspp, act == 4, 1, node_cur, 0, arena, arena_chunks, h, lane);
+                list_append(lepn, act == 1, 2, nb, ne, arena, arena_chunks, h, lane);
+                list_append(lepf, head, 2, nb, ne_run, arena, arena_chunks, h, lane);
+            }
+            n_sp += c_sp; n_spp += c_spp; n_epn += c_epn; n_epf += c_epf;
             const int cn = __reduce_add_sync(0xffffffffu, (act == 1) ? (ne - nb) : 0);
             const int cf = __reduce_add_sync(0xffffffffu, (act == 2) ? (ne - nb) : 0);
             n_epn_part += cn; n_ep_part += cn + cf;
