@@ -430,7 +430,7 @@ def main():
             tt.close()
 
     # ---- FP32 peak probe (FFMA only), timed alone ------------------------------------------------------
-    scratch = torch.zeros(1, dtype=torch.float32, device=dev)
+    scratch = torch.zeros(2, dtype=torch.float32, device=dev)
     P.petar_probe_fp32(20000, scratch, stream)
     torch.cuda.synchronize()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -448,6 +448,8 @@ def main():
         torch.cuda.synchronize()
         a.record(stream); fl = P.petar_probe_fp32_mode(mode, iters, scratch, stream); b.record(stream); b.synchronize()
         probes[name] = fl / (a.elapsed_time(b) * 1e-3) / 1e12
+        if mode >= 8:
+            probes[name + "_sm_mhz"] = float(scratch[1].item())      # SM clock during the loop (tensor-core activity lowers it)
     pk, pk_kind = peaks()
     sm_max = float(pk.get("sm_max_mhz", 1965.0))
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count

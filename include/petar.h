@@ -319,6 +319,8 @@ int petar_probe_fp32(int64_t iters, double* flops_out_host, float* scratch_dev, 
  *           FP32 + 2 MUFU per cell pair) on static operands, iters = 32-cell tiles per CTA, 53 flops per interaction --
  *           8: alone, 9: with the kernel's MMAs (4 x 128x128x8 tf32 per tile) issued beside it through the kernel's
  *           full / empty mbarrier handshake.  Their difference is the cost of the tensor-core work to the CUDA-core loop.
+ *           Modes 8 and 9 need scratch_dev = DEVICE float[2] and leave the SM clock measured during the loop (clock64 against
+ *           %globaltimer, MHz) in scratch_dev[1]: the chip lowers the SM clock while tcgen05.mma instructions are in flight.
  * Errors: PETAR_EINVAL (mode), PETAR_ECUDA.                                                          */
 int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream);
 

@@ -1616,6 +1616,8 @@ __global__ void __launch_bounds__(160, 3) k_probe_tc(float* __restrict__ out, lo
         }
         const float nx = -(t * 0.01f + out[0]), ny = -(t * 0.02f), nz = -(0.5f + out[0]);
         Acc2 p = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        const long long c0 = clock64();
+        unsigned long long g0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
         for (long long k = 0; k < iters; ++k) {
             const int b = (int)(k & 1);
             if (MMA) { mbar_wait(smem_u32(&full[b]), (uint32_t)((k >> 1) & 1)); asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -1649,6 +1651,11 @@ __global__ void __launch_bounds__(160, 3) k_probe_tc(float* __restrict__ out, lo
         }
         const float s = p.ax.x + p.ay.x + p.az.x + p.pot.x + p.ax.y + p.ay.y + p.az.y + p.pot.y;
         if (s == 123.456f) out[0] = s;
+        if (t == 0 && blockIdx.x == 0) {       // SM clock during the loop: cycles per nanosecond of the global timer, in MHz
+            const long long c1 = clock64();
+            unsigned long long g1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+            out[1] = (float)(1.0e3 * (double)(c1 - c0) / (double)(g1 - g0));
+        }
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
