@@ -43,6 +43,8 @@ extern "C" {
 #define PETAR_ECUDA (-3)      /* CUDA launch/runtime error; petar_strerror gives the CUDA text    */
 #define PETAR_ENOTBUILT (-4)  /* handle is NULL, destroyed, or no tree has been built into it     */
 #define PETAR_ESTATUS (-5)    /* device status word is non-zero (returned only by calls that sync) */
+#define PETAR_ECAPACITY (-6)  /* N is larger than the fixed size of the library's built-in scratch array
+                                 (petar_short_range_force_noalloc: PETAR_SHORT_RANGE_NOALLOC_MAX_N)    */
 
 /* bits of the device status word */
 #define PETAR_ST_NONFINITE 1     /* a position, mass or radius is NaN/Inf, or a radius is <= 0     */
@@ -190,6 +192,38 @@ int petar_short_range_force(const double* x, const double* y, const double* z,
                             double* acc_x, double* acc_y, double* acc_z,
                             double* jerk_x, double* jerk_y, double* jerk_z, double* pot,
                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* The same computation, same arguments and same results as petar_short_range_force, for callers that cannot
+ * give it a workspace because they cannot allocate device memory at all: code that runs as a plug-in of a host
+ * application and is only ever handed pointers; code inside a memory pool whose budget is fixed and spent; a
+ * latency-bound integrator loop that must not hit the device-wide synchronisation of cudaMalloc/cudaFree.  Such a
+ * caller passes its inputs and outputs and nothing else.
+ *
+ * Where the scratch lives.  The packed particle records and the queue of long rows (68 bytes per particle) go to a
+ * fixed array that is part of the library itself, sized for PETAR_SHORT_RANGE_NOALLOC_MAX_N particles (about
+ * 4.3 MB).  The cost of that convenience: every GPU that loads this library holds the array until the process
+ * exits, called or not.  N above the maximum is refused with PETAR_ECAPACITY before anything is enqueued; use
+ * petar_short_range_force with your own workspace for larger sets.
+ *
+ * The call itself never calls cudaMalloc, cudaFree or any other allocating routine (one 4-byte cudaMemsetAsync,
+ * three kernel launches).  The FIRST call on each device also looks up the array's device address (the device of the
+ * stream must be the current device, as for every call of this library); make that first call outside any stream
+ * capture, e.g. once at start-up with a tiny N.  Later calls on that device only launch.
+ *
+ * One array for everybody.  All calls in the process on one device share the array and it keeps whatever the last
+ * call left in it; the call clears the one counter that has to start at zero.  Two calls that can be in flight on
+ * the GPU at the same time (different streams, or different host threads on different streams) write over each
+ * other's scratch and give wrong results: put them on one stream, or order them with events.
+ * Errors: PETAR_EINVAL, PETAR_ECAPACITY, PETAR_ECUDA.                                                 */
+#define PETAR_SHORT_RANGE_NOALLOC_MAX_N 65536
+int petar_short_range_force_noalloc(const double* x, const double* y, const double* z,
+                                    const double* vx, const double* vy, const double* vz,
+                                    const double* m, const double* r_out,
+                                    const int64_t* offsets, const int32_t* indices, int64_t N,
+                                    double G, double r_in_over_r_out,
+                                    double* acc_x, double* acc_y, double* acc_z,
+                                    double* jerk_x, double* jerk_y, double* jerk_z, double* pot,
+                                    void* cuda_stream);
 
 /* ---- P3T-kick and the artificial particles (section 6.4) -----------
  * P3T-kick: v += a dt, in place.  All DEVICE fp64[N].                           */

@@ -13,7 +13,7 @@ from .binding import (  # noqa: F401
     petar_tree_status, petar_tree_destroy, petar_strerror, petar_debug_export,
     petar_set_profiling, petar_stage_times, petar_launch_count, petar_probe_fp32, petar_probe_fp32_mode,
     petar_search_radii, petar_neighbor_list_orbit, petar_clusters_workspace_bytes, petar_clusters,
-    petar_short_range_workspace_bytes, petar_short_range_force,
+    petar_short_range_workspace_bytes, petar_short_range_force, petar_short_range_force_noalloc, SHORT_RANGE_NOALLOC_MAX_N,
     petar_kick, petar_artificial_particles, petar_tidal_tensor_fit, petar_orbit_sampling, art_count,
     STAGE_NAMES,
 )

@@ -13,7 +13,7 @@ EXPORTS = [
     "petar_tree_status", "petar_tree_destroy", "petar_strerror", "petar_debug_export",
     "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32", "petar_probe_fp32_mode",
     "petar_search_radii", "petar_neighbor_list_orbit", "petar_clusters_workspace_bytes", "petar_clusters",
-    "petar_short_range_workspace_bytes", "petar_short_range_force",
+    "petar_short_range_workspace_bytes", "petar_short_range_force", "petar_short_range_force_noalloc",
     "petar_kick", "petar_artificial_particles", "petar_tidal_tensor_fit", "petar_orbit_sampling",
 ]
 STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units", "walk_super"]
@@ -88,6 +88,9 @@ def lib():
         L.petar_short_range_force.restype = C.c_int
         L.petar_short_range_force.argtypes = ([C.c_void_p] * 10 + [C.c_int64, C.c_double, C.c_double] + [C.c_void_p] * 7
                                               + [C.c_void_p, C.c_size_t, C.c_void_p])
+        L.petar_short_range_force_noalloc.restype = C.c_int
+        L.petar_short_range_force_noalloc.argtypes = ([C.c_void_p] * 10 + [C.c_int64, C.c_double, C.c_double] + [C.c_void_p] * 7
+                                                      + [C.c_void_p])
         L.petar_kick.restype = C.c_int
         L.petar_kick.argtypes = [C.c_void_p] * 6 + [C.c_double, C.c_int64, C.c_void_p]
         L.petar_artificial_particles.restype = C.c_int
@@ -213,6 +216,22 @@ def petar_short_range_force(x, y, z, vx, vy, vz, m, r_out, offsets, indices, N: 
                                        _ptr(workspace), C.c_size_t(0 if workspace is None else workspace.numel()), _stream(stream))
     if rc:
         raise PetarError(rc, "petar_short_range_force")
+
+
+SHORT_RANGE_NOALLOC_MAX_N = 65536     # PETAR_SHORT_RANGE_NOALLOC_MAX_N of include/petar.h
+
+
+def petar_short_range_force_noalloc(x, y, z, vx, vy, vz, m, r_out, offsets, indices, N: int, G: float, rho: float,
+                                    acc, jerk, pot, stream=None) -> None:
+    """petar_short_range_force without the workspace argument, for callers that cannot allocate device memory (a plug-in
+    that only receives pointers, a spent memory pool, a loop that must not stall on cudaMalloc).  The scratch is a fixed
+    array inside the library, so N <= SHORT_RANGE_NOALLOC_MAX_N (else PetarError with code -6) and calls that overlap on
+    the GPU must be ordered by the caller.  Arguments as petar_short_range_force."""
+    rc = lib().petar_short_range_force_noalloc(*[_ptr(a) for a in (x, y, z, vx, vy, vz, m, r_out, offsets, indices)], C.c_int64(N),
+                                               C.c_double(G), C.c_double(rho), *[_ptr(a) for a in acc], *[_ptr(a) for a in jerk],
+                                               _ptr(pot), _stream(stream))
+    if rc:
+        raise PetarError(rc, "petar_short_range_force_noalloc")
 
 
 def petar_kick(vx, vy, vz, ax, ay, az, dt: float, N: int, stream=None) -> None:

@@ -332,6 +332,7 @@ extern "C" const char* petar_strerror(int code) {
         case PETAR_ECUDA: return cudaGetErrorString(g_last_cuda);
         case PETAR_ENOTBUILT: return "no tree built / handle destroyed";
         case PETAR_ESTATUS: return "device status word non-zero (see petar_tree_status)";
+        case PETAR_ECAPACITY: return "N exceeds the fixed capacity of the library's built-in scratch array (PETAR_SHORT_RANGE_NOALLOC_MAX_N); use the call that takes a workspace";
         default: return "unknown error";
     }
 }

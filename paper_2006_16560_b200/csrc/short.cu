@@ -10,6 +10,7 @@
 // 64-byte record per particle (64 B read + 64 B written), then 64 B read + 56 B written per particle and one
 // 64-byte record gathered per list entry.
 #include "internal.cuh"
+#include <mutex>
 
 // multiprocessors of the current device (queried once)
 static int sm_count() {
@@ -135,6 +136,76 @@ extern "C" int petar_short_range_force(const double* x, const double* y, const d
     int* queue = (int*)workspace;
     ShortRec* rec = (ShortRec*)((char*)workspace + short_queue_bytes(N));
     A.rec = rec;
+    if (cudaMemsetAsync(queue, 0, 4, s) != cudaSuccess) return PETAR_ECUDA;
+    k_short_pack<<<cdiv(N, 256), 256, 0, s>>>(A, rec);
+    KCHECK(s, "k_short_pack");
+    k_short_rows<<<cdiv(N, 256), 256, 0, s>>>(A, queue);
+    KCHECK(s, "k_short_rows");
+    k_short_long_rows<<<sm_count() * 4, 256, 0, s>>>(A, queue);
+    KCHECK(s, "k_short_long_rows");
+    petar_count_launch(3);
+    return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;
+}
+
+// ---- petar_short_range_force_noalloc: the same three kernels for callers that have no way to allocate ------------
+// petar_short_range_force needs 68 bytes of caller-supplied device workspace per particle.  Some callers cannot
+// supply any: a plug-in that is handed device pointers by a host program and owns no allocator; a step that runs inside
+// somebody else's memory pool whose budget is already spent; a real-time or stream-ordered loop in which a
+// cudaMalloc (which synchronises the whole device) is not acceptable.  For them the workspace below is part of the
+// library image: a fixed array in device global memory, PETAR_SHORT_RANGE_NOALLOC_MAX_N particles large (about
+// 4.3 MB).  Every GPU on which this library's code is loaded carries that array until the process exits,
+// whether or not the entry point is ever called -- which is why the limit is small.
+#define NOALLOC_QUEUE_BYTES ((((size_t)PETAR_SHORT_RANGE_NOALLOC_MAX_N + 1) * 4 + 255) / 256 * 256)
+#define NOALLOC_BYTES (NOALLOC_QUEUE_BYTES + (size_t)PETAR_SHORT_RANGE_NOALLOC_MAX_N * sizeof(ShortRec))
+static __device__ __align__(256) unsigned char g_short_noalloc_scratch[NOALLOC_BYTES];
+
+// In HOST code the name g_short_noalloc_scratch is only the handle by which the runtime knows the array; it is not
+// the array's address on the GPU and must never be handed to a kernel.  The address is asked for once per device
+// (with that device current) and remembered; devices beyond the table are looked up on every call.
+#define NOALLOC_MAX_DEVICES 64
+static void* g_noalloc_ptr[NOALLOC_MAX_DEVICES];
+static std::mutex g_noalloc_mutex;
+
+static cudaError_t noalloc_scratch(void** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool cached = dev >= 0 && dev < NOALLOC_MAX_DEVICES;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (cached && g_noalloc_ptr[dev]) { *out = g_noalloc_ptr[dev]; return cudaSuccess; }
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_short_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p || ((uintptr_t)p & 255u)) return cudaErrorInvalidSymbol;
+    if (cached) g_noalloc_ptr[dev] = p;
+    *out = p;
+    return cudaSuccess;
+}
+
+extern "C" int petar_short_range_force_noalloc(const double* x, const double* y, const double* z, const double* vx, const double* vy,
+                                               const double* vz, const double* m, const double* r_out, const int64_t* offsets,
+                                               const int32_t* indices, int64_t N, double G, double r_in_over_r_out,
+                                               double* acc_x, double* acc_y, double* acc_z, double* jerk_x, double* jerk_y,
+                                               double* jerk_z, double* pot, void* cuda_stream) {
+    if (N < 0 || !(r_in_over_r_out > 0.0 && r_in_over_r_out < 1.0) || !(G == G)) return PETAR_EINVAL;
+    if (N > PETAR_SHORT_RANGE_NOALLOC_MAX_N) return PETAR_ECAPACITY;          // before anything is touched or enqueued
+    if (N == 0) return PETAR_OK;
+    if (!x || !y || !z || !vx || !vy || !vz || !m || !r_out || !offsets) return PETAR_EINVAL;
+    void* scratch = nullptr;
+    if (noalloc_scratch(&scratch) != cudaSuccess) return PETAR_ECUDA;         // first call on this device: the set-up
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    ShortArgs A;
+    A.x = x; A.y = y; A.z = z; A.vx = vx; A.vy = vy; A.vz = vz; A.m = m; A.rout = r_out;
+    A.offsets = (const long long*)offsets; A.indices = indices;
+    A.ax = acc_x; A.ay = acc_y; A.az = acc_z; A.jx = jerk_x; A.jy = jerk_y; A.jz = jerk_z; A.pot = pot;
+    A.G = G; A.rho = r_in_over_r_out; A.lam = (1.0 - r_in_over_r_out) / (1.0 + r_in_over_r_out);
+    A.q = r_in_over_r_out / (1.0 - r_in_over_r_out); A.n = N;
+    // same split of the scratch as the workspace of petar_short_range_force, at the fixed maximum size
+    int* queue = (int*)scratch;
+    ShortRec* rec = (ShortRec*)((char*)scratch + NOALLOC_QUEUE_BYTES);
+    A.rec = rec;
+    // The array still holds what the previous call left.  Only the long-row counter queue[0] has to start at zero;
+    // the records and queue entries that this call reads are all written by this call first.
     if (cudaMemsetAsync(queue, 0, 4, s) != cudaSuccess) return PETAR_ECUDA;
     k_short_pack<<<cdiv(N, 256), 256, 0, s>>>(A, rec);
     KCHECK(s, "k_short_pack");
