@@ -77,7 +77,8 @@ typedef struct {
     int64_t n_epep;         /* sum over groups n_i * n_ep   (particle-particle interactions)        */
     int64_t n_epsp;         /* sum over groups n_i * n_sp   (particle-cell interactions)            */
     int64_t n_epep_near;    /* part of n_epep that went through the changeover polynomials          */
-    int64_t n_ep_list;      /* sum over groups of EP leaf ranges                                    */
+    int64_t n_ep_list;      /* sum over groups of EP particle ranges as listed: near leaves one range each,
+                               runs of contiguous far leaves joined into one range (<= the number of leaves) */
     int64_t n_sp_list;      /* sum over groups of accepted cells                                    */
     int64_t list_entries_used; /* 4-byte arena entries used                                         */
     int64_t n_epsp_common;  /* part of n_epsp evaluated super-group-wide (cells every i-group of a
@@ -119,9 +120,10 @@ int petar_tree_rebuild(petar_tree* t, const double* x, const double* y, const do
  *   acc_x, acc_y, acc_z, pot : DEVICE fp64[N], caller's particle order; pot is the specific
  *                              long-range potential phi_L,i (negative).  Any may be NULL (skipped).
  *   counts_host_or_null      : HOST; if non-NULL the call synchronises the stream and fills it, and
- *                              returns PETAR_ESTATUS if the device status word is non-zero.
- * When the status word is non-zero (capacity exceeded, non-finite input) the force kernels write NOTHING:
- * the outputs keep their previous contents; check petar_tree_status (or pass counts) before using them.
+ *                              returns PETAR_ESTATUS if one of the status bits named below is set.
+ * When PETAR_ST_NONFINITE, _NODE_CAP, _LIST_CAP or _STACK is set (the tree or its lists are unusable) the force
+ * kernels write NOTHING: the outputs keep their previous contents; check petar_tree_status (or pass counts) before
+ * using them.  PETAR_ST_NB_CAP (a neighbour fill whose `capacity` was too small) does not affect this call.
  * Errors: PETAR_ENOTBUILT, PETAR_ECUDA, PETAR_ESTATUS.                                              */
 int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_y, double* acc_z, double* pot,
                            petar_counts* counts_host_or_null, void* cuda_stream);

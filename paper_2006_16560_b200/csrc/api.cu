@@ -213,15 +213,23 @@ extern "C" int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_
         CK(launch_walk_supers(t, s));
         CK(cudaEventRecord(t->ev_fork, s));
         CK(cudaStreamWaitEvent(t->side, t->ev_fork, 0));
-        CK(launch_walk_groups(t, t->side, OVERLAP_WALK_CTAS));      // launched first: its CTAs take their place on the SMs before the unit kernels'
-        CK(launch_force_units_table(t, s));
-        CK(cudaEventRecord(t->ev_tab, s));
-        CK(launch_force_units_tc(t, s));
-        CK(cudaStreamWaitEvent(t->side, t->ev_tab, 0));
-        CK(launch_force_units_small(t, t->side));          // the small units and the changeover pairs follow the walk on the side stream,
-        CK(launch_force_near(t, t->side));                 // beside the tail of the tensor-core kernel
-        CK(cudaEventRecord(t->ev_join, t->side));
-        CK(cudaStreamWaitEvent(s, t->ev_join, 0));
+        // From here on the side stream may hold work that uses the workspace: whatever fails, the caller's stream is made to
+        // wait for it before this call returns, so that an error return never leaves work running behind the caller's back.
+        cudaError_t fe = [&]() -> cudaError_t {
+            cudaError_t e;
+            if ((e = launch_walk_groups(t, t->side, OVERLAP_WALK_CTAS)) != cudaSuccess) return e;   // launched first: its CTAs take their place on the SMs before the unit kernels'
+            if ((e = launch_force_units_table(t, s)) != cudaSuccess) return e;
+            if ((e = cudaEventRecord(t->ev_tab, s)) != cudaSuccess) return e;
+            if ((e = launch_force_units_tc(t, s)) != cudaSuccess) return e;
+            if ((e = cudaStreamWaitEvent(t->side, t->ev_tab, 0)) != cudaSuccess) return e;
+            if ((e = launch_force_units_small(t, t->side)) != cudaSuccess) return e;   // the small units and the changeover pairs follow the walk on the side
+            return launch_force_near(t, t->side);                                      // stream, beside the tail of the tensor-core kernel
+        }();
+        cudaError_t je = cudaEventRecord(t->ev_join, t->side);
+        if (je == cudaSuccess) je = cudaStreamWaitEvent(s, t->ev_join, 0);
+        if (je != cudaSuccess) cudaStreamSynchronize(t->side);      // could not order the streams on the device: wait on the host instead
+        CK(fe);
+        CK(je);
         stage_end(t, PETAR_STAGE_FORCE_UNITS, s);
         t->walked = true;
         CK(launch_force_groups(t, acc_x, acc_y, acc_z, pot, s));
@@ -238,7 +246,7 @@ extern "C" int petar_long_range_force(petar_tree* t, double* acc_x, double* acc_
         counts->list_entries_used = (int64_t)hh.arena_top * PETAR_CHUNK;
         counts->n_epsp_common = (int64_t)hh.n_epsp_common;
         counts->n_refined = (int64_t)hh.n_refine;
-        if (hh.status) return PETAR_ESTATUS;
+        if (hh.status & PETAR_ST_FATAL) return PETAR_ESTATUS;      // the bits that made the kernels write nothing
     }
     return PETAR_OK;
 }

@@ -342,7 +342,7 @@ __global__ void __launch_bounds__(NEAR_WARPS * 32) k_force_near(DevHeader* __res
     const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
     NearTile& tl = s_tile[wp];
     const int ng = h->n_groups;
-    if (h->status != 0) return;
+    if (h->status & PETAR_ST_FATAL) return;
     for (;;) {
         int g = 0;
         if (lane == 0) g = atomicAdd(&h->group_ticket4, 1);
@@ -412,7 +412,7 @@ __global__ void __launch_bounds__(FT, FORCE_MIN_CTAS) k_force(DevHeader* __restr
     __shared__ int s_off[FT + 1], s_jb[FT];
     const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
     const int ng = h->n_groups;
-    if (h->status != 0) return;            // capacity exceeded / non-finite input: lists are unusable, write nothing (petar.h)
+    if (h->status & PETAR_ST_FATAL) return;   // capacity exceeded / non-finite input: lists are unusable, write nothing (petar.h)
     const double rcx = h->c[0], rcy = h->c[1], rcz = h->c[2];
     for (;;) {
         __syncthreads();
@@ -609,7 +609,7 @@ __global__ void __launch_bounds__(REFINE_THREADS) k_force_refine(const DevHeader
     __shared__ double s_red[REFINE_THREADS / 32][4];
     const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
     const int nq = h->n_refine;
-    if (h->status != 0) return;
+    if (h->status & PETAR_ST_FATAL) return;
     for (int q = blockIdx.x; q < nq; q += gridDim.x) {          // one CTA per particle
         const int g = A.queue[2 * (size_t)q], pos = A.queue[2 * (size_t)q + 1];
         const GroupRec* gr = &A.grp[g];
@@ -869,7 +869,11 @@ __global__ void __launch_bounds__(UW * 32, UNITS_MIN_CTAS) k_force_units(DevHead
     double* sacc = &s_acc[0][threadIdx.x];
     const int nu = h->unit_off[PETAR_UNIT_CLASSES];
     const int u0 = h->unit_off[first_class];       // units of the classes before first_class belong to k_force_units_tc
-    if (h->status != 0) return;            // see k_force
+    // One read per CTA, then a uniform branch: k_walk may set a bit while this kernel runs beside it, and warps of one CTA
+    // that read different values would part ways before the barriers below.
+    if (threadIdx.x == 0) s_u = *(volatile const int*)&h->status & PETAR_ST_FATAL;
+    __syncthreads();
+    if (s_u) return;                        // see k_force
     for (;;) {
         __syncthreads();                    // s_u and s_acc of the previous unit consumed
         if (threadIdx.x == 0) s_u = u0 + atomicAdd(&h->unit_ticket, 1);
@@ -1005,7 +1009,12 @@ __global__ void __launch_bounds__(TC_THREADS, TC_REG_CTAS) k_force_units_tc(DevH
     TcSmem& sm = *reinterpret_cast<TcSmem*>(tc_smem_raw);
     const int t = threadIdx.x, lane = t & 31, w = t >> 5;
     const int nu = h->unit_off[1];                 // class 0
-    if (h->status != 0) return;
+    // The status is read ONCE per CTA: k_walk runs beside this kernel on the side stream and may set PETAR_ST_LIST_CAP or
+    // PETAR_ST_STACK at any moment.  Were every thread to read it, some warps could leave before mbarrier.init / tcgen05.alloc
+    // and the rest would wait for them for ever.  (A bit set after this point is seen by k_force, which then writes nothing.)
+    if (t == 0) sm.unit = *(volatile const int*)&h->status & PETAR_ST_FATAL;
+    __syncthreads();
+    if (sm.unit) return;                           // (sm.unit is next written by the ticket loop, behind the barrier below)
     if (t == 0) {
         for (int q = 0; q < TC_BUFS; ++q) {
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&sm.full[q])));
@@ -1335,14 +1344,12 @@ cudaError_t launch_force_units_tc(petar_tree* t, cudaStream_t s) {
     Workspace& w = t->w;
     if (t->p.multipole < 2) return cudaSuccess;
     cudaError_t e;
-    static bool tc_attr = false;
-    if (!tc_attr) {
-        // the same (maximal) shared-memory carve-out for every kernel that runs beside another one: an SM only changes its carve-out when idle
-        e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TcSmem)); if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_force_units<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
-        tc_attr = true;
-    }
+    // Function attributes belong to the current device, so they are set on every launch (a host-side table update, no device
+    // work) rather than remembered in a process-wide flag that a second GPU would never see.
+    // The same (maximal) shared-memory carve-out for every kernel that runs beside another one: an SM only changes its carve-out when idle
+    e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TcSmem)); if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_force_units_tc, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_force_units<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e;
     // (the occupancy query reports 1 CTA per SM for a kernel that allocates tensor memory; registers, shared memory and the
     // 512 TMEM columns allow TC_MIN_CTAS, and persistent CTAs that find no ticket left simply exit)
     k_force_units_tc<<<t->sm_count * TC_MIN_CTAS, TC_THREADS, sizeof(TcSmem), s>>>(w.hdr, w.units, w.srec, w.group_cap, w.nw, w.arena, w.nsp, w.pa, w.pb, w.part, w.part_s, (long long)t->N);

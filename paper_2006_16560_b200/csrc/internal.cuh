@@ -4,6 +4,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "../../include/petar.h"
+// status bits that leave the tree or its interaction lists unusable: the force kernels write nothing when one is set.
+// PETAR_ST_NB_CAP is not among them -- a neighbour fill with too small a `capacity` (a supported use of the two-phase
+// call) truncates the caller's index array only; lists, forces and a later, larger fill are unaffected.
+#define PETAR_ST_FATAL (PETAR_ST_NONFINITE | PETAR_ST_NODE_CAP | PETAR_ST_LIST_CAP | PETAR_ST_STACK)
 
 #define PETAR_MAXLEVEL 21
 #define PETAR_NLEVELS 22           // levels 0..21

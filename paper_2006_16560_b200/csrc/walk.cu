@@ -466,8 +466,9 @@ cudaError_t launch_walk_groups(petar_tree* t, cudaStream_t s, int ctas_per_sm) {
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     if (ctas_per_sm > 0 && ctas_per_sm < per_sm) per_sm = ctas_per_sm;
-    static bool attr = false;       // the carve-out of the kernels it runs beside (launch_force_units)
-    if (!attr) { e = cudaFuncSetAttribute(k_walk, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared); if (e != cudaSuccess) return e; attr = true; }
+    // the carve-out of the kernels it runs beside (launch_force_units); per device, hence set on every launch
+    e = cudaFuncSetAttribute(k_walk, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
     k_walk<<<t->sm_count * per_sm, WALK_WARPS * 32, 0, s>>>(w.hdr, w.nw, w.nmac, w.grp, w.srec, w.smap, w.arena, w.arena_chunks, t->p.theta, w.node_cap,
                                                           (long long)t->N, w.group_cap);
     KCHECK(s, "k_walk");

@@ -345,6 +345,73 @@ def test_rebuild_is_deterministic():
     t.close()
 
 
+def test_rebuild_with_moved_particles_and_toggled_search_radii():
+    """petar_tree_rebuild (the call of a time-stepping loop, and what bench.py times) into a handle that holds the
+    leftovers of a DIFFERENT tree: other positions, masses and order, search radii switched off and on again.  Whatever
+    the previous tree left in the workspace or the handle (walk done, neighbour counts kept, header counters, node,
+    group and super-group tables, list arena) must not show: every structure bit-exact against a fresh oracle tree,
+    the lists of EVERY group (not a sample) as sets, forces within TOL, neighbours bit-exact."""
+    w1 = make_workload(2, N=30000, seed=8)
+    w2 = make_workload(2, N=30000, seed=9)
+    perm = np.random.default_rng(4).permutation(w2.N)           # and in another order than the generator's
+    for name in ("x", "y", "z", "m", "r_out"):
+        setattr(w2, name, np.ascontiguousarray(getattr(w2, name)[perm]))
+    rs1 = w1.r_out * (1.0 + np.random.default_rng(1).random(w1.N))
+    rs2 = w2.r_out * (1.0 + 2.0 * np.random.default_rng(2).random(w2.N))
+    t = _gpu_tree(w1, rsearch=rs1)                              # first tree: with search radii, walked, neighbours counted and filled
+    t.force(); t.neighbors()
+    for w, rs in ((w2, None), (w2, rs2), (w1, None)):
+        t.upload(w.x, w.y, w.z, w.m, w.r_out, rs)
+        t.build()                                               # -> petar_tree_rebuild
+        T = _ora_tree(w, rsearch=rs)
+        check_structures(t, T, w)
+        for v in (t.acc_x, t.acc_y, t.acc_z, t.pot):
+            v.fill_(float("nan"))
+        counts = t.force(want_counts=True)
+        check_counts_and_lists(t, T, counts, sample=1 << 30)    # every group
+        g = [_np(v) for v in (t.acc_x, t.acc_y, t.acc_z, t.pot)]
+        ea, ep = _rel_err(g, T.force())
+        assert ea.max() < TOL and ep.max() < TOL, (ea.max(), ep.max())
+        check_neighbors(t, T, w.N)
+    t.close()
+
+
+def test_force_after_neighbour_capacity_overflow():
+    """A neighbour fill with too small a `capacity` is a supported use of the two-phase call; it sets the sticky
+    PETAR_ST_NB_CAP bit.  The interaction lists are untouched by it, so a force call afterwards must still write its
+    results (it used to return PETAR_OK and write nothing) and report no error with counts."""
+    import torch
+    P = _P()
+    w = make_workload(2, N=20011, seed=5)
+    t, T = _gpu_tree(w), _ora_tree(w)
+    P.petar_neighbor_list(t.handle, t.offsets, None, 0)
+    total = int(t.offsets[-1])
+    assert total > 10
+    idx = torch.full((total,), -7, dtype=torch.int32, device="cuda")
+    st = torch.zeros(1, dtype=torch.int32, device="cuda")
+    P.petar_neighbor_list(t.handle, t.offsets, idx, total // 2, st)
+    torch.cuda.synchronize()
+    assert int(st[0]) == 1 and P.petar_tree_status(t.handle) == 16
+    for v in (t.acc_x, t.acc_y, t.acc_z, t.pot):
+        v.fill_(float("nan"))
+    counts = t.force(want_counts=True)                          # no PETAR_ESTATUS: none of the fatal bits is set
+    _, epep, epsp = T.walk_counts()
+    assert (counts.n_epep, counts.n_epsp) == (epep, epsp)
+    g = [_np(v) for v in (t.acc_x, t.acc_y, t.acc_z, t.pot)]
+    assert all(np.all(np.isfinite(v)) for v in g)               # written
+    ea, ep = _rel_err(g, T.force())
+    assert ea.max() < TOL and ep.max() < TOL, (ea.max(), ep.max())
+    # a second force call on the walked tree (the other launch path), and the full-size fill, work as well
+    for v in (t.acc_x, t.acc_y, t.acc_z, t.pot):
+        v.fill_(float("nan"))
+    t.force()
+    g2 = [_np(v) for v in (t.acc_x, t.acc_y, t.acc_z, t.pot)]
+    ea, ep = _rel_err(g2, T.force())
+    assert ea.max() < TOL and ep.max() < TOL, (ea.max(), ep.max())
+    check_neighbors(t, T, w.N)
+    t.close()
+
+
 # ---- BASELINE.json full sizes, in the launch configuration bench.py times -------------------------------
 @pytest.mark.parametrize("cfg", [3, 4])
 def test_full_size(cfg):
