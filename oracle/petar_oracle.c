@@ -27,8 +27,11 @@
  * the O(N^2) short-range definition of part (A), dK/dx against a difference quotient of Eq. 17, the
  * jerk against a difference quotient of the acceleration along x + v t, Newton's two-body jerk
  * inside r_in, and sum m a = sum m j = 0.
- * Parity UNPINNED (the paper prints nothing to pin them to): interaction counts and
- * force error at theta > 0 (only monotonicity sanity checks).
+ * The acceptance RULE of the walk (visit(): l^2 < theta^2 d^2, l = cube edge, d = group box to centre of
+ * mass, reading P8) is pinned by a hand-worked dyadic geometry in which the cell flips at theta = 4/sqrt(116.8125)
+ * (tests/test_oracle_tree.py::test_opening_criterion_flips_at_hand_computed_theta).
+ * Parity UNPINNED (the paper prints nothing to pin them to): the NUMBERS that follow from it on a real
+ * workload -- interaction counts and force error at theta > 0 (only monotonicity sanity checks).
  *
  * Floating point: everything is IEEE double.  Build with -ffp-contract=off so that the
  * compiler fuses nothing; fma() is called explicitly where rule O5/O7/O9 says so.

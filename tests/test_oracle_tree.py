@@ -208,3 +208,68 @@ def test_degenerate_inputs():
     T = oracle.OracleTree(pos[:, 0], pos[:, 1], pos[:, 2], m0, rout, p)
     a = T.force(); d = oracle.direct(pos[:, 0], pos[:, 1], pos[:, 2], m0, rout, p, "long")
     assert np.allclose(a[1], d[1], rtol=1e-13) and np.all(np.isfinite(a[0]))
+
+
+@pytest.mark.parametrize("mirror", [(0, 0, 0), (1, 0, 0), (1, 1, 1)])
+def test_opening_criterion_flips_at_hand_computed_theta(mirror):
+    """Pin of reading P8 (PAPER.md:207 "inside theta ... centre-of-the-mass", :152 theta < 1): a cell is accepted iff
+    l < theta * d, l = edge of its CUBE, d = distance from the group's tight BOX to the cell's CENTRE OF MASS.
+
+    Worked by hand on dyadic coordinates (all values exact in binary).  Anchors at (0,0,0) and (15,15,15) give, by rule O1,
+    c = 7.5, L = 15, v = 7.5 (1 + 2^-20), h = 8: the root cube is [-0.5, 15.5]^3, level-1 edges are 8, level-2 edges 4.
+      cell C  = level-2 cube [11.5,15.5] x [-0.5,3.5] x [-0.5,3.5], l = 4, holding p1 = (12,1,1) with mass 3 and
+                p2 = (15,3,1) with mass 1: com = (12.75, 1.5, 1) -- not the cube centre (13.5, 1.5, 1.5);
+                a leaf with n_leaf = 2; its level-1 parent also holds p3 = (9,6,6), so the parent is split;
+      group G = level-1 cube [-0.5,7.5]^3 with (0,0,0) and (2,1,0): 2 = n_group members, box [0,2] x [0,1] x [0,0].
+    d^2 = (12.75-2)^2 + (1.5-1)^2 + (1-0)^2 = 115.5625 + 0.25 + 1 = 116.8125, so C flips at theta* = 4/sqrt(116.8125) = 0.370099...
+    Thresholds a misreading would give instead (each at least 6 % away from theta*):
+      half edge (l = 2)                       2/sqrt(116.8125) = 0.18505
+      tight box of C as l (longest side 3)    3/sqrt(116.8125) = 0.27757
+      cube centre of C instead of its com     4/sqrt(11.5^2 + 0.5^2 + 1.5^2) = 4/sqrt(134.75)   = 0.34458
+      centre of G (1, 0.5, 0) instead of box  4/sqrt(11.75^2 + 1 + 1)        = 4/sqrt(140.0625) = 0.33799
+      box of G to tight box of C              4/sqrt(10^2 + 0 + 1)           = 4/sqrt(101)      = 0.39801
+      l^2 < theta d^2 (theta not squared)     16/116.8125                                       = 0.13697
+    All but one lie below theta* (they would still accept C just below it), box-to-box lies above (it would still open C
+    just above it); both sides of the flip are asserted.  The mirrored cases put the cell on the low side of the group, so
+    both arms of max(0, lo_g - com, com - hi_g) are used on every axis."""
+    pts = np.array([[0, 0, 0], [2, 1, 0],                    # group G
+                    [12, 1, 1], [15, 3, 1],                  # cell C
+                    [9, 6, 6],                               # makes C's level-1 parent split
+                    [15, 15, 15]], dtype=np.float64)         # anchor
+    m = np.array([1.0, 1.0, 3.0, 1.0, 1.0, 1.0])
+    for k in range(3):
+        if mirror[k]:
+            pts[:, k] = 15.0 - pts[:, k]                     # the root cube [-0.5, 15.5] maps onto itself
+    rout = np.full(6, 1e-3)                                  # nothing comes near: the forced-open rule stays out of it
+    d2 = 10.75 ** 2 + 0.5 ** 2 + 1.0 ** 2
+    assert d2 == 116.8125
+    theta_star = 4.0 / np.sqrt(d2)
+    for wrong in (2 / np.sqrt(d2), 3 / np.sqrt(d2), 4 / np.sqrt(134.75), 4 / np.sqrt(140.0625), 4 / np.sqrt(101.0), 16 / d2):
+        assert abs(wrong / theta_star - 1.0) > 0.06
+
+    def lists(theta):
+        p = oracle.OracleParams.make(theta=theta, multipole=2, n_leaf=2, n_group=2)
+        T = oracle.OracleTree(pts[:, 0], pts[:, 1], pts[:, 2], m, rout, p)
+        c, h = T.root()
+        assert np.array_equal(c, [7.5, 7.5, 7.5]) and h == 8.0                               # rule O1 as worked above
+        nd = T.nodes()
+        lo_c, hi_c = pts[2:4].min(0), pts[2:4].max(0)
+        cell = [n for n in range(T.n_nodes) if nd.level[n] == 2 and np.array_equal(nd.lo[n], lo_c) and np.array_equal(nd.hi[n], hi_c)]
+        assert len(cell) == 1 and nd.leaf[cell[0]] == 1 and nd.M[cell[0]] == 4.0
+        com = (3.0 * pts[2] + 1.0 * pts[3]) / 4.0
+        assert np.array_equal(nd.com[cell[0]], com) and abs(com[0] - 7.5) == 5.25            # 12.75 or its mirror image 2.25
+        gb, ge, glo, ghi, _ = T.groups()
+        grp = [g for g in range(T.n_groups) if np.array_equal(glo[g], pts[0:2].min(0)) and np.array_equal(ghi[g], pts[0:2].max(0))]
+        assert len(grp) == 1 and ge[grp[0]] - gb[grp[0]] == 2
+        sp, ep = T.walk_lists(grp[0])
+        return cell[0], (int(nd.begin[cell[0]]), int(nd.end[cell[0]])), set(sp.tolist()), {(int(b), int(e)) for b, e, _ in ep}
+
+    cid, rng_c, sp, ep = lists(theta_star * (1 + 1e-12))
+    assert cid in sp and rng_c not in ep                     # l < theta d: accepted as one super-particle
+    cid, rng_c, sp, ep = lists(theta_star * (1 - 1e-12))
+    assert cid not in sp and rng_c in ep                     # l > theta d: opened, and C being a leaf its two particles are listed
+    # far from the flip on either side, for good measure
+    cid, rng_c, sp, ep = lists(0.36)
+    assert cid not in sp and rng_c in ep
+    cid, rng_c, sp, ep = lists(0.38)
+    assert cid in sp and rng_c not in ep
