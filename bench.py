@@ -221,9 +221,10 @@ def main():
     quad = params.multipole >= 2
     flop_sp = FLOP_QUAD if quad else FLOP_NEWTON
     flops_units = flop_sp * counts.n_epsp_common                      # phase A: k_force_units_tc + k_force_units (super-group-wide cells)
-    flops_groups = (FLOP_CUT * counts.n_epep_near + FLOP_NEWTON * (counts.n_epep - counts.n_epep_near)
-                    + flop_sp * (counts.n_epsp - counts.n_epsp_common))  # phase B: k_force (the groups' own lists)
-    flops_step = flops_units + flops_groups
+    flops_near = FLOP_CUT * counts.n_epep_near                        # k_force_near: the pairs inside the changeover radius
+    flops_groups = (FLOP_NEWTON * (counts.n_epep - counts.n_epep_near)
+                    + flop_sp * (counts.n_epsp - counts.n_epsp_common))  # phase B: k_force (the groups' own lists, Newtonian pairs + cells)
+    flops_step = flops_units + flops_near + flops_groups
 
     for _ in range(W):
         flush.fill_(1)
@@ -436,20 +437,6 @@ def main():
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(stream); fl = P.petar_probe_fp32(400000, scratch, stream); b.record(stream); b.synchronize()
     probe_tflops = fl / (a.elapsed_time(b) * 1e-3) / 1e12
-    # the other instruction streams of petar_probe_fp32_mode (include/petar.h): the scalar and the packed cell term on register
-    # operands, and the FFMA operand patterns of the register-bank issue model (profiles/fp32_issue_model_r02.md)
-    probes = {}
-    for mode, name, iters in ((1, "ffma_3_distinct_registers", 400000), (2, "quadrupole_cell_term_loop_scalar", 2000),
-                              (3, "quadrupole_cell_term_loop_packed", 2000), (4, "pattern_ffma_3_registers_independent", 200000),
-                              (5, "pattern_ffma_2_registers", 200000), (6, "pattern_ffma_shared_operand", 200000),
-                              (7, "pattern_ffma3_plus_fadd", 200000), (8, "tc_consumer_loop_alone", 20000),
-                              (9, "tc_consumer_loop_beside_mma", 20000)):
-        P.petar_probe_fp32_mode(mode, max(1, iters // 50), scratch, stream)
-        torch.cuda.synchronize()
-        a.record(stream); fl = P.petar_probe_fp32_mode(mode, iters, scratch, stream); b.record(stream); b.synchronize()
-        probes[name] = fl / (a.elapsed_time(b) * 1e-3) / 1e12
-        if mode >= 8:
-            probes[name + "_sm_mhz"] = float(scratch[1].item())      # SM clock during the loop (tensor-core activity lowers it)
     pk, pk_kind = peaks()
     sm_max = float(pk.get("sm_max_mhz", 1965.0))
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
@@ -476,17 +463,25 @@ def main():
         if ms_st > 0.0:
             gbs = bpp * N / (ms_st * 1e-3) / 1e9
             hbm_stages[name] = dict(ms=ms_st, bytes_per_particle=bpp, achieved_gbs=gbs, frac_of_hbm=gbs / hbm_peak)
-    # stage force_units = the unit table, k_force_units_tc (units of 80..128 particles: quadrupole contraction on the tensor cores) and
-    # k_force_units (smaller units, CUDA cores only); the 53 flops per quadrupole interaction are counted wherever they are executed
-    kern = [dict(kernel="k_force_units_tc" if quad else "k_force_units", ms=stage_ms["force_units"], flops_per_launch=float(flops_units)),
-            dict(kernel="k_force", ms=stage_ms["force"], flops_per_launch=float(flops_groups))]
-    kern[0]["ms_alone"], kern[1]["ms_alone"] = stage_seq["force_units"], stage_seq["force"]
+    # k_force (phase B): PETAR_STAGE_FORCE is an event pair around the single k_force launch, on the stream it is launched on, inside
+    # the timed region (nothing runs beside it: the side stream has been joined).  Phase A is a two-stream STAGE (unit table +
+    # k_force_units_tc on the caller's stream; k_walk, k_force_units, k_force_near beside them on the library's side stream) and is
+    # called a stage here; its kernels' time without the walk beside them is `ms_alone` (the sequential call order timed after the
+    # headline region).  The 53 flops per quadrupole interaction are counted wherever they are executed (tensor or CUDA cores).
+    phase_a = "stage force_units (unit table + k_force_units_tc | k_walk + k_force_units + k_force_near)" if quad else \
+              "stage force_units (unit table | k_walk + k_force_units + k_force_near)"
+    kern = [dict(kernel="k_force", timed="event pair around the single launch, in the timed region", ms=stage_ms["force"],
+                 ms_alone=stage_seq["force"], flops_per_launch=float(flops_groups)),
+            dict(kernel=phase_a, timed="event pair around a two-stream stage; ms_alone = the same kernels without k_walk beside them",
+                 ms=stage_ms["force_units"], ms_alone=stage_seq["force_units"], flops_per_launch=float(flops_units),
+                 note="k_force_near's changeover pairs (flops_k_force_near) are credited to neither entry: that kernel runs inside "
+                      "this stage in the timed region and outside every stage in the sequential order")]
     for kd in kern:
         kd["frac_alone"] = kd["flops_per_launch"] / (kd["ms_alone"] * 1e-3) / 1e12 / nominal_fp32 if kd["ms_alone"] > 0 else 0.0
         kd["achieved"] = kd["flops_per_launch"] / (kd["ms"] * 1e-3) / 1e12 if kd["ms"] > 0 else 0.0
         kd["frac"] = kd["achieved"] / nominal_fp32
         kd["share_of_step"] = kd["ms"] / ms_step
-    dom = max(kern, key=lambda kd: kd["ms"])                  # the dominant kernel of the step
+    dom = max(kern, key=lambda kd: kd["ms_alone"])            # the dominant kernel: by its own duration, not by an overlapped stage's
     force_ms = stage_ms["force_units"] + stage_ms["force"]
     achieved_both = flops_step / (force_ms * 1e-3) / 1e12
 
@@ -500,7 +495,8 @@ def main():
                     "step": "petar_tree_build + petar_long_range_force + petar_neighbor_list (count phase + fill phase)",
                     "l2": "256 MB buffer written between timed iterations (L2 flush), outside the per-step CUDA events",
                     "interactions_per_step": int(n_inter), "n_epep": int(counts.n_epep), "n_epsp": int(counts.n_epsp),
-                    "n_epep_changeover": int(counts.n_epep_near), "neighbours": nb_total, "n_groups": int(counts.n_groups),
+                    "n_epep_changeover": int(counts.n_epep_near), "n_epsp_common": int(counts.n_epsp_common),
+                    "n_refined": int(counts.n_refined), "neighbours": nb_total, "n_groups": int(counts.n_groups),
                     "n_nodes": int(counts.n_nodes), "status": status, "multi_gpu": "replicas only (no data-path collective)"},
             stage_ms=stage_ms,
             stage_ms_sequential=dict(stage_seq, step=seq_ms,
@@ -517,17 +513,13 @@ def main():
             clocks=clocks,
             roofline=dict(bound="alu", kernel=dom["kernel"], achieved=dom["achieved"], peak=nominal_fp32, unit="TFLOP/s",
                           frac=dom["frac"],
-                          traffic=TRAFFIC_NCU.get(dom["kernel"]) if (cfg == TRAFFIC_NCU["config"] and args.N is None) else None,
+                          traffic=TRAFFIC_NCU.get(dom["kernel"].split()[0]) if (cfg == TRAFFIC_NCU["config"] and args.N is None) else None,
                           traffic_source=TRAFFIC_NCU["capture"],
                           peak_kind=f"nominal CUDA-core FP32: 2 x 128 lanes x {n_sm} SMs x {sm_max:.0f} MHz (sm_max_mhz of MEASURED_PEAKS.json, {pk_kind})",
                           peak_measured_ffma_probe=probe_tflops, frac_of_probe=dom["achieved"] / probe_tflops,
-                          probes_tflops=probes,
-                          probes_note="cell-term probes: TFLOP/s at 53 flops per interaction; pattern probes: 2 x thread instructions per "
-                                      "second, i.e. value / peak = warp instructions per clock and sub-partition",
-                          frac_of_cell_term_probe=dom["achieved"] / probes["quadrupole_cell_term_loop_packed"],
                           flops_convention=f"{FLOP_NEWTON}/{FLOP_CUT}/{FLOP_QUAD} flops per Newtonian / changeover / quadrupole interaction",
                           flops_per_launch=dom["flops_per_launch"], kernel_ms=dom["ms"], kernel_share_of_step=dom["share_of_step"],
-                          force_kernels=kern, both_force_kernels=dict(ms=force_ms, achieved=achieved_both, frac=achieved_both / nominal_fp32,
+                          flops_k_force_near=float(flops_near), force_kernels=kern, both_force_kernels=dict(ms=force_ms, achieved=achieved_both, frac=achieved_both / nominal_fp32,
                                                                       share_of_step=force_ms / ms_step),
                           hbm_peak_gbs=pk.get("hbm_gbs")),
             wall_s_timed_region=t_wall,

@@ -326,9 +326,12 @@ int petar_debug_export(petar_tree* t, int what, void* dst, size_t dst_bytes, voi
 #define PETAR_STAGE_WALK 6
 #define PETAR_STAGE_FORCE 7
 #define PETAR_STAGE_NEIGHBOR 8
-#define PETAR_STAGE_FORCE_UNITS 9   /* force phase A (k_force_units); PETAR_STAGE_FORCE is phase B (k_force) */
+#define PETAR_STAGE_FORCE_UNITS 9   /* force phase A: a two-stream STAGE (unit table + k_force_units_tc on the caller's stream;
+                                       on a first force call also k_walk, k_force_units, k_force_near on the side stream).
+                                       PETAR_STAGE_FORCE is phase B: the event pair spans the single k_force launch          */
 #define PETAR_STAGE_WALK_SUPER 10   /* super-group walks; PETAR_STAGE_WALK is the per-group walk (k_walk)   */
-#define PETAR_N_STAGES 11
+#define PETAR_STAGE_FORCE_REFINE 11 /* k_force_refine: fp64 re-evaluation of the n_refined near-cancelling particles  */
+#define PETAR_N_STAGES 12
 int petar_set_profiling(int on);
 int petar_stage_times(petar_tree* t, float* stage_ms /* HOST */);
 /* Number of kernel launches the library has enqueued since process start (HOST counter).           */
@@ -339,27 +342,6 @@ int64_t petar_launch_count(void);
  * the caller times it with CUDA events to obtain this GPU's CUDA-core FP32 peak.
  * scratch_dev: DEVICE float[1].                                                                      */
 int petar_probe_fp32(int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream);
-/* The same with a choice of instruction stream ("operand bandwidth"):
- *   mode 0: FFMA whose two other operands are the same for every chain (as petar_probe_fp32);
- *   mode 1: FFMA with three distinct register operands per instruction;
- *   mode 2: the quadrupole cell term (rule O8) with SCALAR fp32 instructions on register operands, 4 i-particles
- *           per thread, cells broadcast from shared memory -- *flops_out_host then counts 53 flops per
- *           interaction (the convention of bench.py): the rate of the round-1 instruction mix;
- *   mode 3: the same term with the PACKED fp32x2 instructions the force kernels use (two packed pairs per thread):
- *           the rate attainable by the kernels' instruction mix with no list, staging or tail cost;
- *   modes 4-7: FFMA operand patterns behind profiles/fp32_issue_model_r02.md -- 4: a = b*c + a (three distinct
- *           registers), 5: a = b*b + a (two), 6: a = b*e + a; c = d*e + c (one operand shared by all), 7: a = b*c + d;
- *           d = a + e.  *flops_out_host = 2 x thread-level instructions, so value / time / (nominal FP32 peak) is
- *           warp instructions per clock and sub-partition;
- *   modes 8, 9: the consumer loop of the tensor-core phase-A kernel (k_force_units_tc: tcgen05.ld of d.B.d and B d, 21 packed
- *           FP32 + 2 MUFU per cell pair) on static operands, iters = 32-cell tiles per CTA, 53 flops per interaction --
- *           8: alone, 9: with the kernel's MMAs (4 x 128x128x8 tf32 per tile) issued beside it through the kernel's
- *           full / empty mbarrier handshake.  Their difference is the cost of the tensor-core work to the CUDA-core loop.
- *           Modes 8 and 9 need scratch_dev = DEVICE float[2] and leave the SM clock measured during the loop (clock64 against
- *           %globaltimer, MHz) in scratch_dev[1]: the chip lowers the SM clock while tcgen05.mma instructions are in flight.
- * Errors: PETAR_EINVAL (mode), PETAR_ECUDA.                                                          */
-int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream);
-
 #ifdef __cplusplus
 }
 #endif

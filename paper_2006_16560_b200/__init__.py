@@ -11,7 +11,7 @@ from .binding import (  # noqa: F401
     lib, library_path, exported_symbols,
     petar_workspace_bytes, petar_tree_build, petar_tree_rebuild, petar_long_range_force, petar_neighbor_list,
     petar_tree_status, petar_tree_destroy, petar_strerror, petar_debug_export,
-    petar_set_profiling, petar_stage_times, petar_launch_count, petar_probe_fp32, petar_probe_fp32_mode,
+    petar_set_profiling, petar_stage_times, petar_launch_count, petar_probe_fp32,
     petar_search_radii, petar_neighbor_list_orbit, petar_clusters_workspace_bytes, petar_clusters,
     petar_short_range_workspace_bytes, petar_short_range_force, petar_short_range_force_noalloc, SHORT_RANGE_NOALLOC_MAX_N,
     petar_kick, petar_artificial_particles, petar_tidal_tensor_fit, petar_orbit_sampling, art_count,

@@ -11,12 +11,12 @@ _LIB = None
 EXPORTS = [
     "petar_workspace_bytes", "petar_tree_build", "petar_tree_rebuild", "petar_long_range_force", "petar_neighbor_list",
     "petar_tree_status", "petar_tree_destroy", "petar_strerror", "petar_debug_export",
-    "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32", "petar_probe_fp32_mode",
+    "petar_set_profiling", "petar_stage_times", "petar_launch_count", "petar_probe_fp32",
     "petar_search_radii", "petar_neighbor_list_orbit", "petar_clusters_workspace_bytes", "petar_clusters",
     "petar_short_range_workspace_bytes", "petar_short_range_force", "petar_short_range_force_noalloc",
     "petar_kick", "petar_artificial_particles", "petar_tidal_tensor_fit", "petar_orbit_sampling",
 ]
-STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units", "walk_super"]
+STAGE_NAMES = ["bbox_keys", "sort", "gather", "tree", "moments", "groups", "walk", "force", "neighbor", "force_units", "walk_super", "force_refine"]
 DBG = dict(HEADER=0, ROOT=1, KEYS=2, PERM=3, NODE_INT=4, NODE_DBL=5, GROUP_INT=6, GROUP_DBL=7, GROUP_CNT=8,
            LIST_OFFS=9, LISTS=10, GROUP_SUPER=11)
 
@@ -114,8 +114,6 @@ def lib():
         L.petar_launch_count.restype = C.c_int64
         L.petar_probe_fp32.restype = C.c_int
         L.petar_probe_fp32.argtypes = [C.c_int64, C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
-        L.petar_probe_fp32_mode.restype = C.c_int
-        L.petar_probe_fp32_mode.argtypes = [C.c_int32, C.c_int64, C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
         _LIB = L
     return _LIB
 
@@ -304,15 +302,6 @@ def petar_probe_fp32(iters: int, scratch, stream=None) -> float:
     rc = lib().petar_probe_fp32(C.c_int64(iters), C.byref(fl), _ptr(scratch), _stream(stream))
     if rc:
         raise PetarError(rc, "petar_probe_fp32")
-    return float(fl.value)
-
-
-def petar_probe_fp32_mode(mode: int, iters: int, scratch, stream=None) -> float:
-    """Probe kernel of the given mode (see petar.h); returns the flops it executes (time it with CUDA events)."""
-    fl = C.c_double(0.0)
-    rc = lib().petar_probe_fp32_mode(C.c_int32(mode), C.c_int64(iters), C.byref(fl), _ptr(scratch), _stream(stream))
-    if rc:
-        raise PetarError(rc, "petar_probe_fp32_mode")
     return float(fl.value)
 
 

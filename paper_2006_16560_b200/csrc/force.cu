@@ -1423,6 +1423,8 @@ cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* a
     else
         k_force<false><<<grid, FT, 0, s>>>(w.hdr, w.grp, w.arena, w.nsp, w.pa, w.pb, w.idx, w.part, w.part_s, (long long)t->N, w.refine_q, ax, ay, az, pot, fc, t->p.G);
     KCHECK(s, "k_force");
+    stage_end(t, PETAR_STAGE_FORCE, s);                     // the event pair of this stage spans the single k_force launch
+    stage_begin(t, PETAR_STAGE_FORCE_REFINE, s);
     {
         const double* rs = w.routs;
         RefineArgs A = {w.grp, w.srec, w.group_cap, w.arena, w.nmac, w.nmom, w.xs, w.ys, w.zs, w.ms, rs, w.idx, w.refine_q,
@@ -1431,7 +1433,7 @@ cudaError_t launch_force_groups(petar_tree* t, double* ax, double* ay, double* a
         KCHECK(s, "k_force_refine");
     }
     petar_count_launch(2);
-    stage_end(t, PETAR_STAGE_FORCE, s);
+    stage_end(t, PETAR_STAGE_FORCE_REFINE, s);
     return cudaGetLastError();
 }
 
@@ -1458,250 +1460,6 @@ __global__ void __launch_bounds__(256) k_probe_fp32(float* __restrict__ out, lon
 #pragma unroll
     for (int k = 0; k < 16; ++k) s += v[k];
     if (s == 123.456f) out[0] = s;      // never true in practice; keeps the chains alive
-}
-
-// mode 1: FFMA with three distinct register operands per instruction
-__global__ void __launch_bounds__(256) k_probe_ffma3(float* __restrict__ out, long long iters) {
-    float a[8], b[8], c[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) { a[k] = (float)(threadIdx.x + k) * 1e-3f; b[k] = 1.0f + 1e-6f * (float)(threadIdx.x + k); c[k] = 1e-3f * (float)(k + 1); }
-    for (long long it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int k = 0; k < 8; ++k) { a[k] = fmaf(b[k], c[k], a[k]); c[k] = fmaf(a[k], b[k], c[k]); }
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) s += a[k] + b[k] + c[k];
-    if (s == 123.456f) out[0] = s;
-}
-// mode 2: the quadrupole cell term of the force kernels on register operands (4 i-particles per thread)
-__global__ void __launch_bounds__(128, 4) k_probe_cell(float* __restrict__ out, long long iters) {
-    __shared__ float4 q0[64], q1[64];
-    __shared__ float2 q2[64];
-    const int t = threadIdx.x;
-    if (t < 64) {
-        q0[t] = make_float4(10.f + t, 20.f - t, 30.f + 0.5f * t, 1.f + 0.01f * t);
-        q1[t] = make_float4(1e-3f * t, -2e-3f * t, 1e-3f * t, 3e-4f * t);
-        q2[t] = make_float2(-1e-4f * t, 2e-4f * t);
-    }
-    __syncthreads();
-    float ix[4], iy[4], iz[4];
-    Acc32 p[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) { ix[k] = t * 0.01f + k + out[0]; iy[k] = t * 0.02f - k; iz[k] = 0.5f * k + out[0]; p[k].ax = p[k].ay = p[k].az = p[k].pot = 0.f; }
-    for (long long it = 0; it < iters; ++it) {
-#pragma unroll 1
-        for (int j = 0; j < 64; ++j) {
-            const float4 a = q0[j], b = q1[j]; const float2 c = q2[j];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) cell_term<true>(p[k], a.x - ix[k], a.y - iy[k], a.z - iz[k], a.w, b.x, b.y, b.z, b.w, c.x, c.y);
-        }
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) s += p[k].ax + p[k].ay + p[k].az + p[k].pot;
-    if (s == 123.456f) out[0] = s;
-}
-
-// mode 3: the PACKED quadrupole cell term of the force kernels (two packed pairs = 4 i-particles per thread, cells broadcast
-// from shared memory as scalars): the rate attainable by the kernels' own instruction mix
-__global__ void __launch_bounds__(128, 4) k_probe_cell2(float* __restrict__ out, long long iters) {
-    __shared__ float4 q0[64], q1[64];
-    __shared__ float2 q2[64];
-    const int t = threadIdx.x;
-    if (t < 64) {
-        q0[t] = make_float4(10.f + t, 20.f - t, 30.f + 0.5f * t, 1.f + 0.01f * t);
-        q1[t] = make_float4(1e-3f * t, -2e-3f * t, 1e-3f * t, 3e-4f * t);
-        q2[t] = make_float2(-1e-4f * t, 2e-4f * t);
-    }
-    __syncthreads();
-    f2 nx[2], ny[2], nz[2];
-    Acc2 p[2];
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-        nx[k] = make_float2(-(t * 0.01f + 2 * k + out[0]), -(t * 0.01f + 2 * k + 1 + out[0]));
-        ny[k] = make_float2(-(t * 0.02f - 2 * k), -(t * 0.02f - 2 * k - 1));
-        nz[k] = make_float2(-(0.5f * k + out[0]), -(0.5f * k + 0.25f + out[0]));
-        p[k].ax = p[k].ay = p[k].az = p[k].pot = make_float2(0.f, 0.f);
-    }
-    for (long long it = 0; it < iters; ++it) {
-#pragma unroll 1
-        for (int j = 0; j < 64; ++j) {
-            const float4 a = q0[j], b = q1[j]; const float2 c = q2[j];
-#pragma unroll
-            for (int k = 0; k < 2; ++k) cell_term2<true>(p[k], add2(bc(a.x), nx[k]), add2(bc(a.y), ny[k]), add2(bc(a.z), nz[k]), a.w, b.x, b.y, b.z, b.w, c.x, c.y);
-        }
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int k = 0; k < 2; ++k) s += p[k].ax.x + p[k].ay.x + p[k].az.x + p[k].pot.x + p[k].ax.y + p[k].ay.y + p[k].az.y + p[k].pot.y;
-    if (s == 123.456f) out[0] = s;
-}
-// modes 4-7: operand patterns that separate the register-bank model from a plain "operands per clock" model
-// (profiles/fp32_issue_model_r02.md).  8 chains per thread, 4 warps per sub-partition.
-template <int PAT>
-__global__ void __launch_bounds__(128) k_probe_pattern(float* __restrict__ out, long long iters, float s0, float s1) {
-    float a[8], b[8], c[8], d[8];
-#pragma unroll
-    // every operand depends on the thread index: a warp-uniform value would be kept in a uniform register, which costs no register-file read
-    for (int i = 0; i < 8; ++i) { a[i] = threadIdx.x * 1e-3f + i; b[i] = 1.0f + 1e-6f * (threadIdx.x + i); c[i] = 1e-3f * (i + 1) + s1 * threadIdx.x; d[i] = 0.5f * i + s0 * threadIdx.x; }
-    const float e = s0 * threadIdx.x + 0.25f;
-    for (long long it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            if (PAT == 4) a[i] = fmaf(b[i], c[i], a[i]);                                    // three distinct registers, independent chains
-            if (PAT == 5) a[i] = fmaf(b[i], b[i], a[i]);                                    // two distinct registers
-            if (PAT == 6) { a[i] = fmaf(b[i], e, a[i]); c[i] = fmaf(d[i], e, c[i]); }       // one operand shared by every instruction
-            if (PAT == 7) { a[i] = fmaf(b[i], c[i], d[i]); d[i] = a[i] + e; }               // FFMA (3 registers) + FADD (2 registers)
-        }
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) s += a[i] + b[i] + c[i] + d[i];
-    if (s == 123.456f) out[0] = s;
-}
-
-// modes 8, 9: the consumer loop of k_force_units_tc (tcgen05.ld of the four numbers per cell, broadcast (c, M) pairs from shared
-// memory, 21 packed FP32 + 2 MUFU per cell pair) on static operands, 2 CTAs of 4 consumer warps per SM.  Mode 8: nothing else runs;
-// mode 9: a fifth warp issues the kernel's MMAs (4 x 128x128x8 tf32 per 32-cell tile) into the other TMEM buffer, with the
-// kernel's full / empty mbarrier handshake -- the difference is what the tensor-core work beside the CUDA-core loop costs.
-template <bool MMA>
-__global__ void __launch_bounds__(160, 3) k_probe_tc(float* __restrict__ out, long long iters) {
-    __shared__ __align__(128) float sA[128 * TC_K];
-    __shared__ __align__(128) float sB[TC_STAGE_BYTES / 4];
-    __shared__ __align__(16) float4 sC[2][TC_CELLS / 2][2];
-    __shared__ __align__(8) unsigned long long full[2], empty[2];
-    __shared__ uint32_t tmem_base;
-    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
-    for (int e = t; e < 128 * TC_K; e += 160) sA[e] = 1e-3f * (float)(e & 63);
-    for (int e = t; e < TC_STAGE_BYTES / 4; e += 160) sB[e] = 2e-3f * (float)(e & 31);
-    if (t < 2 * TC_CELLS) reinterpret_cast<float4*>(sC)[t] = make_float4(10.f + t, 10.5f + t, 20.f - t, 20.5f - t);
-    if (t == 0) {
-        for (int q = 0; q < 2; ++q) {
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&full[q])));
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 4;" :: "r"(smem_u32(&empty[q])));
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;");
-    }
-    if (w == 4) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base)), "n"(2 * TC_N));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-    }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    asm volatile("tcgen05.fence::before_thread_sync;");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;");
-    const uint32_t tmem = tmem_base;
-    if (w == 4) {
-        if (MMA) {
-            const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-            const uint64_t da0 = tc_desc(smem_u32(sA), TC_SBO), db0 = tc_desc(smem_u32(sB), TC_SBO_B);
-            for (long long k = 0; k < iters; ++k) {
-                const int b = (int)(k & 1);
-                mbar_wait(smem_u32(&empty[b]), (uint32_t)(((k >> 1) & 1) ^ 1));
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                if (lane == 0) {
-#pragma unroll
-                    for (int ks = 0; ks < TC_K / 8; ++ks) {
-                        const uint32_t accf = ks > 0;
-                        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-                                     :: "r"(tmem + (uint32_t)b * TC_N), "l"(da0 + (uint64_t)(ks * ((2 * TC_LBO) >> 4))), "l"(db0 + (uint64_t)(ks * ((2 * TC_LBO) >> 4))), "r"(idesc), "r"(accf) : "memory");
-                    }
-                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&full[b])) : "memory");
-                }
-                __syncwarp();
-            }
-        }
-    } else {
-        const uint32_t tl = tmem + ((uint32_t)(w * 32) << 16);
-        if (!MMA) {         // some finite numbers in tensor memory
-            for (int c = 0; c < 2 * TC_N; c += 4) {
-                const uint32_t a = __float_as_uint(1e-3f * (float)(t + c)), b = __float_as_uint(-2e-3f * (float)(c + 1));
-                asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" :: "r"(tl + c), "r"(a), "r"(b), "r"(a), "r"(b));
-            }
-            asm volatile("tcgen05.wait::st.sync.aligned;");
-        }
-        const float nx = -(t * 0.01f + out[0]), ny = -(t * 0.02f), nz = -(0.5f + out[0]);
-        Acc2 p = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
-        const long long c0 = clock64();
-        unsigned long long g0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
-        for (long long k = 0; k < iters; ++k) {
-            const int b = (int)(k & 1);
-            if (MMA) { mbar_wait(smem_u32(&full[b]), (uint32_t)((k >> 1) & 1)); asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-            uint32_t va[16], vb[16];
-            float4 ca[4], cb[4];
-            const uint32_t tcol = tl + (uint32_t)b * TC_N;
-            const float4* cp2 = &sC[b][0][0];
-            tc_ld16(va, tcol);
-#pragma unroll
-            for (int q = 0; q < 4; ++q) ca[q] = cp2[q];
-#pragma unroll
-            for (int hh = 0; hh < TC_N / 16; hh += 2) {
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                tc_ld16(vb, tcol + (hh + 1) * 16);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) cb[q] = cp2[(hh + 1) * 4 + q];
-                tc_pairs(p, va, ca, nx, ny, nz);
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                if (hh + 2 < TC_N / 16) {
-                    tc_ld16(va, tcol + (hh + 2) * 16);
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) ca[q] = cp2[(hh + 2) * 4 + q];
-                }
-                tc_pairs(p, vb, cb, nx, ny, nz);
-            }
-            if (MMA) {
-                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(&empty[b])) : "memory");
-            }
-        }
-        const float s = p.ax.x + p.ay.x + p.az.x + p.pot.x + p.ax.y + p.ay.y + p.az.y + p.pot.y;
-        if (s == 123.456f) out[0] = s;
-        if (t == 0 && blockIdx.x == 0) {       // SM clock during the loop: cycles per nanosecond of the global timer, in MHz
-            const long long c1 = clock64();
-            unsigned long long g1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
-            out[1] = (float)(1.0e3 * (double)(c1 - c0) / (double)(g1 - g0));
-        }
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;");
-    __syncthreads();
-    if (w == 4) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "n"(2 * TC_N));
-}
-
-extern "C" int petar_probe_fp32_mode(int32_t mode, int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream) {
-    if (mode == 0) return petar_probe_fp32(iters, flops_out_host, scratch_dev, cuda_stream);
-    if (mode < 1 || mode > 9) return PETAR_EINVAL;
-    int dev = 0, sm = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return PETAR_ECUDA;
-    if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PETAR_ECUDA;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    if (mode == 1) {
-        const int grid = sm * 8;
-        k_probe_ffma3<<<grid, 256, 0, s>>>(scratch_dev, (long long)iters);
-        if (flops_out_host) *flops_out_host = 2.0 * 16.0 * (double)iters * 256.0 * (double)grid;
-    } else if (mode == 8 || mode == 9) {
-        const int grid = sm * 2;
-        if (mode == 8) k_probe_tc<false><<<grid, 160, 0, s>>>(scratch_dev, (long long)iters);
-        else k_probe_tc<true><<<grid, 160, 0, s>>>(scratch_dev, (long long)iters);
-        if (flops_out_host) *flops_out_host = 53.0 * (double)TC_CELLS * 128.0 * (double)iters * (double)grid;
-    } else if (mode == 2 || mode == 3) {
-        const int grid = sm * 4;
-        if (mode == 2) k_probe_cell<<<grid, 128, 0, s>>>(scratch_dev, (long long)iters);
-        else k_probe_cell2<<<grid, 128, 0, s>>>(scratch_dev, (long long)iters);
-        if (flops_out_host) *flops_out_host = 53.0 * 4.0 * 64.0 * (double)iters * 128.0 * (double)grid;
-    } else {
-        const int grid = sm * 4;        // 4 CTAs x 4 warps per SM: 4 warps per sub-partition
-        const double per = (mode == 6 || mode == 7) ? 2.0 : 1.0;       // instructions per chain and iteration
-        if (mode == 4) k_probe_pattern<4><<<grid, 128, 0, s>>>(scratch_dev, (long long)iters, 0.999f, 1e-3f);
-        if (mode == 5) k_probe_pattern<5><<<grid, 128, 0, s>>>(scratch_dev, (long long)iters, 0.999f, 1e-3f);
-        if (mode == 6) k_probe_pattern<6><<<grid, 128, 0, s>>>(scratch_dev, (long long)iters, 0.999f, 1e-3f);
-        if (mode == 7) k_probe_pattern<7><<<grid, 128, 0, s>>>(scratch_dev, (long long)iters, 0.999f, 1e-3f);
-        // *flops_out_host = thread-level INSTRUCTIONS x 2 (so that value / time / nominal peak = warp instructions per clock and sub-partition)
-        if (flops_out_host) *flops_out_host = 2.0 * 8.0 * per * (double)iters * 128.0 * (double)grid;
-    }
-    petar_count_launch(1);
-    return cudaGetLastError() == cudaSuccess ? PETAR_OK : PETAR_ECUDA;
 }
 
 extern "C" int petar_probe_fp32(int64_t iters, double* flops_out_host, float* scratch_dev, void* cuda_stream) {
