@@ -34,7 +34,7 @@ sys.path.insert(0, ROOT)
 FLOP_NEWTON, FLOP_CUT, FLOP_QUAD = 20, 49, 53      # fixed flops-per-interaction convention
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the force kernels, from the committed `ncu --set full` capture of
 # THIS round's build at config 3 (profiles/ncu_r02_force.md).  Emitted only for that configuration; any other run reports null.
-TRAFFIC_NCU = {"capture": "profiles/ncu_r02_force.md", "config": 3, "k_force_units_tc": 132.8e6, "k_force_units": 132.8e6, "k_force": 1231.3e6}
+TRAFFIC_NCU = {"capture": "profiles/ncu_r03_force.md", "config": 3, "k_force_units_tc": 131.9e6, "k_force_units": 44.6e6, "k_force": 1231.2e6, "stage": 176.5e6}
 
 
 def parse():

@@ -47,6 +47,7 @@ __global__ void k_reset_header(DevHeader* h) {
         h->group_ticket = 0; h->group_ticket2 = 0; h->group_ticket3 = 0; for (int l = 0; l < PETAR_NSUP; ++l) { h->n_super[l] = 0; h->super_ticket[l] = 0; }
         h->n_epep = h->n_epsp = h->n_epep_near = h->n_ep_list = h->n_sp_list = h->n_epsp_common = 0ull; h->nb_total = 0ull;
         for (int l = 0; l < PETAR_NLEVELS + 2; ++l) h->level_off[l] = 0;
+        h->rank_done = 0;
     }
 }
 
@@ -370,42 +371,53 @@ __global__ void __launch_bounds__(RANK_THREADS) k_rank_count(const signed char* 
     if (threadIdx.x < PETAR_NLEVELS) tile_cnt[threadIdx.x * ntile + blockIdx.x] = cnt[threadIdx.x];
 }
 
-// single CTA: per level exclusive scan over tiles; level offsets; node count and capacity check
+// One CTA per tree level: exclusive scan of the level's per-tile node counts, in place (warp shuffles, two barriers per
+// 1024 tiles).  Each CTA leaves its level's total in level_off[l]; the last CTA to finish turns the totals into the level
+// offsets, sets the node count and checks the capacity.  (A single CTA doing the 22 levels one after the other took 0.36 ms
+// at N = 10^7.)
 __global__ void __launch_bounds__(1024) k_rank_scan(int* __restrict__ tile_cnt, int ntile, DevHeader* __restrict__ h, int node_cap) {
-    __shared__ int buf[1024];
-    __shared__ int carry_s;
-    __shared__ int tot[PETAR_NLEVELS];
-    const int t = threadIdx.x;
-    for (int l = 0; l < PETAR_NLEVELS; ++l) {
-        if (t == 0) carry_s = 0;
+    __shared__ int wsum[32];
+    __shared__ int carry_s, last_s;
+    const int t = threadIdx.x, lane = t & 31, wp = t >> 5, l = blockIdx.x;
+    int* row = tile_cnt + (size_t)l * ntile;
+    if (t == 0) carry_s = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < ntile; b0 += 1024) {
+        const int b = b0 + t;
+        const int v = (b < ntile) ? row[b] : 0;
+        int incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int a = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += a; }
+        if (lane == 31) wsum[wp] = incl;
         __syncthreads();
-        int* row = tile_cnt + (size_t)l * ntile;
-        for (int b0 = 0; b0 < ntile; b0 += 1024) {
-            int b = b0 + t;
-            int v = (b < ntile) ? row[b] : 0;
-            buf[t] = v;
-            __syncthreads();
-            for (int o = 1; o < 1024; o <<= 1) {
-                int a = (t >= o) ? buf[t - o] : 0;
-                __syncthreads();
-                buf[t] += a;
-                __syncthreads();
-            }
-            int incl = buf[t], carry = carry_s;
-            if (b < ntile) row[b] = carry + incl - v;
-            __syncthreads();
-            if (t == 1023) carry_s = carry + incl;
-            __syncthreads();
+        if (wp == 0) {
+            const int sv = wsum[lane];
+            int si = sv;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int a = __shfl_up_sync(0xffffffffu, si, o); if (lane >= o) si += a; }
+            wsum[lane] = si - sv;                       // tiles of the warps before this one
         }
-        if (t == 0) tot[l] = carry_s;
+        __syncthreads();
+        const int excl = carry_s + wsum[wp] + incl - v;
+        if (b < ntile) row[b] = excl;
+        __syncthreads();                                // carry_s and wsum read by everybody
+        if (t == 1023) carry_s = excl + v;
         __syncthreads();
     }
     if (t == 0) {
+        ((volatile int*)h->level_off)[l] = carry_s;     // this level's total, for now
+        __threadfence();
+        last_s = atomicAdd(&h->rank_done, 1) == (int)gridDim.x - 1;
+    }
+    __syncthreads();
+    if (last_s && t == 0) {
+        __threadfence();
         int run = 0;
-        for (int l = 0; l < PETAR_NLEVELS; ++l) { h->level_off[l] = run; run += tot[l]; }
+        for (int k = 0; k < PETAR_NLEVELS; ++k) { const int c = ((volatile int*)h->level_off)[k]; h->level_off[k] = run; run += c; }
         h->level_off[PETAR_NLEVELS] = run; h->level_off[PETAR_NLEVELS + 1] = run;
         h->n_nodes = run;
         if (run > node_cap) { atomicOr(&h->status, PETAR_ST_NODE_CAP); }
+        h->rank_done = 0;
     }
 }
 
@@ -800,7 +812,7 @@ cudaError_t launch_tree(petar_tree* t, cudaStream_t s) {
     KCHECK(s, "k_depth");
     k_rank_count<<<ntile, RANK_THREADS, 0, s>>>(w.D, w.depth, n, w.tile_cnt, ntile);
     KCHECK(s, "k_rank_count");
-    k_rank_scan<<<1, 1024, 0, s>>>(w.tile_cnt, ntile, w.hdr, w.node_cap);
+    k_rank_scan<<<PETAR_NLEVELS, 1024, 0, s>>>(w.tile_cnt, ntile, w.hdr, w.node_cap);
     KCHECK(s, "k_rank_scan");
     k_nodes_write<<<ntile, RANK_THREADS, 0, s>>>(w.key, w.D, w.depth, n, w.tile_cnt, ntile, w.hdr, w.nint, w.node_cap);
     KCHECK(s, "k_nodes_write");

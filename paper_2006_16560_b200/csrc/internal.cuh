@@ -46,6 +46,7 @@ struct DevHeader {
     int unit_ticket_tc;            // k_force_units_tc (class-0 units)
     int n_refine;                  // particles queued for the fp64 re-evaluation (k_force_refine)
     int group_ticket4;             // k_force_near
+    int rank_done;                 // k_rank_scan: CTAs (one per level) that have finished; the last one writes level_off and resets it
     unsigned long long n_epep, n_epsp, n_epep_near, n_ep_list, n_sp_list, n_epsp_common;
     unsigned long long nb_total;
 };
