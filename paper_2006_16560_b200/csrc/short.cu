@@ -12,10 +12,10 @@
 #include "internal.cuh"
 #include <mutex>
 
-// multiprocessors of the current device (queried once)
+// multiprocessors of the CURRENT device (asked on every call: a process may drive several GPUs, and the query is a host-side lookup)
 static int sm_count() {
-    static int n = 0;
-    if (n == 0) { int dev = 0; if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148; }
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
     return n;
 }
 

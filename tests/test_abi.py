@@ -60,6 +60,22 @@ def test_error_strings_and_null_handles():
     assert L.petar_tree_build(None, None, None, None, None, None, 10, C.byref(p), None, 0, None, None) == -1
 
 
+def test_noalloc_entry_point_host_checks():
+    """petar_short_range_force_noalloc refuses a size beyond its built-in array, and bad arguments, before it touches the
+    GPU (so this runs without one); the error text names the limit."""
+    L = P.lib()
+    nul = [None] * 10
+    out = [None] * 7
+    big = P.SHORT_RANGE_NOALLOC_MAX_N + 1
+    call = lambda n, rho: L.petar_short_range_force_noalloc(*nul, C.c_int64(n), C.c_double(1.0), C.c_double(rho), *out, None)
+    assert call(big, 0.1) == -6                      # PETAR_ECAPACITY
+    assert call(-1, 0.1) == -1 and call(10, 1.5) == -1 and call(10, 0.1) == -1      # N < 0, bad ratio, NULL arrays
+    assert call(0, 0.1) == 0                          # nothing to do
+    assert "PETAR_SHORT_RANGE_NOALLOC_MAX_N" in P.petar_strerror(-6)
+    hdr = open(os.path.join(ROOT, "include", "petar.h")).read()
+    assert f"#define PETAR_SHORT_RANGE_NOALLOC_MAX_N {P.SHORT_RANGE_NOALLOC_MAX_N}" in hdr
+
+
 def test_product_does_not_import_oracle():
     """The product path must not route through the oracle (or anything under _work/)."""
     pkg = os.path.join(ROOT, "paper_2006_16560_b200")

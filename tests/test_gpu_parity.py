@@ -457,18 +457,19 @@ def test_full_size(cfg):
 
 def test_config5_capacity():
     """Config 5 (N = 10,485,760, everything resident in HBM): structures bit-exact over the whole system;
-    lists, counts, forces and neighbour rows on sampled i-groups the oracle can compute one by one."""
+    forces on 2000 sampled i-groups (~37 000 particles), list membership on 100 and neighbour rows on 300 of them --
+    what the oracle can compute group by group in a few seconds."""
     w = make_workload(5)
     t, T = _gpu_tree(w), _ora_tree(w)
     check_structures(t, T, w)
     counts = t.force(want_counts=True)
     assert _P().petar_tree_status(t.handle) == 0
     rng = np.random.default_rng(5)
-    sel = np.sort(rng.choice(T.n_groups, size=60, replace=False))
+    sel = np.sort(rng.choice(T.n_groups, size=2000, replace=False))
     gc = _np(t.export("GROUP_CNT")).reshape(-1, 4)
     offs, lists = t.export("LISTS")
     offs, lists = _np(offs), _np(lists)
-    for g in sel[:20]:
+    for g in sel[::20]:
         sp, ep = T.walk_lists(int(g))
         assert gc[g, 0] == len(sp) and gc[g, 1] + gc[g, 2] <= len(ep) and gc[g, 3] == int((ep[:, 1] - ep[:, 0]).sum())
         assert np.array_equal(np.sort(lists[offs[3 * g]:offs[3 * g + 1]]), np.sort(sp))
@@ -478,9 +479,12 @@ def test_config5_capacity():
     a = T.force(sel)
     g4 = [_np(v) for v in (t.acc_x, t.acc_y, t.acc_z, t.pot)]
     ea, ep_ = _rel_err(g4, a)
-    assert ea.size > 500 and ea.max() < TOL and ep_.max() < TOL, (ea.max(), ep_.max())
+    print(f"\nconfig 5: {ea.size} particles of {sel.size} sampled groups compared, n_refined = {counts.n_refined}; acceleration error max "
+          f"{ea.max():.3e}, 99.9th percentile {np.quantile(ea, 0.999):.3e}, median {np.median(ea):.3e}; potential error max {ep_.max():.3e}")
+    assert ea.size > 20000 and ea.max() < TOL and ep_.max() < TOL, (ea.max(), ep_.max())
     off, idx = t.neighbors()
     off, idx = _np(off), _np(idx)
+    sel = sel[::7]
     ooff, oidx = T.neighbors(sel)
     key, perm = T.keys()
     gb, ge, *_ = T.groups()
@@ -490,7 +494,7 @@ def test_config5_capacity():
             row = np.sort(idx[off[o]:off[o + 1]])
             assert np.array_equal(row, oidx[ooff[o]:ooff[o + 1]])
             n_checked += len(row)
-    assert n_checked > 50
+    assert n_checked > 300
     # properties that hold at any size
     assert all(np.all(np.isfinite(v)) for v in g4) and np.all(g4[3] < 0)
     assert counts.n_epep + counts.n_epsp > 5e10
